@@ -1,0 +1,179 @@
+/* hyb.h -- C-ABI of the B200-native hybrid tree force evaluation
+ * (Watanabe & Nakasato, "GPU accelerated Hybrid Tree Algorithm for Collision-less N-body
+ * Simulations", arXiv:1406.6158; citations are PAPER.md line numbers).
+ *
+ * One CUDA device, one stream.  The caller (PyTorch in this repository) owns all particle
+ * memory and the scratch workspace; the library only launches kernels on the caller's stream.
+ * No torch types, no C++ types, no exceptions cross this boundary; nothing is printed.
+ *
+ * Every function returns HYB_OK (0) or a negative HYB_ERR_* code; hyb_last_error() gives a
+ * short message for the last failure on that context.
+ *
+ * The canonical computation (what every stage must produce, bit for bit where it is integer)
+ * is the "T-spec" restated in DESIGN.md section 3 from SURVEY.md 8(c).
+ */
+#ifndef HYB_H
+#define HYB_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+/* (x, y, z, w) -- 16-byte aligned.  Positions carry the mass in w (Eq. 2:
+ * r_j and m_j); velocities and accelerations leave w unused (written as 0). */
+typedef struct hyb_float4 {
+    float x, y, z, w;
+} hyb_float4;
+
+typedef struct hyb_ctx hyb_ctx; /* opaque; created by hyb_init, destroyed by hyb_free */
+
+enum { HYB_MAC_THETA = 0, HYB_MAC_ABS = 1 };
+enum { HYB_K_PAPER = 0, HYB_K_POLY7 = 1 };
+
+/* The paper's statement of the problem. */
+typedef struct hyb_params {
+    float G;           /* gravitational constant, Eq. 2                                        */
+    float eps;         /* softening length, Eq. 2; must be > 0                                 */
+    float theta;       /* opening angle for HYB_MAC_THETA (open if d < l/theta); 0 opens all   */
+    float a_err;       /* absolute-MAC accuracy parameter of Eq. 5 (paper: 2^-8); > 0 if used  */
+    float r_in;        /* R_1 of Eq. 10                                                        */
+    float r_out;       /* R_2 of Eq. 10; 0 <= r_in < r_out                                     */
+    float dt_soft;     /* Delta t_s                                              */
+    int32_t n_sub;     /* n: Delta t_h = Delta t_s / n, >= 1                                   */
+    int32_t leaf_max;  /* n_crit: a cell with more particles is split; 1..64     */
+    int32_t group_max; /* sinks that share one traversal (n_vec); leaf_max..64   */
+    int32_t mac;       /* HYB_MAC_THETA or HYB_MAC_ABS (Eq. 5-6)                               */
+    int32_t kfunc;     /* HYB_K_PAPER (Eq. 10).  HYB_K_POLY7 is rejected (not built yet)       */
+    int32_t split;     /* 1 = hybrid (Eq. 7-9); 0 = normal tree (K == 0)     */
+} hyb_params;
+
+enum {
+    HYB_OK = 0,
+    HYB_ERR_INVALID_ARG = -1,
+    HYB_ERR_WORKSPACE_TOO_SMALL = -2,
+    HYB_ERR_NONFINITE_INPUT = -3,   /* a position or mass is NaN/Inf, or a mass is negative     */
+    HYB_ERR_CAPACITY_OVERFLOW = -4, /* node pool or a walk stack overflowed; results invalid    */
+    HYB_ERR_NO_TREE = -5,           /* force call without a tree built for the current positions*/
+    HYB_ERR_CUDA = -6,
+    HYB_ERR_INTERNAL = -7           /* a bounded device-side wait expired (should never happen) */
+};
+
+/* hyb_export selectors.  "n" = particles, "nn" = tree nodes, "ng" = sink groups (read them
+ * with HYB_X_COUNTS first).  All arrays refer to the store order after the last
+ * hyb_build_tree (Morton order). */
+enum {
+    HYB_X_COUNTS = 0,      /* int64[8]: n, nn, ng, node_cap, status_bits, 0, 0, 0               */
+    HYB_X_KEYS_SORTED = 1, /* uint64[n]  63-bit Morton keys, ascending                          */
+    HYB_X_PERM = 2,        /* uint32[n]  perm[j] = index, in the order the build found the
+                              store in, of the particle now in slot j (stable sort)            */
+    HYB_X_LEVEL = 3,       /* uint8[nn]                                                         */
+    HYB_X_FIRST = 4,       /* uint32[nn]                                                        */
+    HYB_X_COUNT = 5,       /* uint32[nn]                                                        */
+    HYB_X_CHILD = 6,       /* uint32[nn] index of first child, 0xFFFFFFFF for a leaf            */
+    HYB_X_NCHILD = 7,      /* uint8[nn]                                                         */
+    HYB_X_PARENT = 8,      /* uint32[nn] 0xFFFFFFFF for the root                                */
+    HYB_X_LEVEL_OFFSET = 9,/* uint32[23]                                                        */
+    HYB_X_COM_M = 10,      /* float[4 nn] centre of mass and mass                               */
+    HYB_X_ROPEN2 = 11,     /* float[nn]  squared opening radius                                 */
+    HYB_X_NLO = 12,        /* float[4 nn] tight box minimum (w unused)                          */
+    HYB_X_NHI = 13,        /* float[4 nn] tight box maximum (w unused)                          */
+    HYB_X_GFIRST = 14,     /* uint32[ng]                                                        */
+    HYB_X_GCOUNT = 15,     /* uint32[ng]                                                        */
+    HYB_X_GLO = 16,        /* float[4 ng]                                                       */
+    HYB_X_GHI = 17,        /* float[4 ng]                                                       */
+    HYB_X_NCELL = 18,      /* uint32[ng] cell-list length of the last walk                      */
+    HYB_X_NPART = 19,      /* uint32[ng] particle-list length of the last walk                  */
+    HYB_X_NHARD = 20,      /* uint32[ng] hard-list length of the last walk                      */
+    HYB_X_INTERACTIONS = 21,/* uint64[2] sum over groups of members x (ncell+npart), members x
+                              nhard, accumulated since hyb_init or the last read of this item   */
+    HYB_X_TIMINGS = 22,    /* float[8] ms accumulated in hyb_step since the last read:
+                              build, soft walk, hard walk, integrate, 0, 0, 0, cycles           */
+    HYB_X_BBOX = 23,       /* float[6] lo xyz, hi xyz of the last build                         */
+    HYB_X_KEYS = 24,       /* uint64[n] keys in the order the build found the store in          */
+    HYB_X_M64 = 25,        /* double[nn] node mass before rounding                              */
+    HYB_X_C64 = 26,        /* double[3 nn] node centre of mass before rounding                  */
+    HYB_X_B2 = 27,         /* double[nn]  B_2 of Eq. 6 (HYB_MAC_ABS only)                       */
+    HYB_X_BMAX = 28        /* double[nn]  b_max of Eq. 5 (HYB_MAC_ABS only)                     */
+};
+
+/* Bytes of device scratch hyb_init needs for n particles with these parameters.
+ * Pure host function (no CUDA call).  Returns 0 if n < 1 or the parameters are invalid. */
+size_t hyb_workspace_bytes(int64_t n, const hyb_params *params);
+
+/* Create a context.
+ *  params          host pointer; copied.
+ *  n               number of particles, 1 <= n < 2^31.
+ *  d_pos_m         DEVICE float4[n], in/out: positions and masses.  Re-ordered
+ *                  into Morton order by every tree build, advanced by hyb_step.
+ *  d_vel           DEVICE float4[n], in/out: velocities, re-ordered with the positions.
+ *  d_a_soft        DEVICE float4[n], out: soft accelerations, Eq. 9 summed over j
+ *                  (split = 0: the full normal-tree acceleration).
+ *  d_a_hard        DEVICE float4[n], out: hard accelerations, Eq. 8 summed over j.
+ *  d_id            DEVICE uint32[n], in/out: caller's particle labels, re-ordered with the
+ *                  positions (fill with 0..n-1 to track the permutation).
+ *  d_workspace     DEVICE scratch of at least hyb_workspace_bytes(n, params), 256-byte aligned.
+ *  device, cuda_stream   CUDA device ordinal and cudaStream_t (as void*) all work is issued on.
+ * All device buffers stay owned by the caller and must outlive the context.  The library
+ * allocates no device memory of its own.  hyb_init itself only zeroes its control block. */
+int hyb_init(hyb_ctx **out, const hyb_params *params, int64_t n,
+             hyb_float4 *d_pos_m, hyb_float4 *d_vel, hyb_float4 *d_a_soft, hyb_float4 *d_a_hard,
+             uint32_t *d_id, void *d_workspace, size_t workspace_bytes, int device, void *cuda_stream);
+
+/* Change parameters that do not affect workspace size (theta, a_err, r_in, r_out, eps, G,
+ * dt_soft, n_sub, mac, split); leaf_max / group_max must be unchanged.  Invalidates the tree. */
+int hyb_set_params(hyb_ctx *ctx, const hyb_params *params);
+
+/* Steps a1-a7: bounding box, 63-bit Morton keys, stable radix sort, re-order of pos/vel/id,
+ * linear octree, centre-of-mass / opening-radius upsweep
+ * and sink groups for the current positions.  Asynchronous. */
+int hyb_build_tree(hyb_ctx *ctx);
+
+/* Step a8 (+a9 at a soft-step).  split = 1: one fused group walk that writes d_a_soft
+ * (cells accepted by the MAC as monopoles, plus (1-K)-weighted neighbours, Eq. 9)
+ * AND d_a_hard (K-weighted neighbours within r_out, Eq. 8).  split = 0: normal-tree walk,
+ * d_a_soft = full acceleration, d_a_hard = 0.  Requires a tree.  Asynchronous. */
+int hyb_soft_force(hyb_ctx *ctx);
+
+/* Step a9 alone (a hard-step): neighbour search cut off at r_out
+ * and the K-weighted direct sum; writes d_a_hard only.  split = 0: writes zeros.
+ * Requires a tree.  Asynchronous. */
+int hyb_hard_force(hyb_ctx *ctx);
+
+/* n_soft_steps cycles of the two-rate leapfrog (Eq. 3-4), in the
+ * kick-drift-kick form of DESIGN.md (reading R21):
+ *   v += dt_s/2 a_soft;  n x { v += dt_h/2 a_hard; x += dt_h v; build; a_hard (and a_soft on the
+ *   last repeat); v += dt_h/2 a_hard };  v += dt_s/2 a_soft.
+ * If the accelerations are not valid for the current positions they are evaluated first.
+ * Leaves a_soft / a_hard valid for the final positions.  Synchronises the stream once at the
+ * end to read the device status word (capacity overflow, non-finite input). */
+int hyb_step(hyb_ctx *ctx, int32_t n_soft_steps);
+
+/* Synchronise the stream and return the device status as an error code. */
+int hyb_sync(hyb_ctx *ctx);
+
+/* Debug / test / bench read-back into HOST memory; synchronises the stream.
+ * *written (optional) receives the byte count; too small a buffer -> HYB_ERR_INVALID_ARG. */
+int hyb_export(hyb_ctx *ctx, int32_t what, void *host_dst, size_t bytes, size_t *written);
+
+/* End-to-end convenience for HOST buffers: allocates device memory, copies the particles in,
+ * runs hyb_step(n_soft_steps) (n_soft_steps = 0: one build + soft-step evaluation only), copies
+ * positions, velocities, ids and both accelerations back, frees everything.  Every pointer is a
+ * HOST pointer to n elements; h_interactions (optional) receives uint64[2] as HYB_X_INTERACTIONS. */
+int hyb_run_host(const hyb_params *params, int64_t n, hyb_float4 *h_pos_m, hyb_float4 *h_vel,
+                 hyb_float4 *h_a_soft, hyb_float4 *h_a_hard, uint32_t *h_id, int32_t n_soft_steps,
+                 int device, uint64_t *h_interactions);
+
+/* Message for the last error on this context ("" if none).  ctx may be NULL (returns the
+ * message of the last failed hyb_init / hyb_run_host on this thread). */
+const char *hyb_last_error(const hyb_ctx *ctx);
+
+/* Destroys the context (host memory and CUDA events only; device buffers are the caller's). */
+void hyb_free(hyb_ctx *ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* HYB_H */

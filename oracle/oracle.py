@@ -109,8 +109,8 @@ class Tree:
         self.ng = lib().orc_tree_ng(self._h)
 
     def __del__(self):
-        if getattr(self, "_h", None):
-            lib().orc_tree_free(self._h)
+        if getattr(self, "_h", None) and _lib is not None:
+            _lib.orc_tree_free(self._h)
             self._h = None
 
     def get(self, name: str) -> np.ndarray:

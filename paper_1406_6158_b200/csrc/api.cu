@@ -1,0 +1,411 @@
+// api.cu -- the C-ABI of include/hyb.h: argument checks, workspace carving, step driver, export.
+#include <math.h>
+#include <stdio.h>
+#include <string.h>
+
+#include <new>
+#include <vector>
+
+#include "common.cuh"
+
+namespace hyb {
+
+static thread_local char g_err[256] = "";
+
+static size_t align_up(size_t x) { return (x + 255) & ~(size_t)255; }
+
+Layout plan_workspace(int64_t n)
+{
+    Layout L;
+    memset(&L, 0, sizeof L);
+    L.n = n;
+    L.node_cap = node_capacity(n);
+    L.group_cap = n;
+    L.rs_tiles = (n + RS_TILE - 1) / RS_TILE;
+    L.node_tiles = (L.node_cap + RS_TILE - 1) / RS_TILE;
+    L.sc_tiles = (n + SC_TILE - 1) / SC_TILE;
+    L.n_walk_warps = 148 * 4 * WK_WARPS;
+    size_t off = 0;
+    auto take = [&](size_t bytes) { size_t o = off; off = align_up(off + bytes); return o; };
+    const size_t N = (size_t)n, NC = (size_t)L.node_cap, GC = (size_t)L.group_cap;
+    L.ctl = take(sizeof(DevCtl));
+    L.key_orig = take(8 * N); L.key_a = take(8 * N); L.key_b = take(8 * N);
+    L.val_a = take(4 * N); L.val_b = take(4 * N);
+    L.pos_tmp = take(16 * N); L.vel_tmp = take(16 * N); L.id_tmp = take(4 * N);
+    L.rs_status = take(4 * 256 * (size_t)L.rs_tiles * RS_PASSES);
+    L.sc_status = take(8 * 2 * (size_t)L.sc_tiles);
+    L.dlev = take(N); L.cnt_slot = take(4 * N); L.gflag = take(N);
+    L.pre_level = take(NC); L.pre_first = take(4 * NC); L.pre_of_bfs = take(4 * NC); L.bfs_of_pre = take(4 * NC);
+    L.node_status = take(4 * 256 * (size_t)L.node_tiles);
+    L.level = take(NC); L.first = take(4 * NC); L.count = take(4 * NC); L.child = take(4 * NC);
+    L.nchild = take(NC); L.parent = take(4 * NC); L.arrived = take(4 * NC);
+    L.nodeA = take(16 * NC); L.nodeB = take(16 * NC); L.nodeC = take(16 * NC); L.meta = take(8 * NC);
+    L.M64 = take(8 * NC); L.S64 = take(24 * NC); L.C64 = take(24 * NC); L.B2 = take(8 * NC); L.bmax2 = take(8 * NC);
+    L.leaf_of = take(4 * N);
+    L.gfirst = take(4 * GC); L.gcount = take(4 * GC); L.glo = take(16 * GC); L.ghi = take(16 * GC);
+    L.ncell = take(4 * GC); L.npart = take(4 * GC); L.nhard = take(4 * GC);
+    L.stacks = take(4 * (size_t)L.n_walk_warps * WK_STACK_CAP);
+    L.total = off;
+    return L;
+}
+
+static bool params_ok(const hyb_params *p, int64_t n, char *msg)
+{
+    auto bad = [&](const char *m) { snprintf(msg, 256, "%s", m); return false; };
+    if (!p) return bad("params is NULL");
+    if (n < 1 || n >= (1ll << 30)) return bad("n must be in [1, 2^30)");
+    if (!(p->eps > 0.0f) || !isfinite(p->eps)) return bad("eps must be finite and > 0");
+    if (!isfinite(p->G)) return bad("G must be finite");
+    if (p->n_sub < 1) return bad("n_sub must be >= 1");
+    if (!isfinite(p->dt_soft)) return bad("dt_soft must be finite");
+    if (p->leaf_max < 1 || p->group_max < p->leaf_max || p->group_max > 64) return bad("need 1 <= leaf_max <= group_max <= 64");
+    if (p->mac != HYB_MAC_THETA && p->mac != HYB_MAC_ABS) return bad("unknown mac");
+    if (p->mac == HYB_MAC_THETA && !(p->theta >= 0.0f && isfinite(p->theta))) return bad("theta must be finite and >= 0");
+    if (p->mac == HYB_MAC_ABS && !(p->a_err > 0.0f && isfinite(p->a_err))) return bad("a_err must be finite and > 0");
+    if (p->kfunc != HYB_K_PAPER) return bad("only HYB_K_PAPER (Eq. 10) is built");
+    if (p->split != 0 && p->split != 1) return bad("split must be 0 or 1");
+    if (p->split == 1 && !(p->r_in >= 0.0f && p->r_out > p->r_in && isfinite(p->r_out))) return bad("need 0 <= r_in < r_out");
+    return true;
+}
+
+static int fail(Ctx *c, int code, const char *msg)
+{
+    snprintf(g_err, sizeof g_err, "%s", msg);
+    if (c) snprintf(c->err, sizeof c->err, "%s", msg);
+    return code;
+}
+static int cuda_fail(Ctx *c, cudaError_t e, const char *where)
+{
+    char m[256];
+    snprintf(m, sizeof m, "%s: %s", where, cudaGetErrorString(e));
+    return fail(c, HYB_ERR_CUDA, m);
+}
+
+static int status_to_error(Ctx *c, u32 st)
+{
+    if (st & ST_NONFINITE) return fail(c, HYB_ERR_NONFINITE_INPUT, "non-finite position/mass or negative mass");
+    if (st & ST_NODE_OVERFLOW) return fail(c, HYB_ERR_CAPACITY_OVERFLOW, "tree node pool overflow");
+    if (st & ST_STACK_OVERFLOW) return fail(c, HYB_ERR_CAPACITY_OVERFLOW, "traversal stack overflow");
+    if (st & ST_WAIT_EXPIRED) return fail(c, HYB_ERR_INTERNAL, "device-side look-back wait expired");
+    return HYB_OK;
+}
+
+static int do_build(Ctx *c)
+{
+    cudaError_t e = launch_build_tree(c);
+    if (e != cudaSuccess) return cuda_fail(c, e, "build_tree");
+    c->tree_valid = true;
+    c->acc_valid = false;
+    return HYB_OK;
+}
+
+static int do_soft(Ctx *c)
+{
+    cudaError_t e = launch_walk(c, c->p.split ? WALK_HYBRID : WALK_NORMAL);
+    if (e != cudaSuccess) return cuda_fail(c, e, "soft walk");
+    return HYB_OK;
+}
+
+static int do_hard(Ctx *c)
+{
+    cudaError_t e = c->p.split ? launch_walk(c, WALK_HARD) : launch_zero_acc(c, c->a_hard);
+    if (e != cudaSuccess) return cuda_fail(c, e, "hard walk");
+    return HYB_OK;
+}
+
+}  // namespace hyb
+
+using namespace hyb;
+
+extern "C" {
+
+size_t hyb_workspace_bytes(int64_t n, const hyb_params *params)
+{
+    char msg[256];
+    if (!params_ok(params, n, msg)) return 0;
+    return plan_workspace(n).total;
+}
+
+int hyb_init(hyb_ctx **out, const hyb_params *params, int64_t n, hyb_float4 *d_pos_m, hyb_float4 *d_vel,
+             hyb_float4 *d_a_soft, hyb_float4 *d_a_hard, uint32_t *d_id, void *d_workspace, size_t workspace_bytes,
+             int device, void *cuda_stream)
+{
+    char msg[256];
+    if (!out) return fail(nullptr, HYB_ERR_INVALID_ARG, "out is NULL");
+    *out = nullptr;
+    if (!params_ok(params, n, msg)) return fail(nullptr, HYB_ERR_INVALID_ARG, msg);
+    if (!d_pos_m || !d_vel || !d_a_soft || !d_a_hard || !d_id || !d_workspace)
+        return fail(nullptr, HYB_ERR_INVALID_ARG, "a device pointer is NULL");
+    if (((uintptr_t)d_workspace & 255) || ((uintptr_t)d_pos_m & 15) || ((uintptr_t)d_vel & 15) ||
+        ((uintptr_t)d_a_soft & 15) || ((uintptr_t)d_a_hard & 15))
+        return fail(nullptr, HYB_ERR_INVALID_ARG, "misaligned device pointer");
+    Layout L = plan_workspace(n);
+    if (workspace_bytes < L.total) return fail(nullptr, HYB_ERR_WORKSPACE_TOO_SMALL, "workspace too small");
+    cudaError_t e = cudaSetDevice(device);
+    if (e != cudaSuccess) return cuda_fail(nullptr, e, "cudaSetDevice");
+    Ctx *c = new (std::nothrow) Ctx;
+    if (!c) return fail(nullptr, HYB_ERR_INTERNAL, "out of host memory");
+    memset(c, 0, sizeof *c);
+    c->p = *params; c->n = n; c->device = device; c->stream = (cudaStream_t)cuda_stream;
+    c->pos = d_pos_m; c->vel = d_vel; c->a_soft = d_a_soft; c->a_hard = d_a_hard; c->id = d_id;
+    c->ws = (char *)d_workspace; c->L = L; c->ctl = (DevCtl *)(c->ws + L.ctl);
+    e = cudaDeviceGetAttribute(&c->num_sms, cudaDevAttrMultiProcessorCount, device);
+    if (e != cudaSuccess) { delete c; return cuda_fail(nullptr, e, "cudaDeviceGetAttribute"); }
+    for (int i = 0; i < 5; i++) {
+        e = cudaEventCreate(&c->ev[i]);
+        if (e != cudaSuccess) { delete c; return cuda_fail(nullptr, e, "cudaEventCreate"); }
+    }
+    c->timing = true;
+    e = cudaMemsetAsync(c->ctl, 0, sizeof(DevCtl), c->stream);
+    if (e != cudaSuccess) { delete c; return cuda_fail(nullptr, e, "cudaMemsetAsync"); }
+    *out = reinterpret_cast<hyb_ctx *>(c);
+    return HYB_OK;
+}
+
+int hyb_set_params(hyb_ctx *ctx, const hyb_params *params)
+{
+    Ctx *c = reinterpret_cast<Ctx *>(ctx);
+    char msg[256];
+    if (!c) return fail(nullptr, HYB_ERR_INVALID_ARG, "ctx is NULL");
+    if (!params_ok(params, c->n, msg)) return fail(c, HYB_ERR_INVALID_ARG, msg);
+    if (params->leaf_max != c->p.leaf_max || params->group_max != c->p.group_max)
+        return fail(c, HYB_ERR_INVALID_ARG, "leaf_max / group_max cannot change after hyb_init");
+    c->p = *params;
+    c->tree_valid = false; c->acc_valid = false;
+    return HYB_OK;
+}
+
+int hyb_build_tree(hyb_ctx *ctx)
+{
+    Ctx *c = reinterpret_cast<Ctx *>(ctx);
+    if (!c) return fail(nullptr, HYB_ERR_INVALID_ARG, "ctx is NULL");
+    cudaSetDevice(c->device);
+    return do_build(c);
+}
+
+int hyb_soft_force(hyb_ctx *ctx)
+{
+    Ctx *c = reinterpret_cast<Ctx *>(ctx);
+    if (!c) return fail(nullptr, HYB_ERR_INVALID_ARG, "ctx is NULL");
+    if (!c->tree_valid) return fail(c, HYB_ERR_NO_TREE, "no tree for the current positions");
+    cudaSetDevice(c->device);
+    int rc = do_soft(c);
+    if (rc == HYB_OK) c->acc_valid = true;
+    return rc;
+}
+
+int hyb_hard_force(hyb_ctx *ctx)
+{
+    Ctx *c = reinterpret_cast<Ctx *>(ctx);
+    if (!c) return fail(nullptr, HYB_ERR_INVALID_ARG, "ctx is NULL");
+    if (!c->tree_valid) return fail(c, HYB_ERR_NO_TREE, "no tree for the current positions");
+    cudaSetDevice(c->device);
+    return do_hard(c);
+}
+
+int hyb_sync(hyb_ctx *ctx)
+{
+    Ctx *c = reinterpret_cast<Ctx *>(ctx);
+    if (!c) return fail(nullptr, HYB_ERR_INVALID_ARG, "ctx is NULL");
+    cudaSetDevice(c->device);
+    u32 st = 0;
+    cudaError_t e = cudaMemcpyAsync(&st, &c->ctl->status, sizeof st, cudaMemcpyDeviceToHost, c->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
+    if (e != cudaSuccess) return cuda_fail(c, e, "hyb_sync");
+    return status_to_error(c, st);
+}
+
+int hyb_step(hyb_ctx *ctx, int32_t n_soft_steps)
+{
+    Ctx *c = reinterpret_cast<Ctx *>(ctx);
+    if (!c) return fail(nullptr, HYB_ERR_INVALID_ARG, "ctx is NULL");
+    if (n_soft_steps < 0) return fail(c, HYB_ERR_INVALID_ARG, "n_soft_steps < 0");
+    cudaSetDevice(c->device);
+    const bool split = c->p.split != 0;
+    const int nsub = c->p.n_sub;
+    const float dts = c->p.dt_soft, dth = dts / (float)nsub;
+    int rc;
+    if (!c->acc_valid) {
+        if ((rc = do_build(c)) != HYB_OK) return rc;
+        if ((rc = do_soft(c)) != HYB_OK) return rc;
+        c->acc_valid = true;
+    }
+    struct Seg { int kind; cudaEvent_t a, b; };     // kind: 0 build, 1 soft, 2 hard, 3 integrate
+    std::vector<Seg> segs;
+    std::vector<cudaEvent_t> pool;
+    auto ev = [&]() { cudaEvent_t e; cudaEventCreate(&e); pool.push_back(e); cudaEventRecord(e, c->stream); return e; };
+    for (int32_t cyc = 0; cyc < n_soft_steps; cyc++) {
+        for (int k = 0; k < nsub; k++) {
+            cudaEvent_t e0 = c->timing ? ev() : nullptr;
+            cudaError_t e;
+            // opening kick(s) + drift.  split = 0: the whole force lives in a_soft and is kicked at dt_h.
+            if (split) e = launch_kick_drift(c, k == 0 ? 0.5f * dts : 0.0f, 0.5f * dth, dth);
+            else e = launch_kick_drift(c, 0.5f * dth, 0.0f, dth);
+            if (e != cudaSuccess) return cuda_fail(c, e, "kick_drift");
+            cudaEvent_t e1 = c->timing ? ev() : nullptr;
+            if ((rc = do_build(c)) != HYB_OK) return rc;
+            cudaEvent_t e2 = c->timing ? ev() : nullptr;
+            const bool soft_step = !split || k == nsub - 1;
+            if (soft_step) rc = do_soft(c); else rc = do_hard(c);
+            if (rc != HYB_OK) return rc;
+            cudaEvent_t e3 = c->timing ? ev() : nullptr;
+            if (split) e = launch_kick_drift(c, k == nsub - 1 ? 0.5f * dts : 0.0f, 0.5f * dth, 0.0f);
+            else e = launch_kick_drift(c, 0.5f * dth, 0.0f, 0.0f);
+            if (e != cudaSuccess) return cuda_fail(c, e, "kick");
+            if (c->timing) {
+                cudaEvent_t e4 = ev();
+                segs.push_back({3, e0, e1}); segs.push_back({0, e1, e2});
+                segs.push_back({soft_step ? 1 : 2, e2, e3}); segs.push_back({3, e3, e4});
+            }
+        }
+        c->acc_valid = true;
+    }
+    rc = hyb_sync(ctx);
+    for (auto &s : segs) { float ms = 0; cudaEventElapsedTime(&ms, s.a, s.b); c->t_acc[s.kind] += ms; }
+    for (auto e : pool) cudaEventDestroy(e);
+    c->t_acc[7] += (float)n_soft_steps;
+    return rc;
+}
+
+int hyb_export(hyb_ctx *ctx, int32_t what, void *host_dst, size_t bytes, size_t *written)
+{
+    Ctx *c = reinterpret_cast<Ctx *>(ctx);
+    if (!c) return fail(nullptr, HYB_ERR_INVALID_ARG, "ctx is NULL");
+    if (!host_dst) return fail(c, HYB_ERR_INVALID_ARG, "host_dst is NULL");
+    cudaSetDevice(c->device);
+    cudaError_t e = cudaStreamSynchronize(c->stream);
+    if (e != cudaSuccess) return cuda_fail(c, e, "hyb_export sync");
+    DevCtl h;
+    e = cudaMemcpy(&h, c->ctl, sizeof h, cudaMemcpyDeviceToHost);
+    if (e != cudaSuccess) return cuda_fail(c, e, "hyb_export ctl");
+    const Layout &L = c->L;
+    const size_t n = (size_t)c->n, nn = h.nn, ng = h.ng;
+    const void *src = nullptr; size_t sz = 0;
+    std::vector<char> tmp;
+    switch (what) {
+    case HYB_X_COUNTS: {
+        int64_t v[8] = {(int64_t)n, (int64_t)nn, (int64_t)ng, L.node_cap, (int64_t)h.status, (int64_t)h.nn_total, 0, 0};
+        if (bytes < sizeof v) return fail(c, HYB_ERR_INVALID_ARG, "buffer too small");
+        memcpy(host_dst, v, sizeof v); if (written) *written = sizeof v; return HYB_OK; }
+    case HYB_X_LEVEL_OFFSET:
+        if (bytes < sizeof h.level_offset) return fail(c, HYB_ERR_INVALID_ARG, "buffer too small");
+        memcpy(host_dst, h.level_offset, sizeof h.level_offset); if (written) *written = sizeof h.level_offset; return HYB_OK;
+    case HYB_X_BBOX:
+        if (bytes < sizeof h.bbox) return fail(c, HYB_ERR_INVALID_ARG, "buffer too small");
+        memcpy(host_dst, h.bbox, sizeof h.bbox); if (written) *written = sizeof h.bbox; return HYB_OK;
+    case HYB_X_INTERACTIONS: {
+        u64 v[2] = {h.inter_soft, h.inter_hard};
+        if (bytes < sizeof v) return fail(c, HYB_ERR_INVALID_ARG, "buffer too small");
+        memcpy(host_dst, v, sizeof v); if (written) *written = sizeof v;
+        cudaMemset(&c->ctl->inter_soft, 0, 2 * sizeof(u64));
+        return HYB_OK; }
+    case HYB_X_TIMINGS:
+        if (bytes < sizeof c->t_acc) return fail(c, HYB_ERR_INVALID_ARG, "buffer too small");
+        memcpy(host_dst, c->t_acc, sizeof c->t_acc); if (written) *written = sizeof c->t_acc;
+        memset(c->t_acc, 0, sizeof c->t_acc);
+        return HYB_OK;
+    case HYB_X_KEYS_SORTED: src = c->ws + L.key_b; sz = 8 * n; break;
+    case HYB_X_KEYS: src = c->ws + L.key_orig; sz = 8 * n; break;
+    case HYB_X_PERM: src = c->ws + L.val_b; sz = 4 * n; break;
+    case HYB_X_LEVEL: src = c->ws + L.level; sz = nn; break;
+    case HYB_X_FIRST: src = c->ws + L.first; sz = 4 * nn; break;
+    case HYB_X_COUNT: src = c->ws + L.count; sz = 4 * nn; break;
+    case HYB_X_CHILD: src = c->ws + L.child; sz = 4 * nn; break;
+    case HYB_X_NCHILD: src = c->ws + L.nchild; sz = nn; break;
+    case HYB_X_PARENT: src = c->ws + L.parent; sz = 4 * nn; break;
+    case HYB_X_COM_M: src = c->ws + L.nodeA; sz = 16 * nn; break;
+    case HYB_X_NLO: src = c->ws + L.nodeB; sz = 16 * nn; break;
+    case HYB_X_NHI: src = c->ws + L.nodeC; sz = 16 * nn; break;
+    case HYB_X_ROPEN2: {
+        if (bytes < 4 * nn) return fail(c, HYB_ERR_INVALID_ARG, "buffer too small");
+        tmp.resize(16 * nn);
+        e = cudaMemcpy(tmp.data(), c->ws + L.nodeB, 16 * nn, cudaMemcpyDeviceToHost);
+        if (e != cudaSuccess) return cuda_fail(c, e, "hyb_export copy");
+        for (size_t i = 0; i < nn; i++) ((float *)host_dst)[i] = ((const float *)tmp.data())[4 * i + 3];
+        if (written) *written = 4 * nn;
+        return HYB_OK; }
+    case HYB_X_GFIRST: src = c->ws + L.gfirst; sz = 4 * ng; break;
+    case HYB_X_GCOUNT: src = c->ws + L.gcount; sz = 4 * ng; break;
+    case HYB_X_GLO: src = c->ws + L.glo; sz = 16 * ng; break;
+    case HYB_X_GHI: src = c->ws + L.ghi; sz = 16 * ng; break;
+    case HYB_X_NCELL: src = c->ws + L.ncell; sz = 4 * ng; break;
+    case HYB_X_NPART: src = c->ws + L.npart; sz = 4 * ng; break;
+    case HYB_X_NHARD: src = c->ws + L.nhard; sz = 4 * ng; break;
+    case HYB_X_M64: src = c->ws + L.M64; sz = 8 * nn; break;
+    case HYB_X_C64: src = c->ws + L.C64; sz = 24 * nn; break;
+    case HYB_X_B2: src = c->ws + L.B2; sz = 8 * nn; break;
+    case HYB_X_BMAX: {
+        if (bytes < 8 * nn) return fail(c, HYB_ERR_INVALID_ARG, "buffer too small");
+        e = cudaMemcpy(host_dst, c->ws + L.bmax2, 8 * nn, cudaMemcpyDeviceToHost);
+        if (e != cudaSuccess) return cuda_fail(c, e, "hyb_export copy");
+        for (size_t i = 0; i < nn; i++) ((double *)host_dst)[i] = sqrt(((double *)host_dst)[i]);
+        if (written) *written = 8 * nn;
+        return HYB_OK; }
+    default: return fail(c, HYB_ERR_INVALID_ARG, "unknown export selector");
+    }
+    if (bytes < sz) return fail(c, HYB_ERR_INVALID_ARG, "buffer too small");
+    if (sz) {
+        e = cudaMemcpy(host_dst, src, sz, cudaMemcpyDeviceToHost);
+        if (e != cudaSuccess) return cuda_fail(c, e, "hyb_export copy");
+    }
+    if (written) *written = sz;
+    return HYB_OK;
+}
+
+int hyb_run_host(const hyb_params *params, int64_t n, hyb_float4 *h_pos_m, hyb_float4 *h_vel, hyb_float4 *h_a_soft,
+                 hyb_float4 *h_a_hard, uint32_t *h_id, int32_t n_soft_steps, int device, uint64_t *h_interactions)
+{
+    char msg[256];
+    if (!params_ok(params, n, msg)) return fail(nullptr, HYB_ERR_INVALID_ARG, msg);
+    if (!h_pos_m || !h_vel || !h_a_soft || !h_a_hard || !h_id) return fail(nullptr, HYB_ERR_INVALID_ARG, "a host pointer is NULL");
+    cudaError_t e = cudaSetDevice(device);
+    if (e != cudaSuccess) return cuda_fail(nullptr, e, "cudaSetDevice");
+    const size_t ws_bytes = plan_workspace(n).total, N = (size_t)n;
+    char *d = nullptr;
+    const size_t o_pos = 0, o_vel = 16 * N, o_as = 32 * N, o_ah = 48 * N, o_id = 64 * N;
+    const size_t o_ws = (68 * N + 255) & ~(size_t)255;
+    e = cudaMalloc(&d, o_ws + ws_bytes);
+    if (e != cudaSuccess) return cuda_fail(nullptr, e, "cudaMalloc");
+    cudaStream_t st = nullptr;
+    int rc = HYB_OK;
+    hyb_ctx *ctx = nullptr;
+    do {
+        if ((e = cudaStreamCreate(&st)) != cudaSuccess) { rc = cuda_fail(nullptr, e, "cudaStreamCreate"); break; }
+        cudaMemcpyAsync(d + o_pos, h_pos_m, 16 * N, cudaMemcpyHostToDevice, st);
+        cudaMemcpyAsync(d + o_vel, h_vel, 16 * N, cudaMemcpyHostToDevice, st);
+        cudaMemcpyAsync(d + o_id, h_id, 4 * N, cudaMemcpyHostToDevice, st);
+        rc = hyb_init(&ctx, params, n, (hyb_float4 *)(d + o_pos), (hyb_float4 *)(d + o_vel), (hyb_float4 *)(d + o_as),
+                      (hyb_float4 *)(d + o_ah), (uint32_t *)(d + o_id), d + o_ws, ws_bytes, device, st);
+        if (rc != HYB_OK) break;
+        reinterpret_cast<Ctx *>(ctx)->timing = false;
+        rc = hyb_step(ctx, n_soft_steps);
+        if (rc != HYB_OK) break;
+        cudaMemcpyAsync(h_pos_m, d + o_pos, 16 * N, cudaMemcpyDeviceToHost, st);
+        cudaMemcpyAsync(h_vel, d + o_vel, 16 * N, cudaMemcpyDeviceToHost, st);
+        cudaMemcpyAsync(h_a_soft, d + o_as, 16 * N, cudaMemcpyDeviceToHost, st);
+        cudaMemcpyAsync(h_a_hard, d + o_ah, 16 * N, cudaMemcpyDeviceToHost, st);
+        cudaMemcpyAsync(h_id, d + o_id, 4 * N, cudaMemcpyDeviceToHost, st);
+        if ((e = cudaStreamSynchronize(st)) != cudaSuccess) { rc = cuda_fail(nullptr, e, "copy back"); break; }
+        if (h_interactions) rc = hyb_export(ctx, HYB_X_INTERACTIONS, h_interactions, 16, nullptr);
+    } while (0);
+    if (ctx) hyb_free(ctx);
+    if (st) cudaStreamDestroy(st);
+    cudaFree(d);
+    return rc;
+}
+
+const char *hyb_last_error(const hyb_ctx *ctx)
+{
+    const Ctx *c = reinterpret_cast<const Ctx *>(ctx);
+    return c ? c->err : g_err;
+}
+
+void hyb_free(hyb_ctx *ctx)
+{
+    Ctx *c = reinterpret_cast<Ctx *>(ctx);
+    if (!c) return;
+    for (int i = 0; i < 5; i++) if (c->ev[i]) cudaEventDestroy(c->ev[i]);
+    delete c;
+}
+
+}  // extern "C"

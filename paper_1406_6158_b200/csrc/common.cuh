@@ -1,0 +1,160 @@
+// common.cuh -- shared declarations of the hyb CUDA library (sm_100a).
+// Product code: shares nothing with oracle/.
+#pragma once
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <stddef.h>
+
+#include "../../include/hyb.h"
+
+namespace hyb {
+
+typedef unsigned int u32;
+typedef unsigned long long u64;
+
+constexpr u32 NOCHILD = 0xFFFFFFFFu;
+constexpr int MAXLEVEL = 21;
+
+// status bits (device control block)
+constexpr u32 ST_NONFINITE = 1u;
+constexpr u32 ST_NODE_OVERFLOW = 2u;
+constexpr u32 ST_STACK_OVERFLOW = 4u;
+constexpr u32 ST_WAIT_EXPIRED = 8u;
+
+// radix sort tiling (onesweep): 256 threads x 16 keys
+constexpr int RS_THREADS = 256;
+constexpr int RS_KPT = 16;
+constexpr int RS_TILE = RS_THREADS * RS_KPT;
+constexpr int RS_PASSES = 8;      // 8 x 8 bits >= 63 bits
+
+// single-value scan tiles (octree preorder, group compaction)
+constexpr int SC_THREADS = 256;
+constexpr int SC_IPT = 4;
+constexpr int SC_TILE = SC_THREADS * SC_IPT;
+
+// walk kernel geometry
+constexpr int WK_WARPS = 8;              // warps per CTA
+constexpr int WK_CELL_CAP = 256;         // monopole buffer entries per warp
+constexpr int WK_PART_CAP = 128;         // K-weighted (near) particle buffer entries per warp
+constexpr int WK_STACK_CAP = 8192;       // traversal stack entries per warp (global memory)
+
+enum WalkMode { WALK_HYBRID = 0, WALK_HARD = 1, WALK_NORMAL = 2 };
+
+// Device control block: lives at the start of the caller's workspace.
+struct DevCtl {
+    u32 status;
+    u32 nn, ng;
+    u32 level_offset[MAXLEVEL + 2];
+    // ---- reset at the start of every build (see reset_build_state) ----
+    u32 bbox_enc[6];            // order-preserving encodings: min xyz, max xyz
+    u32 digit_hist[RS_PASSES * 256];
+    u32 node_hist[256];
+    u32 tile_counter[16];       // dynamic tile ids, one slot per lookback kernel instance
+    u32 nn_total;               // un-clamped node count
+    // ---- derived ----
+    float bbox[6];
+    double L, inv, origin[3];
+    float Lf;
+    u32 digit_base[RS_PASSES * 256];
+    u32 node_base[256];
+    // ---- walk ----
+    u32 group_counter;
+    u64 inter_soft, inter_hard;
+};
+
+struct Layout {   // byte offsets into the workspace; computed by plan_workspace
+    size_t ctl;
+    size_t key_orig, key_a, key_b, val_a, val_b;
+    size_t pos_tmp, vel_tmp, id_tmp;
+    size_t rs_status;           // [RS_PASSES][ntiles][256] u32
+    size_t sc_status;           // [2][nsc_tiles] u64   (preorder scan, group scan)
+    size_t dlev, cnt_slot;      // int8[n], u32[n]
+    size_t gflag;               // u8[n]
+    size_t pre_level, pre_first, pre_of_bfs, bfs_of_pre;   // u8, u32, u32, u32 [node_cap]
+    size_t node_status;         // [ntiles(node_cap)][256] u32
+    size_t level, first, count, child, nchild, parent, arrived;
+    size_t nodeA, nodeB, nodeC, meta;          // float4, float4, float4, uint2
+    size_t M64, S64, C64, B2, bmax2;           // double[nc], [3nc], [3nc], [nc], u64[nc]
+    size_t leaf_of;             // u32[n]
+    size_t gfirst, gcount, glo, ghi, ncell, npart, nhard;   // [group_cap]
+    size_t stacks;              // [n_walk_warps][WK_STACK_CAP] u32
+    size_t total;
+    int64_t n, node_cap, group_cap;
+    int64_t rs_tiles, node_tiles, sc_tiles;
+    int n_walk_warps;
+};
+
+inline int64_t node_capacity(int64_t n) { return 2 * n + 4096; }
+inline int64_t imin64(int64_t a, int64_t b) { return a < b ? a : b; }
+Layout plan_workspace(int64_t n);
+
+struct Ctx {
+    hyb_params p;
+    int64_t n;
+    int device;
+    cudaStream_t stream;
+    int num_sms;
+    hyb_float4 *pos, *vel, *a_soft, *a_hard;
+    u32 *id;
+    char *ws;
+    Layout L;
+    bool tree_valid, acc_valid;
+    cudaEvent_t ev[5];
+    float t_acc[8];
+    bool timing;
+    char err[256];
+    // typed views of the workspace
+    DevCtl *ctl;
+};
+
+template <typename T>
+static inline T *wsptr(const Ctx *c, size_t off) { return reinterpret_cast<T *>(c->ws + off); }
+
+// stage launchers (each enqueues on c->stream and returns the last CUDA error)
+cudaError_t launch_build_tree(Ctx *c);
+cudaError_t launch_walk(Ctx *c, int mode);
+cudaError_t launch_kick_drift(Ctx *c, float c_soft, float c_hard, float dt_drift);
+cudaError_t launch_zero_acc(Ctx *c, hyb_float4 *a);
+
+// ---- device helpers ------------------------------------------------------------------
+__device__ __forceinline__ u32 enc_float(float f)
+{
+    u32 u = __float_as_uint(f);
+    return (u & 0x80000000u) ? ~u : (u | 0x80000000u);
+}
+__device__ __forceinline__ float dec_float(u32 e)
+{
+    return __uint_as_float((e & 0x80000000u) ? (e ^ 0x80000000u) : ~e);
+}
+__device__ __forceinline__ u32 ld_volatile_u32(const u32 *p)
+{
+    return *reinterpret_cast<const volatile u32 *>(p);
+}
+__device__ __forceinline__ u64 ld_volatile_u64(const u64 *p)
+{
+    return *reinterpret_cast<const volatile u64 *>(p);
+}
+
+// Decoupled look-back over one value per tile (status word: bits 63..62 flag, low 62 bits value).
+// Called by ONE thread of the CTA that owns `tile`; returns the exclusive prefix of earlier tiles.
+constexpr u64 LB_AGG = 1ull << 62, LB_PREFIX = 2ull << 62, LB_MASK = (1ull << 62) - 1;
+constexpr int LB_SPIN_LIMIT = 1 << 22;
+__device__ __forceinline__ u64 lookback_single(u64 *status, u32 tile, u64 aggregate, u32 *dev_status)
+{
+    volatile u64 *st = status;
+    if (tile == 0) { st[0] = LB_PREFIX | aggregate; return 0; }
+    st[tile] = LB_AGG | aggregate;
+    u64 excl = 0;
+    for (long long t = (long long)tile - 1; t >= 0; --t) {
+        u64 s; int spins = 0;
+        do { s = st[t]; } while ((s >> 62) == 0 && ++spins < LB_SPIN_LIMIT);
+        if ((s >> 62) == 0) { atomicOr(dev_status, ST_WAIT_EXPIRED); break; }
+        excl += s & LB_MASK;
+        if ((s >> 62) == 2) break;
+    }
+    st[tile] = LB_PREFIX | (excl + aggregate);
+    return excl;
+}
+
+}  // namespace hyb

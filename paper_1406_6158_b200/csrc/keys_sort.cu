@@ -1,0 +1,162 @@
+// keys_sort.cu -- steps a1-a4: bounding box, 63-bit Morton keys, stable onesweep radix sort,
+// re-order of the particle store.  (T2-T6.)
+#include "common.cuh"
+#include "sort.cuh"
+
+namespace hyb {
+
+// ------------------------------------------------------------------ a1: bounding box (T1, T2)
+__global__ void __launch_bounds__(256) bbox_kernel(const float4 *__restrict__ pos, u32 n, DevCtl *ctl)
+{
+    float lo[3] = {INFINITY, INFINITY, INFINITY}, hi[3] = {-INFINITY, -INFINITY, -INFINITY};
+    bool bad = false;
+    for (u32 i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
+        float4 p = __ldg(pos + i);
+        bad |= !(isfinite(p.x) && isfinite(p.y) && isfinite(p.z) && isfinite(p.w)) || p.w < 0.0f;
+        lo[0] = fminf(lo[0], p.x); hi[0] = fmaxf(hi[0], p.x);
+        lo[1] = fminf(lo[1], p.y); hi[1] = fmaxf(hi[1], p.y);
+        lo[2] = fminf(lo[2], p.z); hi[2] = fmaxf(hi[2], p.z);
+    }
+    __shared__ u32 s_enc[6];
+    if (threadIdx.x < 3) s_enc[threadIdx.x] = 0xFFFFFFFFu;
+    else if (threadIdx.x < 6) s_enc[threadIdx.x] = 0u;
+    __syncthreads();
+#pragma unroll
+    for (int a = 0; a < 3; a++) {
+        u32 mn = __reduce_min_sync(0xFFFFFFFFu, enc_float(lo[a]));
+        u32 mx = __reduce_max_sync(0xFFFFFFFFu, enc_float(hi[a]));
+        if ((threadIdx.x & 31) == 0) { atomicMin(&s_enc[a], mn); atomicMax(&s_enc[3 + a], mx); }
+    }
+    if (__any_sync(0xFFFFFFFFu, bad) && (threadIdx.x & 31) == 0) atomicOr(&ctl->status, ST_NONFINITE);
+    __syncthreads();
+    if (threadIdx.x < 3) atomicMin(&ctl->bbox_enc[threadIdx.x], s_enc[threadIdx.x]);
+    else if (threadIdx.x < 6) atomicMax(&ctl->bbox_enc[threadIdx.x], s_enc[threadIdx.x]);
+}
+
+// T3: root cube.  One thread.
+__global__ void root_cube_kernel(DevCtl *ctl)
+{
+    double L = 0.0;
+    for (int a = 0; a < 3; a++) {
+        float lo = dec_float(ctl->bbox_enc[a]), hi = dec_float(ctl->bbox_enc[3 + a]);
+        ctl->bbox[a] = lo; ctl->bbox[3 + a] = hi;
+        double e = __dsub_rn((double)hi, (double)lo);
+        if (e > L) L = e;
+        ctl->origin[a] = (double)lo;
+    }
+    if (!(L > 0.0) || !isfinite(L)) L = 1.0;
+    ctl->L = L;
+    ctl->inv = __ddiv_rn(2097152.0, L);
+    ctl->Lf = __double2float_rn(L);
+}
+
+// ------------------------------------------------------------------ a2: keys (T4, T5)
+__device__ __forceinline__ u64 spread21(u32 q)
+{
+    u64 x = q & 0x1FFFFFu;
+    x = (x | (x << 32)) & 0x001F00000000FFFFull;
+    x = (x | (x << 16)) & 0x001F0000FF0000FFull;
+    x = (x | (x << 8)) & 0x100F00F00F00F00Full;
+    x = (x | (x << 4)) & 0x10C30C30C30C30C3ull;
+    x = (x | (x << 2)) & 0x1249249249249249ull;
+    return x;
+}
+
+__device__ __forceinline__ u32 quantise(float x, double o, double inv)
+{
+    double s = __dmul_rn(__dsub_rn((double)x, o), inv);
+    double f = floor(s);
+    return f >= 2097151.0 ? 2097151u : (f > 0.0 ? (u32)f : 0u);
+}
+
+// also accumulates the eight 8-bit digit histograms the onesweep sort needs
+__global__ void __launch_bounds__(256) keys_kernel(const float4 *__restrict__ pos, u32 n, DevCtl *ctl,
+                                                   u64 *__restrict__ key)
+{
+    __shared__ u32 hist[RS_PASSES * 256];
+    for (int i = threadIdx.x; i < RS_PASSES * 256; i += blockDim.x) hist[i] = 0;
+    __syncthreads();
+    const double ox = ctl->origin[0], oy = ctl->origin[1], oz = ctl->origin[2], inv = ctl->inv;
+    for (u32 i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
+        float4 p = __ldg(pos + i);
+        u64 k = (spread21(quantise(p.x, ox, inv)) << 2) | (spread21(quantise(p.y, oy, inv)) << 1) |
+                spread21(quantise(p.z, oz, inv));
+        key[i] = k;
+#pragma unroll
+        for (int d = 0; d < RS_PASSES; d++) atomicAdd(&hist[d * 256 + (u32)((k >> (8 * d)) & 0xFF)], 1u);
+    }
+    __syncthreads();
+    for (int i = threadIdx.x; i < RS_PASSES * 256; i += blockDim.x)
+        if (hist[i]) atomicAdd(&ctl->digit_hist[i], hist[i]);
+}
+
+// exclusive scan of each 256-bin histogram -> digit_base.  One CTA of 256 threads per pass.
+__global__ void __launch_bounds__(256) digit_base_kernel(DevCtl *ctl)
+{
+    __shared__ u32 s[256];
+    const u32 *h = ctl->digit_hist + blockIdx.x * 256;
+    u32 v = h[threadIdx.x];
+    s[threadIdx.x] = v;
+    __syncthreads();
+    for (int off = 1; off < 256; off <<= 1) {
+        u32 t = threadIdx.x >= off ? s[threadIdx.x - off] : 0;
+        __syncthreads();
+        s[threadIdx.x] += t;
+        __syncthreads();
+    }
+    ctl->digit_base[blockIdx.x * 256 + threadIdx.x] = s[threadIdx.x] - v;
+}
+
+// ------------------------------------------------------------------ a4: re-order (T6)
+__global__ void __launch_bounds__(256) permute_kernel(const u32 *__restrict__ perm, u32 n,
+                                                      const float4 *__restrict__ pos, const float4 *__restrict__ vel,
+                                                      const u32 *__restrict__ id, float4 *__restrict__ pos_o,
+                                                      float4 *__restrict__ vel_o, u32 *__restrict__ id_o)
+{
+    for (u32 j = blockIdx.x * blockDim.x + threadIdx.x; j < n; j += gridDim.x * blockDim.x) {
+        u32 s = perm[j];
+        pos_o[j] = __ldg(pos + s);
+        vel_o[j] = __ldg(vel + s);
+        id_o[j] = __ldg(id + s);
+    }
+}
+
+cudaError_t launch_keys_sort_permute(Ctx *c)
+{
+    const Layout &L = c->L;
+    const u32 n = (u32)c->n;
+    cudaStream_t st = c->stream;
+    DevCtl *ctl = c->ctl;
+    const int grid = (int)imin64((c->n + 255) / 256, (int64_t)c->num_sms * 8);
+
+    bbox_kernel<<<grid, 256, 0, st>>>(reinterpret_cast<const float4 *>(c->pos), n, ctl);
+    root_cube_kernel<<<1, 1, 0, st>>>(ctl);
+    u64 *key_orig = wsptr<u64>(c, L.key_orig), *key_a = wsptr<u64>(c, L.key_a), *key_b = wsptr<u64>(c, L.key_b);
+    u32 *val_a = wsptr<u32>(c, L.val_a), *val_b = wsptr<u32>(c, L.val_b);
+    keys_kernel<<<grid, 256, 0, st>>>(reinterpret_cast<const float4 *>(c->pos), n, ctl, key_orig);
+    digit_base_kernel<<<RS_PASSES, 256, 0, st>>>(ctl);
+
+    u32 *status = wsptr<u32>(c, L.rs_status);
+    const int sgrid = (int)imin64(L.rs_tiles, (int64_t)c->num_sms * 3);
+    const u64 *kin = key_orig; const u32 *vin = nullptr;
+    for (int pass = 0; pass < RS_PASSES; pass++) {
+        u64 *kout = (pass & 1) ? key_b : key_a;
+        u32 *vout = (pass & 1) ? val_b : val_a;
+        cudaError_t e = launch_radix_pass<u64>(kin, vin, kout, vout, nullptr, n, nullptr, 8 * pass,
+                                               ctl->digit_base + pass * 256, status + (size_t)pass * L.rs_tiles * 256,
+                                               &ctl->tile_counter[pass], &ctl->status, sgrid, st);
+        if (e != cudaSuccess) return e;
+        kin = kout; vin = vout;
+    }
+    // RS_PASSES is even: sorted keys in key_b, permutation in val_b
+    float4 *pos_t = wsptr<float4>(c, L.pos_tmp), *vel_t = wsptr<float4>(c, L.vel_tmp);
+    u32 *id_t = wsptr<u32>(c, L.id_tmp);
+    permute_kernel<<<grid, 256, 0, st>>>(val_b, n, reinterpret_cast<const float4 *>(c->pos),
+                                         reinterpret_cast<const float4 *>(c->vel), c->id, pos_t, vel_t, id_t);
+    cudaMemcpyAsync(c->pos, pos_t, sizeof(float4) * (size_t)n, cudaMemcpyDeviceToDevice, st);
+    cudaMemcpyAsync(c->vel, vel_t, sizeof(float4) * (size_t)n, cudaMemcpyDeviceToDevice, st);
+    cudaMemcpyAsync(c->id, id_t, sizeof(u32) * (size_t)n, cudaMemcpyDeviceToDevice, st);
+    return cudaGetLastError();
+}
+
+}  // namespace hyb

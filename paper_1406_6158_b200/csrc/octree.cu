@@ -1,0 +1,506 @@
+// octree.cu -- steps a5-a7: linear octree in breadth-first numbering, moment upsweep with the
+// opening radius, sink groups.  (T7-T11.)
+//
+// Construction is depth-independent (a handful of launches):
+//   preorder : per particle i, the levels at which a node starts at i form the contiguous range
+//              (d(i), top(i)], d(i) = common leading 3-bit digits of key[i-1], key[i] and top(i)
+//              derived from a sliding window of leaf_max+1 keys.  A scan gives each node its
+//              preorder index.
+//   bfs      : one stable counting-sort pass by level turns preorder into breadth-first order.
+//   link     : every node finds its range end, children and parent by binary search in the keys.
+//   upsweep  : leaves first, the last child to arrive computes the parent (fixed summation order).
+#include "common.cuh"
+#include "sort.cuh"
+
+namespace hyb {
+
+__device__ __forceinline__ int lcp_levels(u64 a, u64 b)
+{
+    u64 x = a ^ b;
+    return x ? (__clzll((long long)x) - 1) / 3 : MAXLEVEL;
+}
+
+// ------------------------------------------------------------------ a5: preorder emission
+constexpr int PO_HALO = 64;
+
+__global__ void __launch_bounds__(SC_THREADS) preorder_kernel(
+    const u64 *__restrict__ key, u32 n, int leaf_max, u32 node_cap, DevCtl *ctl, u64 *sc_status,
+    signed char *__restrict__ dlev, u32 *__restrict__ slot, unsigned char *__restrict__ pre_level,
+    u32 *__restrict__ pre_first)
+{
+    __shared__ u64 s_key[SC_TILE + 2 * PO_HALO];
+    __shared__ signed char s_w[SC_TILE + PO_HALO];
+    __shared__ u32 s_hist[MAXLEVEL + 1];
+    __shared__ u32 s_warp[SC_THREADS / 32];
+    __shared__ u32 s_tile;
+    __shared__ u64 s_prefix;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const u32 ntiles = (n + SC_TILE - 1) / SC_TILE;
+    for (;;) {
+        __syncthreads();
+        if (tid == 0) s_tile = atomicAdd(&ctl->tile_counter[8], 1u);
+        if (tid <= MAXLEVEL) s_hist[tid] = 0;
+        __syncthreads();
+        const u32 tile = s_tile;
+        if (tile >= ntiles) break;
+        const long long t0 = (long long)tile * SC_TILE;
+        for (int q = tid; q < SC_TILE + 2 * PO_HALO; q += SC_THREADS) {
+            long long g = t0 - PO_HALO + q;
+            s_key[q] = (g >= 0 && g < (long long)n) ? key[g] : 0ull;
+        }
+        __syncthreads();
+        for (int q = tid; q < SC_TILE + PO_HALO; q += SC_THREADS) {       // w(s), s = t0 - HALO + q
+            long long s = t0 - PO_HALO + q;
+            int w = -1;
+            if (s >= 0 && s + leaf_max < (long long)n) w = lcp_levels(s_key[q], s_key[q + leaf_max]);
+            s_w[q] = (signed char)w;
+        }
+        __syncthreads();
+        int d[SC_IPT], cnt[SC_IPT];
+        u32 mysum = 0;
+#pragma unroll
+        for (int k = 0; k < SC_IPT; k++) {
+            const int li = tid * SC_IPT + k;                 // local index in tile
+            const long long i = t0 + li;
+            d[k] = 0; cnt[k] = 0;
+            if (i < (long long)n) {
+                d[k] = (i == 0) ? -1 : lcp_levels(s_key[PO_HALO + li - 1], s_key[PO_HALO + li]);
+                int lfull = -1;
+                for (int s = 0; s <= leaf_max; s++) lfull = max(lfull, (int)s_w[PO_HALO + li - s]);
+                int top = min(lfull + 1, MAXLEVEL);
+                cnt[k] = max(0, top - d[k]);
+            }
+            mysum += cnt[k];
+        }
+        // block exclusive scan of mysum
+        u32 incl = mysum;
+#pragma unroll
+        for (int off = 1; off < 32; off <<= 1) {
+            u32 t = __shfl_up_sync(0xFFFFFFFFu, incl, off);
+            if (lane >= off) incl += t;
+        }
+        if (lane == 31) s_warp[warp] = incl;
+        __syncthreads();
+        u32 wbase = 0, tile_total = 0;
+#pragma unroll
+        for (int w = 0; w < SC_THREADS / 32; w++) { if (w < warp) wbase += s_warp[w]; tile_total += s_warp[w]; }
+        if (tid == 0) {
+            u64 pre = lookback_single(sc_status, tile, tile_total, &ctl->status);
+            s_prefix = pre;
+            if (tile == ntiles - 1) {
+                u64 tot = pre + tile_total;
+                ctl->nn_total = (u32)min(tot, (u64)0xFFFFFFFFu);
+                ctl->nn = (u32)min(tot, (u64)node_cap);
+                if (tot > node_cap) atomicOr(&ctl->status, ST_NODE_OVERFLOW);
+            }
+        }
+        __syncthreads();
+        u64 p = s_prefix + wbase + incl - mysum;
+#pragma unroll
+        for (int k = 0; k < SC_IPT; k++) {
+            const long long i = t0 + tid * SC_IPT + k;
+            if (i < (long long)n) {
+                dlev[i] = (signed char)d[k];
+                slot[i] = (u32)min(p, (u64)0xFFFFFFFFu);
+                for (int j = 0; j < cnt[k]; j++) {
+                    if (p + j < node_cap) {
+                        pre_level[p + j] = (unsigned char)(d[k] + 1 + j);
+                        pre_first[p + j] = (u32)i;
+                    }
+                    atomicAdd(&s_hist[d[k] + 1 + j], 1u);
+                }
+                p += cnt[k];
+            }
+        }
+        __syncthreads();
+        if (tid <= MAXLEVEL && s_hist[tid]) atomicAdd(&ctl->node_hist[tid], s_hist[tid]);
+    }
+}
+
+// level_offset and the counting-sort bases (clamped to the node pool).  One warp.
+__global__ void level_offset_kernel(DevCtl *ctl)
+{
+    if (threadIdx.x == 0) {
+        // node pool overflow: the counting-sort bases would point past the pool, so drop the tree
+        // (nn = 0 makes every later stage a no-op); the status bit reports the failure.
+        if (ctl->status & ST_NODE_OVERFLOW) ctl->nn = 0;
+        u32 run = 0;
+        for (int l = 0; l <= MAXLEVEL; l++) {
+            ctl->level_offset[l] = min(run, ctl->nn);
+            ctl->node_base[l] = run;
+            run += ctl->node_hist[l];
+        }
+        ctl->level_offset[MAXLEVEL + 1] = min(run, ctl->nn);
+        for (int l = MAXLEVEL + 1; l < 256; l++) ctl->node_base[l] = run;
+    }
+}
+
+// ------------------------------------------------------------------ a5: link
+__device__ __forceinline__ u32 lower_bound_key(const u64 *__restrict__ key, u32 lo, u32 hi, u64 target)
+{
+    while (lo < hi) {           // first index in [lo,hi) with key >= target
+        u32 mid = lo + ((hi - lo) >> 1);
+        if (__ldg(key + mid) < target) lo = mid + 1; else hi = mid;
+    }
+    return lo;
+}
+
+__global__ void __launch_bounds__(256) link_kernel(
+    const u64 *__restrict__ key, u32 n, int leaf_max, const DevCtl *__restrict__ ctl,
+    const unsigned char *__restrict__ level, const u32 *__restrict__ pre_of_bfs, const u32 *__restrict__ bfs_of_pre,
+    const unsigned char *__restrict__ pre_level, const u32 *__restrict__ pre_first,
+    const signed char *__restrict__ dlev, const u32 *__restrict__ slot,
+    u32 *__restrict__ first, u32 *__restrict__ count, u32 *__restrict__ child, unsigned char *__restrict__ nchild,
+    u32 *__restrict__ parent, u32 *__restrict__ arrived, uint2 *__restrict__ meta, u64 *__restrict__ bmax2)
+{
+    const u32 nn = ctl->nn;
+    for (u32 b = blockIdx.x * blockDim.x + threadIdx.x; b < nn; b += gridDim.x * blockDim.x) {
+        const u32 p = pre_of_bfs[b];
+        const int lev = level[b];
+        const u32 f = pre_first[p];
+        const u64 k0 = __ldg(key + f);
+        const int sh = 63 - 3 * lev;
+        u32 end;
+        if (lev == 0) end = n;
+        else end = lower_bound_key(key, f, n, ((k0 >> sh) + 1ull) << sh);
+        const u32 c = end - f;
+        const bool internal = (c > (u32)leaf_max) && lev < MAXLEVEL && (p + 1 < nn);
+        u32 ch = NOCHILD, nc = 0;
+        if (internal) {
+            ch = bfs_of_pre[p + 1];
+            const int shc = sh - 3;
+            u32 pos = f;
+            while (pos < end) {
+                u64 kk = __ldg(key + pos);
+                pos = lower_bound_key(key, pos, end, ((kk >> shc) + 1ull) << shc);
+                nc++;
+            }
+        }
+        u32 par = NOCHILD;
+        if (lev > 0) {
+            const int shp = sh + 3;
+            u32 pf = (lev == 1) ? 0u : lower_bound_key(key, 0, f + 1, (k0 >> shp) << shp);
+            u32 pp = slot[pf] + (u32)(lev - 1 - ((int)dlev[pf] + 1));
+            par = bfs_of_pre[pp];
+        }
+        first[b] = f; count[b] = c; child[b] = ch; nchild[b] = (unsigned char)nc; parent[b] = par;
+        arrived[b] = 0; bmax2[b] = 0ull;
+        meta[b] = internal ? make_uint2(ch, nc) : make_uint2(f, c | 0x80000000u);
+    }
+}
+
+// ------------------------------------------------------------------ a6: upsweep (T8-T10)
+struct NodeArrays {
+    const u32 *first, *count, *child, *parent;
+    const unsigned char *nchild, *level;
+    u32 *arrived;
+    float4 *A, *B, *C;          // com_m | lo, ropen2 | hi, 0
+    double *M64, *S64, *C64, *B2;
+    u32 *leaf_of;
+};
+
+__device__ __forceinline__ double dist2_rn(double ax, double ay, double az, double bx, double by, double bz)
+{
+    double dx = __dsub_rn(ax, bx), dy = __dsub_rn(ay, by), dz = __dsub_rn(az, bz);
+    return __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz));
+}
+
+__device__ __forceinline__ void finish_node(const NodeArrays &na, u32 b, int lev, double M, double Sx, double Sy,
+                                            double Sz, float3 lo, float3 hi, int mac, float Lf, float theta,
+                                            double &Cx, double &Cy, double &Cz)
+{
+    if (M == 0.0) { Cx = (double)lo.x; Cy = (double)lo.y; Cz = (double)lo.z; }
+    else { Cx = __ddiv_rn(Sx, M); Cy = __ddiv_rn(Sy, M); Cz = __ddiv_rn(Sz, M); }
+    float ropen2 = 0.0f;
+    if (mac == HYB_MAC_THETA) {
+        float l = __fmul_rn(Lf, __uint_as_float((u32)(127 - lev) << 23));     // Lf * 2^-lev, exact
+        float r = __fdiv_rn(l, theta);
+        ropen2 = __fmul_rn(r, r);
+    }
+    na.A[b] = make_float4(__double2float_rn(Cx), __double2float_rn(Cy), __double2float_rn(Cz), __double2float_rn(M));
+    na.B[b] = make_float4(lo.x, lo.y, lo.z, ropen2);
+    na.C[b] = make_float4(hi.x, hi.y, hi.z, 0.0f);
+    na.M64[b] = M;
+    na.S64[3 * (size_t)b] = Sx; na.S64[3 * (size_t)b + 1] = Sy; na.S64[3 * (size_t)b + 2] = Sz;
+    na.C64[3 * (size_t)b] = Cx; na.C64[3 * (size_t)b + 1] = Cy; na.C64[3 * (size_t)b + 2] = Cz;
+}
+
+__global__ void __launch_bounds__(128) upsweep_kernel(NodeArrays na, const float4 *__restrict__ pos,
+                                                      const DevCtl *__restrict__ ctl, int mac, float theta)
+{
+    const u32 nn = ctl->nn;
+    const float Lf = ctl->Lf;
+    u32 b = blockIdx.x * blockDim.x + threadIdx.x;
+    if (b >= nn || na.child[b] != NOCHILD) return;
+    // ---- leaf: sequential sums over its particles, ascending (T9)
+    {
+        const u32 f = na.first[b], c = na.count[b];
+        double M = 0.0, Sx = 0.0, Sy = 0.0, Sz = 0.0;
+        float4 p0 = __ldg(pos + f);
+        float3 lo = make_float3(p0.x, p0.y, p0.z), hi = lo;
+        for (u32 j = f; j < f + c; j++) {
+            float4 p = __ldg(pos + j);
+            double m = (double)p.w;
+            M = __dadd_rn(M, m);
+            Sx = __dadd_rn(Sx, __dmul_rn(m, (double)p.x));
+            Sy = __dadd_rn(Sy, __dmul_rn(m, (double)p.y));
+            Sz = __dadd_rn(Sz, __dmul_rn(m, (double)p.z));
+            lo.x = fminf(lo.x, p.x); lo.y = fminf(lo.y, p.y); lo.z = fminf(lo.z, p.z);
+            hi.x = fmaxf(hi.x, p.x); hi.y = fmaxf(hi.y, p.y); hi.z = fmaxf(hi.z, p.z);
+            if (mac == HYB_MAC_ABS) na.leaf_of[j] = b;
+        }
+        double Cx, Cy, Cz;
+        finish_node(na, b, na.level[b], M, Sx, Sy, Sz, lo, hi, mac, Lf, theta, Cx, Cy, Cz);
+        if (mac == HYB_MAC_ABS) {
+            double B2 = 0.0;
+            for (u32 j = f; j < f + c; j++) {
+                float4 p = __ldg(pos + j);
+                double d2 = dist2_rn((double)p.x, (double)p.y, (double)p.z, Cx, Cy, Cz);
+                B2 = __dadd_rn(B2, __dmul_rn((double)p.w, d2));
+            }
+            na.B2[b] = B2;
+        }
+    }
+    // ---- climb: the last child to arrive computes the parent, children in ascending order
+    u32 cur = b;
+    for (;;) {
+        const u32 par = na.parent[cur];
+        if (par == NOCHILD) break;
+        __threadfence();
+        const u32 old = atomicAdd(&na.arrived[par], 1u);
+        const u32 nc = na.nchild[par];
+        if (old + 1 != nc) break;
+        __threadfence();
+        const u32 c0 = na.child[par];
+        double M = 0.0, Sx = 0.0, Sy = 0.0, Sz = 0.0;
+        float3 lo, hi;
+        for (u32 q = c0; q < c0 + nc; q++) {
+            M = __dadd_rn(M, __ldcg(na.M64 + q));
+            Sx = __dadd_rn(Sx, __ldcg(na.S64 + 3 * (size_t)q));
+            Sy = __dadd_rn(Sy, __ldcg(na.S64 + 3 * (size_t)q + 1));
+            Sz = __dadd_rn(Sz, __ldcg(na.S64 + 3 * (size_t)q + 2));
+            float4 bl = __ldcg(na.B + q), bh = __ldcg(na.C + q);
+            if (q == c0) { lo = make_float3(bl.x, bl.y, bl.z); hi = make_float3(bh.x, bh.y, bh.z); }
+            else {
+                lo.x = fminf(lo.x, bl.x); lo.y = fminf(lo.y, bl.y); lo.z = fminf(lo.z, bl.z);
+                hi.x = fmaxf(hi.x, bh.x); hi.y = fmaxf(hi.y, bh.y); hi.z = fmaxf(hi.z, bh.z);
+            }
+        }
+        double Cx, Cy, Cz;
+        finish_node(na, par, na.level[par], M, Sx, Sy, Sz, lo, hi, mac, Lf, theta, Cx, Cy, Cz);
+        if (mac == HYB_MAC_ABS) {            // parallel-axis sum of the children's B_2 (T10)
+            double B2 = 0.0;
+            for (u32 q = c0; q < c0 + nc; q++) {
+                double d2 = dist2_rn(__ldcg(na.C64 + 3 * (size_t)q), __ldcg(na.C64 + 3 * (size_t)q + 1),
+                                     __ldcg(na.C64 + 3 * (size_t)q + 2), Cx, Cy, Cz);
+                B2 = __dadd_rn(B2, __dadd_rn(__ldcg(na.B2 + q), __dmul_rn(__ldcg(na.M64 + q), d2)));
+            }
+            na.B2[par] = B2;
+        }
+        cur = par;
+    }
+}
+
+// exact b_max^2 (Eq. 5; R9): every particle visits its ancestors, one level per iteration so that
+// the lanes of a warp meet at the same node; bit patterns of non-negative doubles order as u64.
+__global__ void __launch_bounds__(256) bmax_kernel(const float4 *__restrict__ pos, u32 n,
+                                                   const u32 *__restrict__ leaf_of, const u32 *__restrict__ parent,
+                                                   const unsigned char *__restrict__ level,
+                                                   const double *__restrict__ C64, u64 *bmax2)
+{
+    const u32 j = blockIdx.x * blockDim.x + threadIdx.x;
+    const bool live = j < n;
+    float4 p = live ? __ldg(pos + j) : make_float4(0, 0, 0, 0);
+    u32 node = live ? leaf_of[j] : NOCHILD;
+    int nl = live ? (int)level[node] : -1;
+    for (int l = MAXLEVEL; l >= 0; --l) {
+        const bool act = (nl == l);
+        u64 bits = 0;
+        if (act) {
+            double d2 = dist2_rn((double)p.x, (double)p.y, (double)p.z, C64[3 * (size_t)node],
+                                 C64[3 * (size_t)node + 1], C64[3 * (size_t)node + 2]);
+            bits = (u64)__double_as_longlong(d2);
+        }
+        int same;
+        __match_all_sync(0xFFFFFFFFu, act ? node : NOCHILD, &same);
+        if (same) {
+            if (act) {                       // whole warp at one node
+#pragma unroll
+                for (int off = 16; off; off >>= 1) {
+                    u64 o = __shfl_xor_sync(0xFFFFFFFFu, bits, off);
+                    bits = o > bits ? o : bits;
+                }
+                if ((threadIdx.x & 31) == 0) atomicMax(bmax2 + node, bits);
+            }
+        } else if (act) atomicMax(bmax2 + node, bits);
+        if (act) { node = parent[node]; nl = l - 1; }
+    }
+}
+
+__global__ void __launch_bounds__(256) ropen_abs_kernel(const DevCtl *__restrict__ ctl, const u64 *__restrict__ bmax2,
+                                                        const double *__restrict__ B2, float a_err, float4 *nodeB)
+{
+    const u32 nn = ctl->nn;
+    const u32 b = blockIdx.x * blockDim.x + threadIdx.x;
+    if (b >= nn) return;
+    double bm = __dsqrt_rn(__longlong_as_double((long long)bmax2[b]));
+    double t3 = __dsqrt_rn(__ddiv_rn(__dmul_rn(3.0, B2[b]), (double)a_err));
+    double t5 = __ddiv_rn(__dmul_rn(bm, bm), 4.0);
+    double rb = __dadd_rn(__ddiv_rn(bm, 2.0), __dsqrt_rn(__dadd_rn(t5, t3)));
+    float r = __double2float_rn(rb);
+    nodeB[b].w = __fmul_rn(r, r);
+}
+
+// ------------------------------------------------------------------ a7: groups (T11)
+__global__ void __launch_bounds__(256) gmark_kernel(const DevCtl *__restrict__ ctl, const u32 *__restrict__ first,
+                                                    const u32 *__restrict__ count, const u32 *__restrict__ child,
+                                                    const u32 *__restrict__ parent, int group_max,
+                                                    unsigned char *gflag)
+{
+    const u32 nn = ctl->nn;
+    const u32 b = blockIdx.x * blockDim.x + threadIdx.x;
+    if (b >= nn) return;
+    const u32 c = count[b], f = first[b], gm = (u32)group_max;
+    if (c <= gm) {
+        if (b == 0 || count[parent[b]] > gm) gflag[f] = 1;
+    } else if (child[b] == NOCHILD) {
+        for (u32 s = f; s < f + c; s += gm) gflag[s] = 1;       // level-21 leaf cut into chunks
+    }
+}
+
+__global__ void __launch_bounds__(SC_THREADS) gscan_kernel(const unsigned char *__restrict__ gflag, u32 n, DevCtl *ctl,
+                                                           u64 *sc_status, u32 *__restrict__ gfirst)
+{
+    __shared__ u32 s_warp[SC_THREADS / 32];
+    __shared__ u32 s_tile;
+    __shared__ u64 s_prefix;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const u32 ntiles = (n + SC_TILE - 1) / SC_TILE;
+    for (;;) {
+        __syncthreads();
+        if (tid == 0) s_tile = atomicAdd(&ctl->tile_counter[9], 1u);
+        __syncthreads();
+        const u32 tile = s_tile;
+        if (tile >= ntiles) break;
+        const u32 i0 = tile * SC_TILE + tid * SC_IPT;
+        u32 fl[SC_IPT], mysum = 0;
+#pragma unroll
+        for (int k = 0; k < SC_IPT; k++) { fl[k] = (i0 + k < n) ? gflag[i0 + k] : 0u; mysum += fl[k]; }
+        u32 incl = mysum;
+#pragma unroll
+        for (int off = 1; off < 32; off <<= 1) {
+            u32 t = __shfl_up_sync(0xFFFFFFFFu, incl, off);
+            if (lane >= off) incl += t;
+        }
+        if (lane == 31) s_warp[warp] = incl;
+        __syncthreads();
+        u32 wbase = 0, tile_total = 0;
+#pragma unroll
+        for (int w = 0; w < SC_THREADS / 32; w++) { if (w < warp) wbase += s_warp[w]; tile_total += s_warp[w]; }
+        if (tid == 0) {
+            u64 pre = lookback_single(sc_status, tile, tile_total, &ctl->status);
+            s_prefix = pre;
+            if (tile == ntiles - 1) ctl->ng = (u32)(pre + tile_total);
+        }
+        __syncthreads();
+        u32 g = (u32)s_prefix + wbase + incl - mysum;
+#pragma unroll
+        for (int k = 0; k < SC_IPT; k++) if (fl[k]) gfirst[g++] = i0 + k;
+    }
+}
+
+__global__ void __launch_bounds__(256) ginfo_kernel(const DevCtl *__restrict__ ctl, u32 n,
+                                                    const float4 *__restrict__ pos, const u32 *__restrict__ gfirst,
+                                                    u32 *__restrict__ gcount, float4 *__restrict__ glo,
+                                                    float4 *__restrict__ ghi)
+{
+    const u32 ng = ctl->ng;
+    for (u32 g = blockIdx.x * blockDim.x + threadIdx.x; g < ng; g += gridDim.x * blockDim.x) {
+        const u32 f = gfirst[g], e = (g + 1 < ng) ? gfirst[g + 1] : n;
+        float4 p = __ldg(pos + f);
+        float3 lo = make_float3(p.x, p.y, p.z), hi = lo;
+        for (u32 j = f + 1; j < e; j++) {
+            p = __ldg(pos + j);
+            lo.x = fminf(lo.x, p.x); lo.y = fminf(lo.y, p.y); lo.z = fminf(lo.z, p.z);
+            hi.x = fmaxf(hi.x, p.x); hi.y = fmaxf(hi.y, p.y); hi.z = fmaxf(hi.z, p.z);
+        }
+        gcount[g] = e - f;
+        glo[g] = make_float4(lo.x, lo.y, lo.z, 0.0f);
+        ghi[g] = make_float4(hi.x, hi.y, hi.z, 0.0f);
+    }
+}
+
+// ------------------------------------------------------------------ host side
+cudaError_t launch_keys_sort_permute(Ctx *c);
+
+cudaError_t launch_build_tree(Ctx *c)
+{
+    const Layout &L = c->L;
+    const u32 n = (u32)c->n;
+    cudaStream_t st = c->stream;
+    DevCtl *ctl = c->ctl;
+    // reset per-build device state
+    cudaMemsetAsync(reinterpret_cast<char *>(ctl) + offsetof(DevCtl, bbox_enc), 0,
+                    offsetof(DevCtl, bbox) - offsetof(DevCtl, bbox_enc), st);
+    cudaMemsetAsync(reinterpret_cast<char *>(ctl) + offsetof(DevCtl, bbox_enc), 0xFF, 3 * sizeof(u32), st);
+    cudaMemsetAsync(c->ws + L.rs_status, 0, sizeof(u32) * 256 * (size_t)L.rs_tiles * RS_PASSES, st);
+    cudaMemsetAsync(c->ws + L.sc_status, 0, sizeof(u64) * 2 * (size_t)L.sc_tiles, st);
+    cudaMemsetAsync(c->ws + L.node_status, 0, sizeof(u32) * 256 * (size_t)L.node_tiles, st);
+    cudaMemsetAsync(c->ws + L.gflag, 0, (size_t)n, st);
+
+    cudaError_t e = launch_keys_sort_permute(c);
+    if (e != cudaSuccess) return e;
+
+    const u64 *key = wsptr<u64>(c, L.key_b);
+    u64 *sc_status = wsptr<u64>(c, L.sc_status);
+    const int sc_grid = (int)imin64(L.sc_tiles, (int64_t)c->num_sms * 8);
+    signed char *dlev = wsptr<signed char>(c, L.dlev);
+    u32 *slot = wsptr<u32>(c, L.cnt_slot);
+    unsigned char *pre_level = wsptr<unsigned char>(c, L.pre_level);
+    u32 *pre_first = wsptr<u32>(c, L.pre_first);
+    preorder_kernel<<<sc_grid, SC_THREADS, 0, st>>>(key, n, c->p.leaf_max, (u32)L.node_cap, ctl, sc_status, dlev, slot,
+                                                    pre_level, pre_first);
+    level_offset_kernel<<<1, 32, 0, st>>>(ctl);
+    unsigned char *level = wsptr<unsigned char>(c, L.level);
+    u32 *pre_of_bfs = wsptr<u32>(c, L.pre_of_bfs), *bfs_of_pre = wsptr<u32>(c, L.bfs_of_pre);
+    const int ngrid = (int)imin64(L.node_tiles, (int64_t)c->num_sms * 3);
+    e = launch_radix_pass<unsigned char>(pre_level, nullptr, level, pre_of_bfs, bfs_of_pre, 0, &ctl->nn, 0,
+                                         ctl->node_base, wsptr<u32>(c, L.node_status), &ctl->tile_counter[10],
+                                         &ctl->status, ngrid, st);
+    if (e != cudaSuccess) return e;
+
+    u32 *first = wsptr<u32>(c, L.first), *count = wsptr<u32>(c, L.count), *child = wsptr<u32>(c, L.child);
+    u32 *parent = wsptr<u32>(c, L.parent), *arrived = wsptr<u32>(c, L.arrived);
+    unsigned char *nchild = wsptr<unsigned char>(c, L.nchild);
+    uint2 *meta = wsptr<uint2>(c, L.meta);
+    u64 *bmax2 = wsptr<u64>(c, L.bmax2);
+    const int node_grid = (int)imin64((L.node_cap + 255) / 256, (int64_t)c->num_sms * 16);
+    link_kernel<<<node_grid, 256, 0, st>>>(key, n, c->p.leaf_max, ctl, level, pre_of_bfs, bfs_of_pre, pre_level,
+                                           pre_first, dlev, slot, first, count, child, nchild, parent, arrived, meta,
+                                           bmax2);
+    NodeArrays na;
+    na.first = first; na.count = count; na.child = child; na.parent = parent; na.nchild = nchild; na.level = level;
+    na.arrived = arrived;
+    na.A = wsptr<float4>(c, L.nodeA); na.B = wsptr<float4>(c, L.nodeB); na.C = wsptr<float4>(c, L.nodeC);
+    na.M64 = wsptr<double>(c, L.M64); na.S64 = wsptr<double>(c, L.S64); na.C64 = wsptr<double>(c, L.C64);
+    na.B2 = wsptr<double>(c, L.B2); na.leaf_of = wsptr<u32>(c, L.leaf_of);
+    const int full_node_grid = (int)((L.node_cap + 127) / 128);
+    upsweep_kernel<<<full_node_grid, 128, 0, st>>>(na, reinterpret_cast<const float4 *>(c->pos), ctl, c->p.mac,
+                                                   c->p.theta);
+    if (c->p.mac == HYB_MAC_ABS) {
+        bmax_kernel<<<(n + 255) / 256, 256, 0, st>>>(reinterpret_cast<const float4 *>(c->pos), n, na.leaf_of, parent,
+                                                     level, na.C64, bmax2);
+        ropen_abs_kernel<<<(int)((L.node_cap + 255) / 256), 256, 0, st>>>(ctl, bmax2, na.B2, c->p.a_err, na.B);
+    }
+    unsigned char *gflag = wsptr<unsigned char>(c, L.gflag);
+    gmark_kernel<<<(int)((L.node_cap + 255) / 256), 256, 0, st>>>(ctl, first, count, child, parent, c->p.group_max,
+                                                                  gflag);
+    u32 *gfirst = wsptr<u32>(c, L.gfirst);
+    gscan_kernel<<<sc_grid, SC_THREADS, 0, st>>>(gflag, n, ctl, sc_status + L.sc_tiles, gfirst);
+    ginfo_kernel<<<(int)imin64((c->n + 255) / 256, (int64_t)c->num_sms * 8), 256, 0, st>>>(
+        ctl, n, reinterpret_cast<const float4 *>(c->pos), gfirst, wsptr<u32>(c, L.gcount), wsptr<float4>(c, L.glo),
+        wsptr<float4>(c, L.ghi));
+    return cudaGetLastError();
+}
+
+}  // namespace hyb

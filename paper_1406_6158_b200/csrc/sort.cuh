@@ -1,0 +1,157 @@
+// sort.cuh -- one pass of a stable least-significant-digit radix sort, "onesweep" style:
+// every tile ranks its keys locally and obtains the global offset of each of its 256 digit
+// buckets by decoupled look-back over the tiles before it, so keys are read once and written
+// once per pass.  Stability (ties keep input order, T6) holds because the local rank
+// is taken in input order and tile prefixes follow tile order.
+#pragma once
+#include "common.cuh"
+
+namespace hyb {
+
+constexpr u32 RS_FLAG_AGG = 1u << 30, RS_FLAG_PREFIX = 2u << 30, RS_VALUE_MASK = (1u << 30) - 1;
+
+struct RadixSmem {
+    u64 keys[RS_TILE];
+    u32 vals[RS_TILE];
+    u32 warp_cnt[RS_THREADS / 32][256];
+    u32 digit_start[256];
+    u32 global_off[256];
+    u32 scan_tmp[8];
+    u32 tile;
+};
+
+// n_dev (optional) overrides n with a device-side count (tree nodes).
+// vin == nullptr: values are the global input indices (first pass).
+// inv_out (optional): inv_out[value] = output position (the inverse permutation).
+template <typename KeyT>
+__global__ void __launch_bounds__(RS_THREADS) radix_pass_kernel(
+    const KeyT *__restrict__ kin, const u32 *__restrict__ vin, KeyT *__restrict__ kout, u32 *__restrict__ vout,
+    u32 *__restrict__ inv_out, u32 n_host, const u32 *__restrict__ n_dev, int shift,
+    const u32 *__restrict__ digit_base, u32 *status, u32 *tile_counter, u32 *dev_status)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    RadixSmem &sm = *reinterpret_cast<RadixSmem *>(smem_raw);
+    const u32 n = n_dev ? *n_dev : n_host;
+    const u32 ntiles = (n + RS_TILE - 1) / RS_TILE;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const u32 lt_mask = (1u << lane) - 1u;
+
+    for (;;) {
+        __syncthreads();   // previous iteration's smem is dead
+        if (tid == 0) sm.tile = atomicAdd(tile_counter, 1u);
+        for (int i = tid; i < (RS_THREADS / 32) * 256; i += RS_THREADS) (&sm.warp_cnt[0][0])[i] = 0;
+        __syncthreads();
+        const u32 tile = sm.tile;
+        if (tile >= ntiles) break;
+        const u32 base = tile * RS_TILE + warp * (32 * RS_KPT);
+        const u32 tile_n = min((u32)RS_TILE, n - tile * RS_TILE);
+
+        KeyT key[RS_KPT];
+        u32 val[RS_KPT];
+        u32 rank[RS_KPT];
+#pragma unroll
+        for (int k = 0; k < RS_KPT; k++) {
+            u32 idx = base + k * 32 + lane;
+            bool ok = idx < n;
+            key[k] = ok ? kin[idx] : (KeyT)0;
+            val[k] = ok ? (vin ? vin[idx] : idx) : 0xFFFFFFFFu;
+        }
+        // stable rank of every key among the keys of this warp with the same digit
+#pragma unroll
+        for (int k = 0; k < RS_KPT; k++) {
+            u32 idx = base + k * 32 + lane;
+            bool ok = idx < n;
+            u32 d = ok ? (u32)((key[k] >> shift) & 0xFF) : 256u;
+            u32 peers = __match_any_sync(0xFFFFFFFFu, d);
+            u32 c = ok ? sm.warp_cnt[warp][d] : 0u;
+            __syncwarp();
+            rank[k] = c + __popc(peers & lt_mask);
+            if (ok && (peers & lt_mask) == 0) sm.warp_cnt[warp][d] = c + __popc(peers);
+            __syncwarp();
+        }
+        __syncthreads();
+        // thread d: exclusive scan of digit d over the warps, tile total
+        u32 total = 0;
+#pragma unroll
+        for (int w = 0; w < RS_THREADS / 32; w++) {
+            u32 t = sm.warp_cnt[w][tid];
+            sm.warp_cnt[w][tid] = total;
+            total += t;
+        }
+        // publish + look back (thread d for digit d)
+        u32 excl = 0;
+        {
+            volatile u32 *st = status;
+            const size_t me = (size_t)tile * 256 + tid;
+            if (tile == 0) st[me] = RS_FLAG_PREFIX | total;
+            else {
+                st[me] = RS_FLAG_AGG | total;
+                for (long long t = (long long)tile - 1; t >= 0; --t) {
+                    u32 s; int spins = 0;
+                    do { s = st[(size_t)t * 256 + tid]; } while ((s >> 30) == 0 && ++spins < LB_SPIN_LIMIT);
+                    if ((s >> 30) == 0) { atomicOr(dev_status, ST_WAIT_EXPIRED); break; }
+                    excl += s & RS_VALUE_MASK;
+                    if ((s >> 30) == 2) break;
+                }
+                st[me] = RS_FLAG_PREFIX | (excl + total);
+            }
+        }
+        // block exclusive scan of the digit totals -> digit_start
+        u32 incl = total;
+#pragma unroll
+        for (int off = 1; off < 32; off <<= 1) {
+            u32 t = __shfl_up_sync(0xFFFFFFFFu, incl, off);
+            if (lane >= off) incl += t;
+        }
+        if (lane == 31) sm.scan_tmp[warp] = incl;
+        __syncthreads();
+        u32 wbase = 0;
+#pragma unroll
+        for (int w = 0; w < RS_THREADS / 32; w++) wbase += (w < warp) ? sm.scan_tmp[w] : 0u;
+        const u32 dstart = wbase + incl - total;
+        sm.digit_start[tid] = dstart;
+        sm.global_off[tid] = digit_base[tid] + excl - dstart;
+        __syncthreads();
+        // scatter into shared memory in sorted-by-digit order
+#pragma unroll
+        for (int k = 0; k < RS_KPT; k++) {
+            u32 idx = base + k * 32 + lane;
+            if (idx < n) {
+                u32 d = (u32)((key[k] >> shift) & 0xFF);
+                u32 lp = sm.digit_start[d] + sm.warp_cnt[warp][d] + rank[k];
+                reinterpret_cast<KeyT *>(sm.keys)[lp] = key[k];
+                sm.vals[lp] = val[k];
+            }
+        }
+        __syncthreads();
+        for (u32 i = tid; i < tile_n; i += RS_THREADS) {
+            KeyT k = reinterpret_cast<KeyT *>(sm.keys)[i];
+            u32 d = (u32)((k >> shift) & 0xFF);
+            u32 g = sm.global_off[d] + i;
+            kout[g] = k;
+            u32 v = sm.vals[i];
+            vout[g] = v;
+            if (inv_out) inv_out[v] = g;
+        }
+    }
+}
+
+template <typename KeyT>
+static cudaError_t launch_radix_pass(const KeyT *kin, const u32 *vin, KeyT *kout, u32 *vout, u32 *inv_out, u32 n_host,
+                                     const u32 *n_dev, int shift, const u32 *digit_base, u32 *status,
+                                     u32 *tile_counter, u32 *dev_status, int grid, cudaStream_t st)
+{
+    static bool attr_set = false;
+    if (!attr_set) {
+        cudaError_t e = cudaFuncSetAttribute(radix_pass_kernel<KeyT>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                             (int)sizeof(RadixSmem));
+        if (e != cudaSuccess) return e;
+        attr_set = true;
+    }
+    radix_pass_kernel<KeyT><<<grid, RS_THREADS, sizeof(RadixSmem), st>>>(kin, vin, kout, vout, inv_out, n_host, n_dev,
+                                                                         shift, digit_base, status, tile_counter,
+                                                                         dev_status);
+    return cudaGetLastError();
+}
+
+}  // namespace hyb

@@ -1,0 +1,70 @@
+"""-m gpu: the CUDA path (through the C-ABI) against the oracle, stage by stage."""
+import numpy as np
+import pytest
+
+from oracle import oracle as O
+from workloads import CONFIGS, make_ic
+
+pytestmark = pytest.mark.gpu
+
+from gpu_util import check_forces, compare_tree, make_hyb  # noqa: E402
+
+
+def _run_case(cfg, pos, vel, **over):
+    h = make_hyb(cfg, pos, vel, **over)
+    h.build_tree()
+    h.sync()
+    t = O.Tree(pos, O.params_from(cfg, **over))
+    compare_tree(h, t, abs_mode=over.get("mac", cfg.mac) == 1)
+    res = check_forces(h, t, split=over.get("split", cfg.split) == 1)
+    h.close()
+    return res
+
+
+@pytest.mark.parametrize("mac", [0, 1])
+def test_cfg0_all_stages(mac):
+    cfg = CONFIGS[0]
+    pos, vel = make_ic(cfg.kind, cfg.n, cfg.seed)
+    print(_run_case(cfg, pos, vel, mac=mac))
+
+
+def test_cfg0_normal_tree():
+    cfg = CONFIGS[0]
+    pos, vel = make_ic(cfg.kind, cfg.n, cfg.seed)
+    print(_run_case(cfg, pos, vel, split=0))
+
+
+@pytest.mark.parametrize("n,kind,leaf,group", [(20011, "plummer", 16, 64), (9973, "hernquist", 8, 32),
+                                               (33333, "cold_sphere", 16, 64), (5000, "two_plummer", 1, 1),
+                                               (1, "cold_sphere", 8, 32), (2, "cold_sphere", 8, 32),
+                                               (37, "plummer", 8, 32)])
+def test_ragged_sizes(n, kind, leaf, group):
+    cfg = CONFIGS[1].with_(n=n, kind=kind, leaf_max=leaf, group_max=group)
+    pos, vel = make_ic(kind, n, 17)
+    print(_run_case(cfg, pos, vel))
+
+
+def test_coincident_points_and_depth_limit():
+    cfg = CONFIGS[0].with_(leaf_max=4, group_max=8)
+    rng = np.random.default_rng(2)
+    pos = np.zeros((3000, 4), np.float32)
+    pos[:, :3] = rng.normal(size=(3000, 3))
+    pos[100:400, :3] = pos[100, :3]                # 300 coincident points -> level-21 leaf, chunked groups
+    pos[500:520, :3] = pos[500, :3]
+    pos[:, 3] = 1.0 / 3000
+    vel = np.zeros_like(pos)
+    print(_run_case(cfg, pos, vel))
+
+
+def test_theta_zero_opens_everything():
+    cfg = CONFIGS[0].with_(n=1500, theta=0.0)
+    pos, vel = make_ic("plummer", 1500, 3)
+    h = make_hyb(cfg, pos, vel)
+    h.build_tree(); h.soft_force(); h.sync()
+    assert np.all(h.export("ncell") == 0) and np.all(h.export("npart") == 1500)
+    at, ah, as_ = O.direct(pos, cfg.G, cfg.eps, cfg.r_in, cfg.r_out)
+    perm = h.export("perm")
+    tot = (h.a_soft + h.a_hard).cpu().numpy()[:, :3]
+    err = np.linalg.norm(tot - at[perm], axis=1) / np.linalg.norm(at[perm], axis=1)
+    assert err.max() < 1e-4 and np.sqrt(np.mean(err ** 2)) < 1e-5
+    h.close()
