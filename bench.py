@@ -1,0 +1,248 @@
+#!/usr/bin/env python
+"""bench.py -- one JSON line for the hybrid tree force path.
+
+A "step" is one soft cycle Delta t_s of the whole hot path on BASELINE.json's N = 2^20 workload
+(configs[2]: Hernquist sphere): n tree builds, one fused soft+hard walk, n-1 hard walks, kick/drift.
+metric = pairwise interactions evaluated per second (sum over groups of members x list length).
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config I]
+
+N > 1 runs under torchrun, one independent replica per rank (the path does not shard: "replicas
+only"); value is the whole-job aggregate over ranks, time the max over ranks.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+# flop conventions: monopole pair 23 (north_star), K-weighted pairs from the
+# instruction list of walk.cu: fused soft+hard pair 43, hard-only pair 36.
+FLOP_MONO, FLOP_KFUSED, FLOP_KHARD = 23.0, 43.0, 36.0
+N_SM, FP32_LANES = 148, 128          # B200: guide's unit counts
+
+
+def clock_sampler(stop, out, index):
+    """sample SM clock and throttle reasons with NVML while the timed region runs"""
+    try:
+        import pynvml as nv
+        nv.nvmlInit()
+        h = nv.nvmlDeviceGetHandleByIndex(index)
+        out["sm_max_mhz"] = nv.nvmlDeviceGetMaxClockInfo(h, nv.NVML_CLOCK_SM)
+        names = {nv.nvmlClocksThrottleReasonSwPowerCap: "sw_power_cap",
+                 nv.nvmlClocksThrottleReasonHwSlowdown: "hw_slowdown",
+                 nv.nvmlClocksThrottleReasonSwThermalSlowdown: "sw_thermal_slowdown",
+                 nv.nvmlClocksThrottleReasonHwThermalSlowdown: "hw_thermal_slowdown",
+                 nv.nvmlClocksThrottleReasonHwPowerBrakeSlowdown: "hw_power_brake"}
+        while not stop.is_set():
+            out["samples"].append(nv.nvmlDeviceGetClockInfo(h, nv.NVML_CLOCK_SM))
+            r = nv.nvmlDeviceGetCurrentClocksThrottleReasons(h)
+            for bit, nm in names.items():
+                if r & bit:
+                    out["reasons"].add(nm)
+            time.sleep(0.002)
+    except Exception as e:  # noqa: BLE001
+        out["error"] = repr(e)
+
+
+def oracle_sample(cfg, pos, seconds):
+    """times the oracle (as it stands) on a bounded sample of the workload: full tree build, then
+    the fused soft+hard force evaluation on evenly spaced sink groups for about `seconds`."""
+    import numpy as np
+    from oracle import oracle as O
+    P = O.params_from(cfg)
+    t0 = time.perf_counter()
+    tree = O.Tree(pos, P)
+    t_build = time.perf_counter() - t0
+    probe = np.linspace(0, tree.ng - 1, num=min(tree.ng, 256)).astype(np.int64)
+    t0 = time.perf_counter()
+    _, _, inter = tree.forces(O.MODE_HYBRID, probe)
+    t_probe = time.perf_counter() - t0
+    want = int(min(tree.ng, max(256, len(probe) * seconds / max(t_probe, 1e-6))))
+    gsel = np.unique(np.linspace(0, tree.ng - 1, num=want).astype(np.int64))
+    reps = 0
+    n_inter = 0.0
+    t0 = time.perf_counter()
+    while True:
+        _, _, inter = tree.forces(O.MODE_HYBRID, gsel)
+        n_inter += inter[0] + inter[1]
+        reps += 1
+        dt = time.perf_counter() - t0
+        if dt >= 0.8 * seconds or reps >= 64:
+            break
+    return {"value": n_inter / dt, "unit": "interactions/s", "cores": O.num_threads(), "kind": "oracle",
+            "sample": f"{reps} x fp64 soft+hard force evaluation on {len(gsel)} of {tree.ng} sink groups "
+                      f"({n_inter:.3e} interactions in {dt:.2f} s; full tree build {t_build:.2f} s not included)"}, \
+        (tree, gsel, n_inter, dt)
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=2)
+    ap.add_argument("--cpu-seconds", type=float, default=12.0)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer leg (profiling runs)")
+    args = ap.parse_args()
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+
+    from workloads import CONFIGS, make_ic
+    cfg = CONFIGS[args.config]
+    config = {"workload": f"{cfg.name}: {cfg.kind} N={cfg.n}, eps={cfg.eps}, theta={cfg.theta}, leaf<={cfg.leaf_max}, "
+                          f"group<={cfg.group_max}, r_in={cfg.r_in}, r_out={cfg.r_out}, dt_soft=1/{round(1 / cfg.dt_soft)}, "
+                          f"n_sub={cfg.n_sub}, seed {cfg.seed}",
+              "step": "one soft cycle: n_sub tree builds + 1 fused soft/hard walk + (n_sub-1) hard walks + kick/drift",
+              "l2": "256 MiB L2 flush between timed steps", "replicas": world}
+
+    if args.impl == "reference":
+        # the oracle, as it stands, on the host cores; rank 0 only
+        if rank != 0:
+            return
+        pos, vel = make_ic(cfg.kind, cfg.n, cfg.seed)
+        per_step = max(1.0, min(args.cpu_seconds, 120.0 / max(1, args.steps + args.warmup)))
+        cb, (tree, gsel, _, _) = oracle_sample(cfg, pos, per_step)
+        from oracle import oracle as O
+        times, inters = [], []
+        for i in range(args.warmup + args.steps):
+            t0 = time.perf_counter()
+            _, _, inter = tree.forces(O.MODE_HYBRID, gsel)
+            dt = time.perf_counter() - t0
+            if i >= args.warmup:
+                times.append(dt); inters.append(inter[0] + inter[1])
+        value = sum(inters) / sum(times)
+        cb["value"] = value
+        print(json.dumps({"impl": "reference", "metric": "interactions/s", "value": value, "unit": "interactions/s",
+                          "n_gpus": 0, "steps": args.steps, "warmup": args.warmup,
+                          "ms_per_step": 1e3 * sum(times) / len(times), "higher_is_better": True, "scaling": "weak",
+                          "vs_baseline": None, "dtype": "f64", "data": "synthetic", "config": config,
+                          "cpu_baseline": cb,
+                          "e2e": {"value": value, "unit": "interactions/s", "h2d_bytes_per_step": 0,
+                                  "d2h_bytes_per_step": 0}, "gpu_launches": 0}))
+        return
+
+    import numpy as np
+    import torch
+    import torch.distributed as dist
+    from paper_1406_6158_b200 import Hyb, HybParams, hyb_run_host
+
+    torch.cuda.set_device(local_rank)
+    if world > 1:
+        dist.init_process_group("nccl")
+    pos, vel = make_ic(cfg.kind, cfg.n, cfg.seed + rank)       # independent replica per rank
+    P = HybParams.from_config(cfg)
+    dpos = torch.from_numpy(pos).cuda(); dvel = torch.from_numpy(vel).cuda()
+    h = Hyb(P, dpos, dvel)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
+    h.step(0)                                                   # initial tree + forces (not a timed step)
+    for _ in range(args.warmup):
+        h.step(1)
+    h.export("interactions"); h.export("timings")
+    launches0 = int(h.export("counts")[6])
+
+    clk = {"samples": [], "reasons": set()}
+    stop = threading.Event()
+    th = threading.Thread(target=clock_sampler, args=(stop, clk, local_rank), daemon=True)
+    th.start()
+    if world > 1:
+        dist.barrier()
+    torch.cuda.synchronize()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    for a, b in ev:
+        flush.zero_()                                           # L2 flush, outside the event pair
+        a.record()
+        h.step(1)
+        b.record()
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    stop.set(); th.join()
+    total_ms = sum(a.elapsed_time(b) for a, b in ev)
+    inter = h.export("interactions").astype(np.float64)
+    stage = h.export("timings").astype(np.float64)
+    launches = int(h.export("counts")[6]) - launches0
+    t = torch.tensor([total_ms], dtype=torch.float64, device="cuda")
+    tot_inter = torch.tensor([inter.sum()], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        dist.all_reduce(tot_inter, op=dist.ReduceOp.SUM)
+    total_ms = float(t.item())
+    value = float(tot_inter.item()) / (total_ms * 1e-3)
+
+    # ---- roofline of the dominant kernel (the fused soft+hard group walk), rank 0's numbers
+    K = args.steps
+    soft_ms = stage[1] / K                                       # one launch per step
+    fused_hard = inter[1] / cfg.n_sub                           # hard pairs evaluated inside the soft-step walk
+    mono = inter[0] - fused_hard                                # plain monopole pairs (cells + far particles)
+    flops = (FLOP_MONO * mono + FLOP_KFUSED * fused_hard) / K
+    sm = sorted(clk["samples"])
+    sm_mhz = sm[len(sm) // 2] if sm else None
+    sm_max = clk.get("sm_max_mhz", 1965)
+    peak = N_SM * FP32_LANES * 2 * sm_max * 1e6 / 1e12
+    traffic = None
+    tpath = os.path.join(ROOT, "profiles", "traffic.json")
+    if os.path.exists(tpath):
+        traffic = json.load(open(tpath)).get("walk_hybrid_dram_bytes_per_launch")
+    achieved = flops / (soft_ms * 1e-3) / 1e12
+    roofline = {"bound": "alu", "kernel": "walk_kernel<HYBRID> (fused soft+hard group walk)", "achieved": achieved,
+                "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak, "traffic": traffic,
+                "peak_source": f"derived: {N_SM} SMs x {FP32_LANES} FP32 lanes x 2 flop x {sm_max} MHz max SM clock "
+                               "(MEASURED_PEAKS.json has no FP32 CUDA-core figure)",
+                "frac_at_sampled_clock": (achieved / (N_SM * FP32_LANES * 2 * sm_mhz * 1e6 / 1e12)) if sm_mhz else None,
+                "interactions_per_s": (mono + fused_hard) / K / (soft_ms * 1e-3),
+                "flop_per_pair": {"monopole": FLOP_MONO, "k_fused": FLOP_KFUSED, "k_hard": FLOP_KHARD},
+                "hard_walk": {"interactions_per_s": (inter[1] - fused_hard) / max(stage[2] * 1e-3, 1e-12),
+                              "tflops": FLOP_KHARD * (inter[1] - fused_hard) / max(stage[2] * 1e-3, 1e-12) / 1e12}}
+    stages = {"build_ms": stage[0] / K, "soft_ms": soft_ms, "hard_ms": stage[2] / K, "integrate_ms": stage[3] / K}
+
+    # ---- end to end through the C-ABI with HOST buffers (pinned), copies inside the timed region
+    e2e = None
+    if rank == 0 and not args.no_e2e:
+        hp = torch.from_numpy(pos).pin_memory(); hv = torch.from_numpy(vel).pin_memory()
+        hid = torch.arange(cfg.n, dtype=torch.int32).pin_memory()
+        p0, v0 = hp.clone(), hv.clone()
+        e_int, e_t = 0.0, 0.0
+        for i in range(2 + 3):
+            hp.copy_(p0); hv.copy_(v0)
+            t0 = time.perf_counter()
+            _, _, it = hyb_run_host(P, hp.numpy(), hv.numpy(), hid.numpy(), 1, local_rank)
+            dt = time.perf_counter() - t0
+            if i >= 2:
+                e_int += float(it.sum()); e_t += dt
+        n = cfg.n
+        e2e = {"value": e_int / e_t, "unit": "interactions/s", "h2d_bytes_per_step": 36 * n,
+               "d2h_bytes_per_step": 68 * n, "ms_per_call": 1e3 * e_t / 3,
+               "what": "hyb_run_host: upload pos/vel/id, initial tree+forces, one soft cycle, download "
+                       "pos/vel/id/a_soft/a_hard; device alloc/free inside"}
+
+    cpu_baseline = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        cpu_baseline, _ = oracle_sample(cfg, pos, args.cpu_seconds)
+
+    if rank == 0:
+        print(json.dumps({
+            "metric": "interactions/s", "value": value, "unit": "interactions/s", "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": total_ms / K, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f32", "data": "synthetic", "config": config, "stages": stages,
+            "interactions_per_step": {"soft": inter[0] / K, "hard": inter[1] / K},
+            "roofline": roofline, "cpu_baseline": cpu_baseline, "e2e": e2e, "gpu_launches": launches,
+            "clocks": {"sm_mhz": sm_mhz, "sm_max_mhz": sm_max, "reasons": sorted(clk["reasons"]),
+                       "samples": len(sm), **({"error": clk["error"]} if "error" in clk else {})}}))
+    h.close()
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

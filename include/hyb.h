@@ -65,7 +65,8 @@ enum {
  * with HYB_X_COUNTS first).  All arrays refer to the store order after the last
  * hyb_build_tree (Morton order). */
 enum {
-    HYB_X_COUNTS = 0,      /* int64[8]: n, nn, ng, node_cap, status_bits, 0, 0, 0               */
+    HYB_X_COUNTS = 0,      /* int64[8]: n, nn, ng, node_cap, status bits, nodes before clamping,
+                              kernels launched since hyb_init, 0                                */
     HYB_X_KEYS_SORTED = 1, /* uint64[n]  63-bit Morton keys, ascending                          */
     HYB_X_PERM = 2,        /* uint32[n]  perm[j] = index, in the order the build found the
                               store in, of the particle now in slot j (stable sort)            */
@@ -105,7 +106,7 @@ size_t hyb_workspace_bytes(int64_t n, const hyb_params *params);
 
 /* Create a context.
  *  params          host pointer; copied.
- *  n               number of particles, 1 <= n < 2^31.
+ *  n               number of particles, 1 <= n < 2^30.
  *  d_pos_m         DEVICE float4[n], in/out: positions and masses.  Re-ordered
  *                  into Morton order by every tree build, advanced by hyb_step.
  *  d_vel           DEVICE float4[n], in/out: velocities, re-ordered with the positions.

@@ -96,6 +96,9 @@ static int do_build(Ctx *c)
     if (e != cudaSuccess) return cuda_fail(c, e, "build_tree");
     c->tree_valid = true;
     c->acc_valid = false;
+    // bbox, root cube, keys, digit bases, 8 sort passes, permute | preorder, level offsets, level sort,
+    // link, upsweep, group mark / scan / info (+ b_max, r_b in absolute-MAC mode)
+    c->launches += 13 + 8 + (c->p.mac == HYB_MAC_ABS ? 2 : 0);
     return HYB_OK;
 }
 
@@ -103,6 +106,7 @@ static int do_soft(Ctx *c)
 {
     cudaError_t e = launch_walk(c, c->p.split ? WALK_HYBRID : WALK_NORMAL);
     if (e != cudaSuccess) return cuda_fail(c, e, "soft walk");
+    c->launches += 1;
     return HYB_OK;
 }
 
@@ -110,6 +114,7 @@ static int do_hard(Ctx *c)
 {
     cudaError_t e = c->p.split ? launch_walk(c, WALK_HARD) : launch_zero_acc(c, c->a_hard);
     if (e != cudaSuccess) return cuda_fail(c, e, "hard walk");
+    c->launches += 1;
     return HYB_OK;
 }
 
@@ -252,6 +257,7 @@ int hyb_step(hyb_ctx *ctx, int32_t n_soft_steps)
             if (split) e = launch_kick_drift(c, k == nsub - 1 ? 0.5f * dts : 0.0f, 0.5f * dth, 0.0f);
             else e = launch_kick_drift(c, 0.5f * dth, 0.0f, 0.0f);
             if (e != cudaSuccess) return cuda_fail(c, e, "kick");
+            c->launches += 2;
             if (c->timing) {
                 cudaEvent_t e4 = ev();
                 segs.push_back({3, e0, e1}); segs.push_back({0, e1, e2});
@@ -284,7 +290,7 @@ int hyb_export(hyb_ctx *ctx, int32_t what, void *host_dst, size_t bytes, size_t 
     std::vector<char> tmp;
     switch (what) {
     case HYB_X_COUNTS: {
-        int64_t v[8] = {(int64_t)n, (int64_t)nn, (int64_t)ng, L.node_cap, (int64_t)h.status, (int64_t)h.nn_total, 0, 0};
+        int64_t v[8] = {(int64_t)n, (int64_t)nn, (int64_t)ng, L.node_cap, (int64_t)h.status, (int64_t)h.nn_total, (int64_t)c->launches, 0};
         if (bytes < sizeof v) return fail(c, HYB_ERR_INVALID_ARG, "buffer too small");
         memcpy(host_dst, v, sizeof v); if (written) *written = sizeof v; return HYB_OK; }
     case HYB_X_LEVEL_OFFSET:

@@ -103,6 +103,7 @@ struct Ctx {
     cudaEvent_t ev[5];
     float t_acc[8];
     bool timing;
+    unsigned long long launches;   // kernels launched since hyb_init
     char err[256];
     // typed views of the workspace
     DevCtl *ctl;
