@@ -106,7 +106,7 @@ size_t hyb_workspace_bytes(int64_t n, const hyb_params *params);
 
 /* Create a context.
  *  params          host pointer; copied.
- *  n               number of particles, 1 <= n < 2^30.
+ *  n               number of particles, 1 <= n <= 2^28 - 2048 (tree node indices are 29-bit).
  *  d_pos_m         DEVICE float4[n], in/out: positions and masses.  Re-ordered
  *                  into Morton order by every tree build, advanced by hyb_step.
  *  d_vel           DEVICE float4[n], in/out: velocities, re-ordered with the positions.

@@ -24,7 +24,6 @@ Layout plan_workspace(int64_t n)
     L.rs_tiles = (n + RS_TILE - 1) / RS_TILE;
     L.node_tiles = (L.node_cap + RS_TILE - 1) / RS_TILE;
     L.sc_tiles = (n + SC_TILE - 1) / SC_TILE;
-    L.n_walk_warps = 148 * 4 * WK_WARPS;
     size_t off = 0;
     auto take = [&](size_t bytes) { size_t o = off; off = align_up(off + bytes); return o; };
     const size_t N = (size_t)n, NC = (size_t)L.node_cap, GC = (size_t)L.group_cap;
@@ -44,7 +43,6 @@ Layout plan_workspace(int64_t n)
     L.leaf_of = take(4 * N);
     L.gfirst = take(4 * GC); L.gcount = take(4 * GC); L.glo = take(16 * GC); L.ghi = take(16 * GC);
     L.ncell = take(4 * GC); L.npart = take(4 * GC); L.nhard = take(4 * GC);
-    L.stacks = take(4 * (size_t)L.n_walk_warps * WK_STACK_CAP);
     L.total = off;
     return L;
 }
@@ -53,7 +51,7 @@ static bool params_ok(const hyb_params *p, int64_t n, char *msg)
 {
     auto bad = [&](const char *m) { snprintf(msg, 256, "%s", m); return false; };
     if (!p) return bad("params is NULL");
-    if (n < 1 || n >= (1ll << 30)) return bad("n must be in [1, 2^30)");
+    if (n < 1 || node_capacity(n) > (1ll << 29)) return bad("n must be in [1, 2^28 - 2048]");
     if (!(p->eps > 0.0f) || !isfinite(p->eps)) return bad("eps must be finite and > 0");
     if (!isfinite(p->G)) return bad("G must be finite");
     if (p->n_sub < 1) return bad("n_sub must be >= 1");

@@ -37,7 +37,6 @@ constexpr int SC_TILE = SC_THREADS * SC_IPT;
 constexpr int WK_WARPS = 8;              // warps per CTA
 constexpr int WK_CELL_CAP = 256;         // monopole buffer entries per warp
 constexpr int WK_PART_CAP = 128;         // K-weighted (near) particle buffer entries per warp
-constexpr int WK_STACK_CAP = 8192;       // traversal stack entries per warp (global memory)
 
 enum WalkMode { WALK_HYBRID = 0, WALK_HARD = 1, WALK_NORMAL = 2 };
 
@@ -78,11 +77,9 @@ struct Layout {   // byte offsets into the workspace; computed by plan_workspace
     size_t M64, S64, C64, B2, bmax2;           // double[nc], [3nc], [3nc], [nc], u64[nc]
     size_t leaf_of;             // u32[n]
     size_t gfirst, gcount, glo, ghi, ncell, npart, nhard;   // [group_cap]
-    size_t stacks;              // [n_walk_warps][WK_STACK_CAP] u32
     size_t total;
     int64_t n, node_cap, group_cap;
     int64_t rs_tiles, node_tiles, sc_tiles;
-    int n_walk_warps;
 };
 
 inline int64_t node_capacity(int64_t n) { return 2 * n + 4096; }
