@@ -1,6 +1,7 @@
 // api.cu -- the C-ABI of include/hyb.h: argument checks, workspace carving, step driver, export.
 #include <math.h>
 #include <stdio.h>
+#include <stddef.h>
 #include <string.h>
 
 #include <new>
@@ -38,7 +39,7 @@ Layout plan_workspace(int64_t n)
     L.node_status = take(4 * 256 * (size_t)L.node_tiles);
     L.level = take(NC); L.first = take(4 * NC); L.count = take(4 * NC); L.child = take(4 * NC);
     L.nchild = take(NC); L.parent = take(4 * NC); L.arrived = take(4 * NC);
-    L.nodeA = take(16 * NC); L.nodeB = take(16 * NC); L.nodeC = take(16 * NC); L.meta = take(8 * NC);
+    L.nodes = take(sizeof(NodeRec) * NC);
     L.M64 = take(8 * NC); L.S64 = take(24 * NC); L.C64 = take(24 * NC); L.B2 = take(8 * NC); L.bmax2 = take(8 * NC);
     L.leaf_of = take(4 * N);
     L.gfirst = take(4 * GC); L.gcount = take(4 * GC); L.glo = take(16 * GC); L.ghi = take(16 * GC);
@@ -317,16 +318,16 @@ int hyb_export(hyb_ctx *ctx, int32_t what, void *host_dst, size_t bytes, size_t 
     case HYB_X_CHILD: src = c->ws + L.child; sz = 4 * nn; break;
     case HYB_X_NCHILD: src = c->ws + L.nchild; sz = nn; break;
     case HYB_X_PARENT: src = c->ws + L.parent; sz = 4 * nn; break;
-    case HYB_X_COM_M: src = c->ws + L.nodeA; sz = 16 * nn; break;
-    case HYB_X_NLO: src = c->ws + L.nodeB; sz = 16 * nn; break;
-    case HYB_X_NHI: src = c->ws + L.nodeC; sz = 16 * nn; break;
-    case HYB_X_ROPEN2: {
-        if (bytes < 4 * nn) return fail(c, HYB_ERR_INVALID_ARG, "buffer too small");
-        tmp.resize(16 * nn);
-        e = cudaMemcpy(tmp.data(), c->ws + L.nodeB, 16 * nn, cudaMemcpyDeviceToHost);
-        if (e != cudaSuccess) return cuda_fail(c, e, "hyb_export copy");
-        for (size_t i = 0; i < nn; i++) ((float *)host_dst)[i] = ((const float *)tmp.data())[4 * i + 3];
-        if (written) *written = 4 * nn;
+    case HYB_X_COM_M: case HYB_X_NLO: case HYB_X_NHI: case HYB_X_ROPEN2: {      // strided fields of NodeRec
+        const size_t off = what == HYB_X_COM_M ? offsetof(NodeRec, A) : what == HYB_X_NHI ? offsetof(NodeRec, C)
+                           : what == HYB_X_NLO ? offsetof(NodeRec, B) : offsetof(NodeRec, B) + 12;
+        const size_t w = what == HYB_X_ROPEN2 ? 4 : 16;
+        if (bytes < w * nn) return fail(c, HYB_ERR_INVALID_ARG, "buffer too small");
+        if (nn) {
+            e = cudaMemcpy2D(host_dst, w, c->ws + L.nodes + off, sizeof(NodeRec), w, nn, cudaMemcpyDeviceToHost);
+            if (e != cudaSuccess) return cuda_fail(c, e, "hyb_export copy");
+        }
+        if (written) *written = w * nn;
         return HYB_OK; }
     case HYB_X_GFIRST: src = c->ws + L.gfirst; sz = 4 * ng; break;
     case HYB_X_GCOUNT: src = c->ws + L.gcount; sz = 4 * ng; break;

@@ -62,6 +62,15 @@ struct DevCtl {
     u64 inter_soft, inter_hard;
 };
 
+// One tree node as the walk reads it: 64 bytes, children of a cell are contiguous (T7).
+struct __align__(16) NodeRec {
+    float4 A;        // centre of mass, mass (T9)
+    float4 B;        // tight box minimum, squared opening radius (T8, T10)
+    float4 C;        // tight box maximum, 0
+    uint2 meta;      // cell: (first child, nchild);  leaf: (first particle, count | 0x80000000)
+    uint2 pad;
+};
+
 struct Layout {   // byte offsets into the workspace; computed by plan_workspace
     size_t ctl;
     size_t key_orig, key_a, key_b, val_a, val_b;
@@ -73,7 +82,7 @@ struct Layout {   // byte offsets into the workspace; computed by plan_workspace
     size_t pre_level, pre_first, pre_of_bfs, bfs_of_pre;   // u8, u32, u32, u32 [node_cap]
     size_t node_status;         // [ntiles(node_cap)][256] u32
     size_t level, first, count, child, nchild, parent, arrived;
-    size_t nodeA, nodeB, nodeC, meta;          // float4, float4, float4, uint2
+    size_t nodes;                              // NodeRec[node_cap]
     size_t M64, S64, C64, B2, bmax2;           // double[nc], [3nc], [3nc], [nc], u64[nc]
     size_t leaf_of;             // u32[n]
     size_t gfirst, gcount, glo, ghi, ncell, npart, nhard;   // [group_cap]

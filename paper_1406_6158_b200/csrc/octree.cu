@@ -151,7 +151,7 @@ __global__ void __launch_bounds__(256) link_kernel(
     const unsigned char *__restrict__ pre_level, const u32 *__restrict__ pre_first,
     const signed char *__restrict__ dlev, const u32 *__restrict__ slot,
     u32 *__restrict__ first, u32 *__restrict__ count, u32 *__restrict__ child, unsigned char *__restrict__ nchild,
-    u32 *__restrict__ parent, u32 *__restrict__ arrived, uint2 *__restrict__ meta, u64 *__restrict__ bmax2)
+    u32 *__restrict__ parent, u32 *__restrict__ arrived, NodeRec *__restrict__ rec, u64 *__restrict__ bmax2)
 {
     const u32 nn = ctl->nn;
     for (u32 b = blockIdx.x * blockDim.x + threadIdx.x; b < nn; b += gridDim.x * blockDim.x) {
@@ -185,7 +185,7 @@ __global__ void __launch_bounds__(256) link_kernel(
         }
         first[b] = f; count[b] = c; child[b] = ch; nchild[b] = (unsigned char)nc; parent[b] = par;
         arrived[b] = 0; bmax2[b] = 0ull;
-        meta[b] = internal ? make_uint2(ch, nc) : make_uint2(f, c | 0x80000000u);
+        rec[b].meta = internal ? make_uint2(ch, nc) : make_uint2(f, c | 0x80000000u);
     }
 }
 
@@ -194,7 +194,7 @@ struct NodeArrays {
     const u32 *first, *count, *child, *parent;
     const unsigned char *nchild, *level;
     u32 *arrived;
-    float4 *A, *B, *C;          // com_m | lo, ropen2 | hi, 0
+    NodeRec *rec;               // A = com_m, B = lo | ropen2, C = hi | 0
     double *M64, *S64, *C64, *B2;
     u32 *leaf_of;
 };
@@ -217,9 +217,9 @@ __device__ __forceinline__ void finish_node(const NodeArrays &na, u32 b, int lev
         float r = __fdiv_rn(l, theta);
         ropen2 = __fmul_rn(r, r);
     }
-    na.A[b] = make_float4(__double2float_rn(Cx), __double2float_rn(Cy), __double2float_rn(Cz), __double2float_rn(M));
-    na.B[b] = make_float4(lo.x, lo.y, lo.z, ropen2);
-    na.C[b] = make_float4(hi.x, hi.y, hi.z, 0.0f);
+    na.rec[b].A = make_float4(__double2float_rn(Cx), __double2float_rn(Cy), __double2float_rn(Cz), __double2float_rn(M));
+    na.rec[b].B = make_float4(lo.x, lo.y, lo.z, ropen2);
+    na.rec[b].C = make_float4(hi.x, hi.y, hi.z, 0.0f);
     na.M64[b] = M;
     na.S64[3 * (size_t)b] = Sx; na.S64[3 * (size_t)b + 1] = Sy; na.S64[3 * (size_t)b + 2] = Sz;
     na.C64[3 * (size_t)b] = Cx; na.C64[3 * (size_t)b + 1] = Cy; na.C64[3 * (size_t)b + 2] = Cz;
@@ -279,7 +279,7 @@ __global__ void __launch_bounds__(128) upsweep_kernel(NodeArrays na, const float
             Sx = __dadd_rn(Sx, __ldcg(na.S64 + 3 * (size_t)q));
             Sy = __dadd_rn(Sy, __ldcg(na.S64 + 3 * (size_t)q + 1));
             Sz = __dadd_rn(Sz, __ldcg(na.S64 + 3 * (size_t)q + 2));
-            float4 bl = __ldcg(na.B + q), bh = __ldcg(na.C + q);
+            float4 bl = __ldcg(&na.rec[q].B), bh = __ldcg(&na.rec[q].C);
             if (q == c0) { lo = make_float3(bl.x, bl.y, bl.z); hi = make_float3(bh.x, bh.y, bh.z); }
             else {
                 lo.x = fminf(lo.x, bl.x); lo.y = fminf(lo.y, bl.y); lo.z = fminf(lo.z, bl.z);
@@ -338,7 +338,7 @@ __global__ void __launch_bounds__(256) bmax_kernel(const float4 *__restrict__ po
 }
 
 __global__ void __launch_bounds__(256) ropen_abs_kernel(const DevCtl *__restrict__ ctl, const u64 *__restrict__ bmax2,
-                                                        const double *__restrict__ B2, float a_err, float4 *nodeB)
+                                                        const double *__restrict__ B2, float a_err, NodeRec *rec)
 {
     const u32 nn = ctl->nn;
     const u32 b = blockIdx.x * blockDim.x + threadIdx.x;
@@ -348,7 +348,7 @@ __global__ void __launch_bounds__(256) ropen_abs_kernel(const DevCtl *__restrict
     double t5 = __ddiv_rn(__dmul_rn(bm, bm), 4.0);
     double rb = __dadd_rn(__ddiv_rn(bm, 2.0), __dsqrt_rn(__dadd_rn(t5, t3)));
     float r = __double2float_rn(rb);
-    nodeB[b].w = __fmul_rn(r, r);
+    rec[b].B.w = __fmul_rn(r, r);
 }
 
 // ------------------------------------------------------------------ a7: groups (T11)
@@ -472,16 +472,16 @@ cudaError_t launch_build_tree(Ctx *c)
     u32 *first = wsptr<u32>(c, L.first), *count = wsptr<u32>(c, L.count), *child = wsptr<u32>(c, L.child);
     u32 *parent = wsptr<u32>(c, L.parent), *arrived = wsptr<u32>(c, L.arrived);
     unsigned char *nchild = wsptr<unsigned char>(c, L.nchild);
-    uint2 *meta = wsptr<uint2>(c, L.meta);
+    NodeRec *rec = wsptr<NodeRec>(c, L.nodes);
     u64 *bmax2 = wsptr<u64>(c, L.bmax2);
     const int node_grid = (int)imin64((L.node_cap + 255) / 256, (int64_t)c->num_sms * 16);
     link_kernel<<<node_grid, 256, 0, st>>>(key, n, c->p.leaf_max, ctl, level, pre_of_bfs, bfs_of_pre, pre_level,
-                                           pre_first, dlev, slot, first, count, child, nchild, parent, arrived, meta,
+                                           pre_first, dlev, slot, first, count, child, nchild, parent, arrived, rec,
                                            bmax2);
     NodeArrays na;
     na.first = first; na.count = count; na.child = child; na.parent = parent; na.nchild = nchild; na.level = level;
     na.arrived = arrived;
-    na.A = wsptr<float4>(c, L.nodeA); na.B = wsptr<float4>(c, L.nodeB); na.C = wsptr<float4>(c, L.nodeC);
+    na.rec = rec;
     na.M64 = wsptr<double>(c, L.M64); na.S64 = wsptr<double>(c, L.S64); na.C64 = wsptr<double>(c, L.C64);
     na.B2 = wsptr<double>(c, L.B2); na.leaf_of = wsptr<u32>(c, L.leaf_of);
     const int full_node_grid = (int)((L.node_cap + 127) / 128);
@@ -490,7 +490,7 @@ cudaError_t launch_build_tree(Ctx *c)
     if (c->p.mac == HYB_MAC_ABS) {
         bmax_kernel<<<(n + 255) / 256, 256, 0, st>>>(reinterpret_cast<const float4 *>(c->pos), n, na.leaf_of, parent,
                                                      level, na.C64, bmax2);
-        ropen_abs_kernel<<<(int)((L.node_cap + 255) / 256), 256, 0, st>>>(ctl, bmax2, na.B2, c->p.a_err, na.B);
+        ropen_abs_kernel<<<(int)((L.node_cap + 255) / 256), 256, 0, st>>>(ctl, bmax2, na.B2, c->p.a_err, rec);
     }
     unsigned char *gflag = wsptr<unsigned char>(c, L.gflag);
     gmark_kernel<<<(int)((L.node_cap + 255) / 256), 256, 0, st>>>(ctl, first, count, child, parent, c->p.group_max,

@@ -25,17 +25,18 @@ namespace hyb {
 
 struct WalkArgs {
     const float4 *pos;            // Morton-ordered particles (x,y,z,m)
-    const float4 *nodeA, *nodeB, *nodeC;
-    const uint2 *meta;
+    const NodeRec *nodes;
     const u32 *gfirst, *gcount;
     const float4 *glo, *ghi;
     u32 *ncell, *npart, *nhard;
     float4 *a_soft, *a_hard;
     DevCtl *ctl;
     float G, eps2, rout, kc0, kc1;   // Y = sat(kc0 + kc1 r)
+    unsigned long long zero64;       // 0, passed as an argument so that it is opaque to the compiler
 };
 
 constexpr int WK_SMAX = 4;          // most sinks per lane
+constexpr int WK_PAD_SLACK = 64;    // spare buffer entries for padding to a multiple of P U (<= 16 * 4)
 constexpr u32 FULL = 0xFFFFFFFFu;
 constexpr u32 DESC_MASK = 0x1FFFFFFFu;      // node index bits of a stack descriptor
 
@@ -43,9 +44,11 @@ template <int MODE>
 struct SmemLayout {                 // per warp
     static constexpr int cell_cap = MODE == WALK_HARD ? 0 : WK_CELL_CAP;
     static constexpr int part_cap = MODE == WALK_NORMAL ? 0 : WK_PART_CAP;
-    static constexpr int stack_cap = MODE == WALK_HARD ? 512 : 768;
-    static constexpr int lq_cap = 64;
-    static constexpr size_t bytes = 16 * (size_t)(cell_cap + part_cap) + 4 * (size_t)stack_cap + 8 * 2 * (size_t)lq_cap;
+    static constexpr int stack_cap = 512;
+    static constexpr int lq_cap = 96;
+    static constexpr int cell_alloc = cell_cap ? cell_cap + WK_PAD_SLACK : 0;
+    static constexpr int part_alloc = part_cap ? part_cap + WK_PAD_SLACK : 0;
+    static constexpr size_t bytes = 16 * (size_t)(cell_alloc + part_alloc) + 4 * (size_t)stack_cap + 8 * 2 * (size_t)lq_cap;
     static constexpr int ctas_per_sm = MODE == WALK_HARD ? 3 : 2;
 };
 
@@ -63,20 +66,85 @@ __device__ __forceinline__ float sqrt_approx(float x)
     return r;
 }
 
-// monopole (Eq. 2): 3 sub + 3 fma + rsqrt + 3 mul + 3 fma = 12 FP32-pipe instructions + 1 MUFU
-__device__ __forceinline__ void mono(const float4 s, const float3 x, float eps2, float3 &a)
+// ---- packed FP32 (Blackwell FADD2 / FMUL2 / FFMA2: two IEEE fp32 operations per lane per
+// instruction at the same per-flop pipe rate, i.e. half the issue slots).  A "pair" holds the same
+// quantity for two sinks of a lane in one 64-bit register pair.
+typedef unsigned long long f2;
+__device__ __forceinline__ f2 pk(float lo, float hi)
 {
-    float dx = s.x - x.x, dy = s.y - x.y, dz = s.z - x.z;
+    f2 r;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
+    return r;
+}
+__device__ __forceinline__ void upk(f2 p, float &lo, float &hi)
+{
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(p));
+}
+__device__ __forceinline__ f2 fma2(f2 a, f2 b, f2 c)
+{
+    f2 r;
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c));
+    return r;
+}
+__device__ __forceinline__ f2 add2(f2 a, f2 b)
+{
+    f2 r;
+    asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
+    return r;
+}
+__device__ __forceinline__ f2 mul2(f2 a, f2 b)
+{
+    f2 r;
+    asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
+    return r;
+}
+
+// Sinks of one lane: pair p holds sink slots 2p and 2p+1.  Positions are stored negated so that
+// r_j - r_i is one packed add.
+struct Sinks {
+    f2 nx[2], ny[2], nz[2];       // -x_i
+    f2 sx[2], sy[2], sz[2];       // soft (or normal-tree) accumulators
+    f2 hx[2], hy[2], hz[2];       // hard accumulators
+};
+
+// monopole (Eq. 2) for two sinks: 3 add2 + 3 fma2 + 2 rsqrt + 3 mul2 + 3 fma2
+//   = 12 FP32-pipe instructions (24 pipe cycles) + 2 MUFU per pair of interactions
+__device__ __forceinline__ void mono2(const float4 s, f2 nx, f2 ny, f2 nz, float eps2, f2 &ax, f2 &ay, f2 &az)
+{
+    const f2 dx = add2(pk(s.x, s.x), nx), dy = add2(pk(s.y, s.y), ny), dz = add2(pk(s.z, s.z), nz);
+    f2 r2 = fma2(dx, dx, pk(eps2, eps2));
+    r2 = fma2(dy, dy, r2);
+    r2 = fma2(dz, dz, r2);
+    float r2a, r2b;
+    upk(r2, r2a, r2b);
+    const f2 ri = pk(rsqrt_approx(r2a), rsqrt_approx(r2b));
+    const f2 ri2 = mul2(ri, ri);
+    const f2 mr = mul2(pk(s.w, s.w), ri);
+    const f2 mr3 = mul2(mr, ri2);
+    ax = fma2(mr3, dx, ax);
+    ay = fma2(mr3, dy, ay);
+    az = fma2(mr3, dz, az);
+}
+
+// the same for the single sink held in the low half of a pair (S = 3)
+__device__ __forceinline__ void mono1(const float4 s, f2 nx, f2 ny, f2 nz, float eps2, f2 &ax, f2 &ay, f2 &az)
+{
+    float x, y, z, a0, a1, a2, t;
+    upk(nx, x, t); upk(ny, y, t); upk(nz, z, t);
+    float hx, hy, hz;
+    upk(ax, a0, hx); upk(ay, a1, hy); upk(az, a2, hz);
+    const float dx = s.x + x, dy = s.y + y, dz = s.z + z;
     float r2 = fmaf(dx, dx, eps2);
     r2 = fmaf(dy, dy, r2);
     r2 = fmaf(dz, dz, r2);
-    float ri = rsqrt_approx(r2);
-    float ri2 = ri * ri;
-    float mr = s.w * ri;
-    float mr3 = mr * ri2;
-    a.x = fmaf(mr3, dx, a.x);
-    a.y = fmaf(mr3, dy, a.y);
-    a.z = fmaf(mr3, dz, a.z);
+    const float ri = rsqrt_approx(r2);
+    const float ri2 = ri * ri;
+    const float mr = s.w * ri;
+    const float mr3 = mr * ri2;
+    a0 = fmaf(mr3, dx, a0);
+    a1 = fmaf(mr3, dy, a1);
+    a2 = fmaf(mr3, dz, a2);
+    ax = pk(a0, hx); ay = pk(a1, hy); az = pk(a2, hz);
 }
 
 // Eq. 10 with Y clamped to [0,1]: K = t^3 (10 - 15 t + 6 t^2), t = Y^2 (T15)
@@ -88,55 +156,117 @@ __device__ __forceinline__ float kfun(float r, float kc0, float kc1)
     return (t * t) * (t * poly);
 }
 
-// K-weighted pair (Eq. 8, 9): hard part K F, and (SOFT) the soft part (1 - K) F
+// K-weighted pair (Eq. 8, 9) for two sinks: hard part K F, and (SOFT) the soft part (1 - K) F.
+// fused: 25 FP32-pipe instruction equivalents + 4 MUFU per pair of interactions; hard only: 21 + 4.
 template <bool SOFT>
-__device__ __forceinline__ void kpair(const float4 s, const float3 x, float eps2, float kc0, float kc1, float3 &as,
-                                      float3 &ah)
+__device__ __forceinline__ void kpair2(const float4 s, f2 nx, f2 ny, f2 nz, float eps2, float kc0, float kc1, f2 &sx,
+                                       f2 &sy, f2 &sz, f2 &hx, f2 &hy, f2 &hz)
 {
-    float dx = s.x - x.x, dy = s.y - x.y, dz = s.z - x.z;
+    const f2 dx = add2(pk(s.x, s.x), nx), dy = add2(pk(s.y, s.y), ny), dz = add2(pk(s.z, s.z), nz);
+    f2 r2u = mul2(dx, dx);
+    r2u = fma2(dy, dy, r2u);
+    r2u = fma2(dz, dz, r2u);
+    const f2 r2e = add2(r2u, pk(eps2, eps2));
+    float ua, ub, ea, eb;
+    upk(r2u, ua, ub); upk(r2e, ea, eb);
+    const f2 ri = pk(rsqrt_approx(ea), rsqrt_approx(eb));
+    const float Ya = __saturatef(fmaf(sqrt_approx(ua), kc1, kc0)), Yb = __saturatef(fmaf(sqrt_approx(ub), kc1, kc0));
+    const f2 Y = pk(Ya, Yb);
+    const f2 t = mul2(Y, Y);
+    const f2 poly = fma2(fma2(pk(6.0f, 6.0f), t, pk(-15.0f, -15.0f)), t, pk(10.0f, 10.0f));
+    const f2 K = mul2(mul2(t, t), mul2(t, poly));
+    const f2 ri2 = mul2(ri, ri);
+    const f2 mr = mul2(pk(s.w, s.w), ri);
+    const f2 mr3 = mul2(mr, ri2);
+    const f2 wh = mul2(K, mr3);
+    hx = fma2(wh, dx, hx);
+    hy = fma2(wh, dy, hy);
+    hz = fma2(wh, dz, hz);
+    if (SOFT) {
+        const f2 ws = fma2(wh, pk(-1.0f, -1.0f), mr3);
+        sx = fma2(ws, dx, sx);
+        sy = fma2(ws, dy, sy);
+        sz = fma2(ws, dz, sz);
+    }
+}
+
+template <bool SOFT>
+__device__ __forceinline__ void kpair1(const float4 s, f2 nx, f2 ny, f2 nz, float eps2, float kc0, float kc1, f2 &sx,
+                                       f2 &sy, f2 &sz, f2 &hx, f2 &hy, f2 &hz)
+{
+    float x, y, z, t;
+    upk(nx, x, t); upk(ny, y, t); upk(nz, z, t);
+    const float dx = s.x + x, dy = s.y + y, dz = s.z + z;
     float r2u = dx * dx;
     r2u = fmaf(dy, dy, r2u);
     r2u = fmaf(dz, dz, r2u);
-    float ri = rsqrt_approx(r2u + eps2);
-    float r = sqrt_approx(r2u);
-    float ri2 = ri * ri;
-    float mr = s.w * ri;
-    float mr3 = mr * ri2;
-    float wh = kfun(r, kc0, kc1) * mr3;
-    ah.x = fmaf(wh, dx, ah.x);
-    ah.y = fmaf(wh, dy, ah.y);
-    ah.z = fmaf(wh, dz, ah.z);
+    const float ri = rsqrt_approx(r2u + eps2);
+    const float r = sqrt_approx(r2u);
+    const float ri2 = ri * ri;
+    const float mr = s.w * ri;
+    const float mr3 = mr * ri2;
+    const float wh = kfun(r, kc0, kc1) * mr3;
+    float a0, a1, a2, b0, b1, b2;
+    upk(hx, a0, b0); upk(hy, a1, b1); upk(hz, a2, b2);
+    hx = pk(fmaf(wh, dx, a0), b0); hy = pk(fmaf(wh, dy, a1), b1); hz = pk(fmaf(wh, dz, a2), b2);
     if (SOFT) {
-        float ws = mr3 - wh;
-        as.x = fmaf(ws, dx, as.x);
-        as.y = fmaf(ws, dy, as.y);
-        as.z = fmaf(ws, dz, as.z);
+        const float ws = mr3 - wh;
+        upk(sx, a0, b0); upk(sy, a1, b1); upk(sz, a2, b2);
+        sx = pk(fmaf(ws, dx, a0), b0); sy = pk(fmaf(ws, dy, a1), b1); sz = pk(fmaf(ws, dz, a2), b2);
     }
 }
 
-template <int S>
-__device__ __forceinline__ void eval_mono(const float4 *buf, int cnt, int part, int P, const float3 (&x)[WK_SMAX],
-                                          float eps2, float3 (&acc)[WK_SMAX])
+// Buffer evaluation.  The caller pads the buffer with zero-mass entries to a multiple of P U, so every
+// part runs the same number of iterations and an iteration is U S independent pair chains.
+template <int S, int U>
+__device__ __forceinline__ void eval_mono(const float4 *buf, int cnt, int part, int P, Sinks &k, float eps2)
 {
-#pragma unroll 2
-    for (int j = part; j < cnt; j += P) {
-        const float4 s = buf[j];
+    if (part >= P) return;
+    const float4 *p = buf + part;
+    const int step = P * U;
+    for (int j = 0; j < cnt; j += step, p += step) {
+        float4 s[U];
 #pragma unroll
-        for (int k = 0; k < S; k++) mono(s, x[k], eps2, acc[k]);
+        for (int u = 0; u < U; u++) s[u] = p[u * P];
+#pragma unroll
+        for (int u = 0; u < U; u++) {
+#pragma unroll
+            for (int q = 0; q < S / 2; q++) mono2(s[u], k.nx[q], k.ny[q], k.nz[q], eps2, k.sx[q], k.sy[q], k.sz[q]);
+            if (S & 1) mono1(s[u], k.nx[S / 2], k.ny[S / 2], k.nz[S / 2], eps2, k.sx[S / 2], k.sy[S / 2], k.sz[S / 2]);
+        }
     }
 }
 
-template <int S, bool SOFT>
-__device__ __forceinline__ void eval_near(const float4 *buf, int cnt, int part, int P, const float3 (&x)[WK_SMAX],
-                                          float eps2, float kc0, float kc1, float3 (&as)[WK_SMAX],
-                                          float3 (&ah)[WK_SMAX])
+template <int S, int U, bool SOFT>
+__device__ __forceinline__ void eval_near(const float4 *buf, int cnt, int part, int P, Sinks &k, float eps2, float kc0,
+                                          float kc1)
 {
-#pragma unroll 1
-    for (int j = part; j < cnt; j += P) {
-        const float4 s = buf[j];
+    if (part >= P) return;
+    const float4 *p = buf + part;
+    const int step = P * U;
+    for (int j = 0; j < cnt; j += step, p += step) {
+        float4 s[U];
 #pragma unroll
-        for (int k = 0; k < S; k++) kpair<SOFT>(s, x[k], eps2, kc0, kc1, as[k], ah[k]);
+        for (int u = 0; u < U; u++) s[u] = p[u * P];
+#pragma unroll
+        for (int u = 0; u < U; u++) {
+#pragma unroll
+            for (int q = 0; q < S / 2; q++)
+                kpair2<SOFT>(s[u], k.nx[q], k.ny[q], k.nz[q], eps2, kc0, kc1, k.sx[q], k.sy[q], k.sz[q], k.hx[q], k.hy[q],
+                             k.hz[q]);
+            if (S & 1)
+                kpair1<SOFT>(s[u], k.nx[S / 2], k.ny[S / 2], k.nz[S / 2], eps2, kc0, kc1, k.sx[S / 2], k.sy[S / 2],
+                             k.sz[S / 2], k.hx[S / 2], k.hy[S / 2], k.hz[S / 2]);
+        }
     }
+}
+
+// zero-mass entries up to the next multiple of `step` (the buffers have WK_PAD_SLACK spare entries)
+__device__ __forceinline__ int pad_buffer(float4 *buf, int cnt, int step, float4 dummy, int lane)
+{
+    const int padded = ((cnt + step - 1) / step) * step;
+    for (int i = cnt + lane; i < padded; i += 32) buf[i] = dummy;
+    return padded;
 }
 
 __device__ __forceinline__ u32 warp_excl_scan(u32 v, int lane, u32 &total)
@@ -163,8 +293,8 @@ __global__ void __launch_bounds__(WK_WARPS * 32, SmemLayout<MODE>::ctas_per_sm) 
     const int oct = lane >> 3, sub = lane & 7;
     unsigned char *wbase = smem_raw + (size_t)warp * SL::bytes;
     float4 *cellbuf = reinterpret_cast<float4 *>(wbase);
-    float4 *partbuf = cellbuf + SL::cell_cap;
-    u32 *stack = reinterpret_cast<u32 *>(partbuf + SL::part_cap);
+    float4 *partbuf = cellbuf + SL::cell_alloc;
+    u32 *stack = reinterpret_cast<u32 *>(partbuf + SL::part_alloc);
     uint2 *lq0 = reinterpret_cast<uint2 *>(stack + SL::stack_cap);     // far leaves
     uint2 *lq1 = lq0 + SL::lq_cap;                                     // near leaves
     float *red = reinterpret_cast<float *>(wbase);                     // reduction scratch (buffers are empty then)
@@ -193,176 +323,200 @@ __global__ void __launch_bounds__(WK_WARPS * 32, SmemLayout<MODE>::ctas_per_sm) 
             if (4 * P3 >= best) { best = 4 * P3; S = 3; A = A3; P = P3; }
             if (3 * P4 >= best) { S = 4; A = A4; P = P4; }
         }
+        P = min(P, 16);                   // groups of one or two sinks: keeps the padding step P U <= 64
+        const int US = S == 2 ? 4 : 2;                                // sources per evaluation iteration (monopoles)
         const int aidx = lane % A;
         const int part = (lane / A < P) ? lane / A : 0x40000000;     // idle lanes never enter the loops
-        float3 x[WK_SMAX], as[WK_SMAX], ah[WK_SMAX];
+        const float4 dummy = make_float4(glo.x, glo.y, glo.z, 0.0f); // zero-mass padding entry
+        Sinks sk;
 #pragma unroll
-        for (int k = 0; k < WK_SMAX; k++) {
-            const int si = aidx + k * A;
-            const float4 p = __ldg(a.pos + gf + ((k < S && si < n) ? si : 0));
-            x[k] = make_float3(p.x, p.y, p.z);
-            as[k] = make_float3(0.0f, 0.0f, 0.0f);
-            ah[k] = make_float3(0.0f, 0.0f, 0.0f);
+        for (int q = 0; q < 2; q++) {
+            const int s0 = aidx + 2 * q * A, s1 = s0 + A;
+            const float4 p0 = __ldg(a.pos + gf + ((2 * q < S && s0 < n) ? s0 : 0));
+            const float4 p1 = __ldg(a.pos + gf + ((2 * q + 1 < S && s1 < n) ? s1 : 0));
+            // the 64-bit integer add of an (opaque) zero makes each pair the result of a real instruction,
+            // so it lives in an aligned register pair instead of being re-packed from p0 / p1 at every use
+            sk.nx[q] = pk(-p0.x, -p1.x) + a.zero64; sk.ny[q] = pk(-p0.y, -p1.y) + a.zero64;
+            sk.nz[q] = pk(-p0.z, -p1.z) + a.zero64;
+            sk.sx[q] = sk.sy[q] = sk.sz[q] = 0ull;
+            sk.hx[q] = sk.hy[q] = sk.hz[q] = 0ull;
         }
 
         u32 ncell = 0, npart = 0, nhard = 0;
         int ncb = 0, npb = 0;             // buffer fills
         int nlq0 = 0, nlq1 = 0;           // leaf queue fills
-        int sp = 0;
+        int sp = 1;
         bool trav_done = false, flush_mono = false, flush_near = false, overflow = false;
+        bool slow = false;                // something other than a plain traversal iteration is pending
         int ex_near = 0;                  // pending expansion: target buffer, this lane's leaf, progress
         u32 ex_first = 0, ex_cnt = 0, ex_off = 0, ex_T = 0, ex_done = 0;
-
-        // current batch of nodes (one per lane); starts with the root alone
-        bool have = lane == 0;
-        u32 node = 0;
-        float4 nA = make_float4(0, 0, 0, 0), nB = nA, nC = nA;
-        uint2 mt = make_uint2(0, 0);
-        if (have) {
-            nB = __ldg(a.nodeB); nC = __ldg(a.nodeC); mt = __ldg(a.meta);
-            if (MODE != WALK_HARD) nA = __ldg(a.nodeA);
-        }
+        if (lane == 0) stack[0] = 0u;     // the root alone: "first child" 0, nchild - 1 = 0
+        __syncwarp();
 
         for (;;) {
-            // ---- evaluation: the only call sites
-            if (HAS_MONO && flush_mono) {
-                __syncwarp();
-                if (S == 2) eval_mono<2>(cellbuf, ncb, part, P, x, eps2, as);
-                else if (S == 3) eval_mono<3>(cellbuf, ncb, part, P, x, eps2, as);
-                else eval_mono<4>(cellbuf, ncb, part, P, x, eps2, as);
-                ncb = 0; flush_mono = false;
-                __syncwarp();
-            }
-            if (HAS_NEAR && flush_near) {
-                __syncwarp();
-                if (S == 2) eval_near<2, MODE == WALK_HYBRID>(partbuf, npb, part, P, x, eps2, kc0, kc1, as, ah);
-                else if (S == 3) eval_near<3, MODE == WALK_HYBRID>(partbuf, npb, part, P, x, eps2, kc0, kc1, as, ah);
-                else eval_near<4, MODE == WALK_HYBRID>(partbuf, npb, part, P, x, eps2, kc0, kc1, as, ah);
-                npb = 0; flush_near = false;
-                __syncwarp();
-            }
-            // ---- pending leaf expansion: every lane copies the part of its leaf that fits
-            if (ex_done < ex_T) {
-                const bool tonear = HAS_NEAR && (!HAS_MONO || ex_near);
-                float4 *buf = tonear ? partbuf : cellbuf;
-                const int cap = tonear ? SL::part_cap : SL::cell_cap;
-                int fill = tonear ? npb : ncb;
-                const u32 take = min((u32)(cap - fill), ex_T - ex_done);
-                const u32 lo = max(ex_off, ex_done), hi = min(ex_off + ex_cnt, ex_done + take);
-                for (u32 e = lo; e < hi; e++) buf[fill + (e - ex_done)] = __ldg(a.pos + ex_first + (e - ex_off));
-                fill += (int)take; ex_done += take;
-                if (tonear) npb = fill; else ncb = fill;
-                if (ex_done < ex_T) { if (tonear) flush_near = true; else flush_mono = true; }    // buffer is full
-                continue;
-            }
-            // ---- start an expansion when a leaf queue holds a full batch (or at the end)
-            {
-                int cls = -1;
-                if (HAS_MONO && (nlq0 >= 32 || (trav_done && nlq0 > 0))) cls = 0;
-                else if (HAS_NEAR && (nlq1 >= 32 || (trav_done && nlq1 > 0))) cls = 1;
-                if (cls >= 0) {
+            if (slow) {
+                // ---- evaluation: the only call sites
+                if (HAS_MONO && flush_mono) {
+                    const int cnt = pad_buffer(cellbuf, ncb, P * US, dummy, lane);
                     __syncwarp();
-                    int &nlq = cls ? nlq1 : nlq0;
-                    const uint2 *q = cls ? lq1 : lq0;
-                    const int m = min(32, nlq);
-                    uint2 lf = make_uint2(0, 0);
-                    if (lane < m) lf = q[nlq - m + lane];
-                    nlq -= m;
-                    ex_first = lf.x; ex_cnt = lf.y;
-                    ex_off = warp_excl_scan(ex_cnt, lane, ex_T);
-                    ex_done = 0; ex_near = cls;
+                    if (S == 2) eval_mono<2, 4>(cellbuf, cnt, part, P, sk, eps2);
+                    else if (S == 3) eval_mono<3, 2>(cellbuf, cnt, part, P, sk, eps2);
+                    else eval_mono<4, 2>(cellbuf, cnt, part, P, sk, eps2);
+                    ncb = 0; flush_mono = false;
                     __syncwarp();
+                }
+                if (HAS_NEAR && flush_near) {
+                    const int cnt = pad_buffer(partbuf, npb, P * 2, dummy, lane);
+                    __syncwarp();
+                    if (S == 2) eval_near<2, 2, MODE == WALK_HYBRID>(partbuf, cnt, part, P, sk, eps2, kc0, kc1);
+                    else if (S == 3) eval_near<3, 2, MODE == WALK_HYBRID>(partbuf, cnt, part, P, sk, eps2, kc0, kc1);
+                    else eval_near<4, 2, MODE == WALK_HYBRID>(partbuf, cnt, part, P, sk, eps2, kc0, kc1);
+                    npb = 0; flush_near = false;
+                    __syncwarp();
+                }
+                // ---- pending leaf expansion: every lane copies the part of its leaf that fits
+                if (ex_done < ex_T) {
+                    const bool tonear = HAS_NEAR && (!HAS_MONO || ex_near);
+                    float4 *buf = tonear ? partbuf : cellbuf;
+                    const int cap = tonear ? SL::part_cap : SL::cell_cap;
+                    int fill = tonear ? npb : ncb;
+                    const u32 take = min((u32)(cap - fill), ex_T - ex_done);
+                    const u32 lo = max(ex_off, ex_done), hi = min(ex_off + ex_cnt, ex_done + take);
+#pragma unroll 4
+                    for (u32 e = lo; e < hi; e++) buf[fill + (e - ex_done)] = __ldg(a.pos + ex_first + (e - ex_off));
+                    fill += (int)take; ex_done += take;
+                    if (tonear) npb = fill; else ncb = fill;
+                    if (ex_done < ex_T) { if (tonear) flush_near = true; else flush_mono = true; }    // buffer is full
                     continue;
                 }
-            }
-            if (trav_done) {
-                if (HAS_MONO && ncb > 0) { flush_mono = true; continue; }
-                if (HAS_NEAR && npb > 0) { flush_near = true; continue; }
-                break;
-            }
-            // ---- traversal iteration on the current batch
-            if (HAS_MONO && ncb > SL::cell_cap - 32) { flush_mono = true; continue; }
-            bool accept = false, open_int = false, leaf_far = false, leaf_near = false;
-            if (have) {
-                // T12: box-box distance (rule (b)), fp32, one rounding per operation
-                float fx = fmaxf(0.0f, fmaxf(__fsub_rn(nB.x, ghi.x), __fsub_rn(glo.x, nC.x)));
-                float fy = fmaxf(0.0f, fmaxf(__fsub_rn(nB.y, ghi.y), __fsub_rn(glo.y, nC.y)));
-                float fz = fmaxf(0.0f, fmaxf(__fsub_rn(nB.z, ghi.z), __fsub_rn(glo.z, nC.z)));
-                float d2b = __fadd_rn(__fadd_rn(__fmul_rn(fx, fx), __fmul_rn(fy, fy)), __fmul_rn(fz, fz));
-                const bool near = d2b < rout2;
-                bool open;
-                if (MODE == WALK_HARD) open = near;
-                else {
-                    float ex = fmaxf(0.0f, fmaxf(__fsub_rn(glo.x, nA.x), __fsub_rn(nA.x, ghi.x)));
-                    float ey = fmaxf(0.0f, fmaxf(__fsub_rn(glo.y, nA.y), __fsub_rn(nA.y, ghi.y)));
-                    float ez = fmaxf(0.0f, fmaxf(__fsub_rn(glo.z, nA.z), __fsub_rn(nA.z, ghi.z)));
-                    float d2a = __fadd_rn(__fadd_rn(__fmul_rn(ex, ex), __fmul_rn(ey, ey)), __fmul_rn(ez, ez));
-                    const bool mac_open = d2a < nB.w;
-                    open = (MODE == WALK_NORMAL) ? mac_open : (mac_open || near);
+                // ---- start an expansion when a leaf queue holds a full batch (or at the end)
+                {
+                    int cls = -1;
+                    if (HAS_MONO && (nlq0 >= 32 || (trav_done && nlq0 > 0))) cls = 0;
+                    else if (HAS_NEAR && (nlq1 >= 32 || (trav_done && nlq1 > 0))) cls = 1;
+                    if (cls >= 0) {
+                        __syncwarp();
+                        int &nlq = cls ? nlq1 : nlq0;
+                        const uint2 *q = cls ? lq1 : lq0;
+                        const int m = min(32, nlq);
+                        uint2 lf = make_uint2(0, 0);
+                        if (lane < m) lf = q[nlq - m + lane];
+                        nlq -= m;
+                        ex_first = lf.x; ex_cnt = lf.y;
+                        ex_off = warp_excl_scan(ex_cnt, lane, ex_T);
+                        ex_done = 0; ex_near = cls;
+                        __syncwarp();
+                        continue;
+                    }
                 }
-                const bool is_leaf = (mt.y & 0x80000000u) != 0;
-                accept = !open && MODE != WALK_HARD;
-                open_int = open && !is_leaf;
-                leaf_near = open && is_leaf && near && MODE != WALK_NORMAL;
-                leaf_far = open && is_leaf && !leaf_near;
+                if (HAS_MONO && ncb > SL::cell_cap - 64) { flush_mono = true; continue; }
+                if (trav_done) {
+                    if (HAS_MONO && ncb > 0) { flush_mono = true; continue; }
+                    if (HAS_NEAR && npb > 0) { flush_near = true; continue; }
+                    break;
+                }
+                slow = false;
             }
-            // opened cells: push one descriptor each
-            {
-                const u32 bal = __ballot_sync(FULL, open_int);
-                const int npush = __popc(bal);
-                if (sp + npush > SL::stack_cap) { overflow = true; break; }
-                if (open_int) stack[sp + __popc(bal & lt_mask)] = mt.x | ((mt.y - 1u) << 29);
-                sp += npush;
-            }
-            __syncwarp();
-            // pop the next batch and request its node records
-            const int npop = min(4, sp);
-            bool have_n = false;
-            u32 node_n = 0;
-            if (oct < npop) {
-                const u32 d = stack[sp - 1 - oct];
-                node_n = (d & DESC_MASK) + (u32)sub;
-                have_n = (u32)sub <= (d >> 29);
+            // ---- traversal iteration: pop up to eight descriptors, lane (oct, sub) tests child sub of
+            //      descriptors oct and oct + 4
+            const int npop = min(8, sp);
+            bool have[2];
+            float4 nA[2], nB[2], nC[2];
+            uint2 mt[2];
+#pragma unroll
+            for (int h = 0; h < 2; h++) {
+                have[h] = false;
+                const int slot = oct + 4 * h;
+                if (slot < npop) {
+                    const u32 d = stack[sp - 1 - slot];
+                    have[h] = (u32)sub <= (d >> 29);
+                    if (have[h]) {
+                        const NodeRec *r = a.nodes + ((d & DESC_MASK) + (u32)sub);
+                        nB[h] = __ldg(&r->B); nC[h] = __ldg(&r->C); mt[h] = __ldg(&r->meta);
+                        if (MODE != WALK_HARD) nA[h] = __ldg(&r->A);
+                    }
+                }
             }
             sp -= npop;
-            float4 nA_n = make_float4(0, 0, 0, 0), nB_n = nA_n, nC_n = nA_n;
-            uint2 mt_n = make_uint2(0, 0);
-            if (have_n) {
-                nB_n = __ldg(a.nodeB + node_n); nC_n = __ldg(a.nodeC + node_n); mt_n = __ldg(a.meta + node_n);
-                if (MODE != WALK_HARD) nA_n = __ldg(a.nodeA + node_n);
+            __syncwarp();
+            bool accept[2], open_int[2], leaf_far[2], leaf_near[2];
+#pragma unroll
+            for (int h = 0; h < 2; h++) {
+                accept[h] = open_int[h] = leaf_far[h] = leaf_near[h] = false;
+                if (have[h]) {
+                    // T12: box-box distance (rule (b)), fp32, one rounding per operation
+                    float fx = fmaxf(0.0f, fmaxf(__fsub_rn(nB[h].x, ghi.x), __fsub_rn(glo.x, nC[h].x)));
+                    float fy = fmaxf(0.0f, fmaxf(__fsub_rn(nB[h].y, ghi.y), __fsub_rn(glo.y, nC[h].y)));
+                    float fz = fmaxf(0.0f, fmaxf(__fsub_rn(nB[h].z, ghi.z), __fsub_rn(glo.z, nC[h].z)));
+                    float d2b = __fadd_rn(__fadd_rn(__fmul_rn(fx, fx), __fmul_rn(fy, fy)), __fmul_rn(fz, fz));
+                    const bool near = d2b < rout2;
+                    bool open;
+                    if (MODE == WALK_HARD) open = near;
+                    else {
+                        float ex = fmaxf(0.0f, fmaxf(__fsub_rn(glo.x, nA[h].x), __fsub_rn(nA[h].x, ghi.x)));
+                        float ey = fmaxf(0.0f, fmaxf(__fsub_rn(glo.y, nA[h].y), __fsub_rn(nA[h].y, ghi.y)));
+                        float ez = fmaxf(0.0f, fmaxf(__fsub_rn(glo.z, nA[h].z), __fsub_rn(nA[h].z, ghi.z)));
+                        float d2a = __fadd_rn(__fadd_rn(__fmul_rn(ex, ex), __fmul_rn(ey, ey)), __fmul_rn(ez, ez));
+                        const bool mac_open = d2a < nB[h].w;
+                        open = (MODE == WALK_NORMAL) ? mac_open : (mac_open || near);
+                    }
+                    const bool is_leaf = (mt[h].y & 0x80000000u) != 0;
+                    accept[h] = !open && MODE != WALK_HARD;
+                    open_int[h] = open && !is_leaf;
+                    leaf_near[h] = open && is_leaf && near && MODE != WALK_NORMAL;
+                    leaf_far[h] = open && is_leaf && !leaf_near[h];
+                }
             }
+            // opened cells: push one descriptor each
+#pragma unroll
+            for (int h = 0; h < 2; h++) {
+                const u32 bal = __ballot_sync(FULL, open_int[h]);
+                const int npush = __popc(bal);
+                if (sp + npush > SL::stack_cap) { overflow = true; break; }
+                if (open_int[h]) stack[sp + __popc(bal & lt_mask)] = mt[h].x | ((mt[h].y - 1u) << 29);
+                sp += npush;
+            }
+            if (overflow) break;
             // accepted cells -> monopole buffer
             if (HAS_MONO) {
-                const u32 bal = __ballot_sync(FULL, accept);
-                if (accept) cellbuf[ncb + __popc(bal & lt_mask)] = nA;
-                ncb += __popc(bal);
-                ncell += __popc(bal);
+#pragma unroll
+                for (int h = 0; h < 2; h++) {
+                    const u32 bal = __ballot_sync(FULL, accept[h]);
+                    if (accept[h]) cellbuf[ncb + __popc(bal & lt_mask)] = nA[h];
+                    ncb += __popc(bal);
+                    ncell += __popc(bal);
+                }
             }
             // opened leaves -> queues
             if (HAS_MONO) {
-                const u32 bal = __ballot_sync(FULL, leaf_far);
-                if (bal) {
-                    const u32 cnt = leaf_far ? (mt.y & 0x7FFFFFFFu) : 0u;
-                    if (leaf_far) lq0[nlq0 + __popc(bal & lt_mask)] = make_uint2(mt.x, cnt);
-                    nlq0 += __popc(bal);
-                    npart += __reduce_add_sync(FULL, cnt);
+#pragma unroll
+                for (int h = 0; h < 2; h++) {
+                    const u32 bal = __ballot_sync(FULL, leaf_far[h]);
+                    if (bal) {
+                        const u32 cnt = leaf_far[h] ? (mt[h].y & 0x7FFFFFFFu) : 0u;
+                        if (leaf_far[h]) lq0[nlq0 + __popc(bal & lt_mask)] = make_uint2(mt[h].x, cnt);
+                        nlq0 += __popc(bal);
+                        npart += __reduce_add_sync(FULL, cnt);
+                    }
                 }
             }
             if (HAS_NEAR) {
-                const u32 bal = __ballot_sync(FULL, leaf_near);
-                if (bal) {
-                    const u32 cnt = leaf_near ? (mt.y & 0x7FFFFFFFu) : 0u;
-                    if (leaf_near) lq1[nlq1 + __popc(bal & lt_mask)] = make_uint2(mt.x, cnt);
-                    nlq1 += __popc(bal);
-                    const u32 tot = __reduce_add_sync(FULL, cnt);
-                    npart += tot; nhard += tot;
+#pragma unroll
+                for (int h = 0; h < 2; h++) {
+                    const u32 bal = __ballot_sync(FULL, leaf_near[h]);
+                    if (bal) {
+                        const u32 cnt = leaf_near[h] ? (mt[h].y & 0x7FFFFFFFu) : 0u;
+                        if (leaf_near[h]) lq1[nlq1 + __popc(bal & lt_mask)] = make_uint2(mt[h].x, cnt);
+                        nlq1 += __popc(bal);
+                        const u32 tot = __reduce_add_sync(FULL, cnt);
+                        npart += tot; nhard += tot;
+                    }
                 }
             }
-            // rotate
-            have = have_n; node = node_n; nA = nA_n; nB = nB_n; nC = nC_n; mt = mt_n;
-            if (npop == 0) trav_done = true;
+            __syncwarp();
+            trav_done = sp == 0;
+            slow = trav_done || nlq0 >= 32 || nlq1 >= 32 || (HAS_MONO && ncb > SL::cell_cap - 64);
         }
-        (void)node;
         __syncwarp();
         if (overflow && lane == 0) atomicOr(&a.ctl->status, ST_STACK_OVERFLOW);
 
@@ -370,10 +524,20 @@ __global__ void __launch_bounds__(WK_WARPS * 32, SmemLayout<MODE>::ctas_per_sm) 
         //      component c of sink slot k for all 32 lanes; lane (aidx, part) sums rows part, part+P, ...
         float v[WK_SMAX * C];
 #pragma unroll
-        for (int k = 0; k < WK_SMAX; k++) {
-            if (MODE != WALK_HARD) { v[k * C + 0] = as[k].x; v[k * C + 1] = as[k].y; v[k * C + 2] = as[k].z; }
-            if (MODE == WALK_HYBRID) { v[k * C + 3] = ah[k].x; v[k * C + 4] = ah[k].y; v[k * C + 5] = ah[k].z; }
-            if (MODE == WALK_HARD) { v[k * C + 0] = ah[k].x; v[k * C + 1] = ah[k].y; v[k * C + 2] = ah[k].z; }
+        for (int q = 0; q < 2; q++) {
+            const int k0 = 2 * q, k1 = 2 * q + 1;
+            if (MODE != WALK_HARD) {
+                upk(sk.sx[q], v[k0 * C + 0], v[k1 * C + 0]); upk(sk.sy[q], v[k0 * C + 1], v[k1 * C + 1]);
+                upk(sk.sz[q], v[k0 * C + 2], v[k1 * C + 2]);
+            }
+            if (MODE == WALK_HYBRID) {
+                upk(sk.hx[q], v[k0 * C + 3], v[k1 * C + 3]); upk(sk.hy[q], v[k0 * C + 4], v[k1 * C + 4]);
+                upk(sk.hz[q], v[k0 * C + 5], v[k1 * C + 5]);
+            }
+            if (MODE == WALK_HARD) {
+                upk(sk.hx[q], v[k0 * C + 0], v[k1 * C + 0]); upk(sk.hy[q], v[k0 * C + 1], v[k1 * C + 1]);
+                upk(sk.hz[q], v[k0 * C + 2], v[k1 * C + 2]);
+            }
         }
         if (P > 1) {
             const int rows = S * C;
@@ -457,8 +621,7 @@ cudaError_t launch_walk(Ctx *c, int mode)
     const Layout &L = c->L;
     WalkArgs a;
     a.pos = reinterpret_cast<const float4 *>(c->pos);
-    a.nodeA = wsptr<float4>(c, L.nodeA); a.nodeB = wsptr<float4>(c, L.nodeB); a.nodeC = wsptr<float4>(c, L.nodeC);
-    a.meta = wsptr<uint2>(c, L.meta);
+    a.nodes = wsptr<NodeRec>(c, L.nodes);
     a.gfirst = wsptr<u32>(c, L.gfirst); a.gcount = wsptr<u32>(c, L.gcount);
     a.glo = wsptr<float4>(c, L.glo); a.ghi = wsptr<float4>(c, L.ghi);
     a.ncell = wsptr<u32>(c, L.ncell); a.npart = wsptr<u32>(c, L.npart); a.nhard = wsptr<u32>(c, L.nhard);
@@ -467,6 +630,7 @@ cudaError_t launch_walk(Ctx *c, int mode)
     a.G = c->p.G; a.eps2 = c->p.eps * c->p.eps; a.rout = c->p.r_out;
     const float w = c->p.r_out - c->p.r_in;
     a.kc0 = c->p.r_out / w; a.kc1 = -1.0f / w;
+    a.zero64 = 0ull;
     cudaMemsetAsync(&c->ctl->group_counter, 0, sizeof(u32), c->stream);
     if (mode == WALK_HYBRID) return launch_walk_mode<WALK_HYBRID>(c, a);
     if (mode == WALK_HARD) return launch_walk_mode<WALK_HARD>(c, a);
