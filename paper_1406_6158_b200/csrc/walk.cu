@@ -218,23 +218,90 @@ __device__ __forceinline__ void kpair1(const float4 s, f2 nx, f2 ny, f2 nz, floa
 
 // Buffer evaluation.  The caller pads the buffer with zero-mass entries to a multiple of P U, so every
 // part runs the same number of iterations and an iteration is U S independent pair chains.
+// The U sources x (S/2 pairs [+ 1 single]) chains of an iteration are written stage by stage
+// (differences, r^2, rsqrt, products, accumulation) so that independent chains are interleaved and
+// the FMA pipe is not left waiting on one chain's latency.
 template <int S, int U>
 __device__ __forceinline__ void eval_mono(const float4 *buf, int cnt, int part, int P, Sinks &k, float eps2)
 {
+    constexpr int NP = S / 2;
+    constexpr bool ODD = (S & 1) != 0;
     if (part >= P) return;
     const float4 *p = buf + part;
     const int step = P * U;
+    const f2 EPS = pk(eps2, eps2);
+    float ox = 0, oy = 0, oz = 0, oax = 0, oay = 0, oaz = 0, keepx = 0, keepy = 0, keepz = 0;
+    if (ODD) {                      // the single sink lives in the low half of pair NP
+        float t;
+        upk(k.nx[NP], ox, t); upk(k.ny[NP], oy, t); upk(k.nz[NP], oz, t);
+        upk(k.sx[NP], oax, keepx); upk(k.sy[NP], oay, keepy); upk(k.sz[NP], oaz, keepz);
+    }
     for (int j = 0; j < cnt; j += step, p += step) {
         float4 s[U];
 #pragma unroll
         for (int u = 0; u < U; u++) s[u] = p[u * P];
+        f2 dx[U][NP > 0 ? NP : 1], dy[U][NP > 0 ? NP : 1], dz[U][NP > 0 ? NP : 1], w[U][NP > 0 ? NP : 1];
+        float ex[U], ey[U], ez[U], ew[U];
 #pragma unroll
         for (int u = 0; u < U; u++) {
 #pragma unroll
-            for (int q = 0; q < S / 2; q++) mono2(s[u], k.nx[q], k.ny[q], k.nz[q], eps2, k.sx[q], k.sy[q], k.sz[q]);
-            if (S & 1) mono1(s[u], k.nx[S / 2], k.ny[S / 2], k.nz[S / 2], eps2, k.sx[S / 2], k.sy[S / 2], k.sz[S / 2]);
+            for (int q = 0; q < NP; q++) {
+                dx[u][q] = add2(pk(s[u].x, s[u].x), k.nx[q]);
+                dy[u][q] = add2(pk(s[u].y, s[u].y), k.ny[q]);
+                dz[u][q] = add2(pk(s[u].z, s[u].z), k.nz[q]);
+            }
+            if (ODD) { ex[u] = s[u].x + ox; ey[u] = s[u].y + oy; ez[u] = s[u].z + oz; }
+        }
+#pragma unroll
+        for (int u = 0; u < U; u++) {
+#pragma unroll
+            for (int q = 0; q < NP; q++) w[u][q] = fma2(dx[u][q], dx[u][q], EPS);
+            if (ODD) ew[u] = fmaf(ex[u], ex[u], eps2);
+        }
+#pragma unroll
+        for (int u = 0; u < U; u++) {
+#pragma unroll
+            for (int q = 0; q < NP; q++) w[u][q] = fma2(dy[u][q], dy[u][q], w[u][q]);
+            if (ODD) ew[u] = fmaf(ey[u], ey[u], ew[u]);
+        }
+#pragma unroll
+        for (int u = 0; u < U; u++) {
+#pragma unroll
+            for (int q = 0; q < NP; q++) w[u][q] = fma2(dz[u][q], dz[u][q], w[u][q]);
+            if (ODD) ew[u] = fmaf(ez[u], ez[u], ew[u]);
+        }
+#pragma unroll
+        for (int u = 0; u < U; u++) {
+#pragma unroll
+            for (int q = 0; q < NP; q++) {
+                float a, b;
+                upk(w[u][q], a, b);
+                w[u][q] = pk(rsqrt_approx(a), rsqrt_approx(b));
+            }
+            if (ODD) ew[u] = rsqrt_approx(ew[u]);
+        }
+#pragma unroll
+        for (int u = 0; u < U; u++) {
+#pragma unroll
+            for (int q = 0; q < NP; q++) {
+                const f2 ri2 = mul2(w[u][q], w[u][q]);
+                const f2 mr = mul2(pk(s[u].w, s[u].w), w[u][q]);
+                w[u][q] = mul2(mr, ri2);
+            }
+            if (ODD) { const float ri2 = ew[u] * ew[u]; const float mr = s[u].w * ew[u]; ew[u] = mr * ri2; }
+        }
+#pragma unroll
+        for (int u = 0; u < U; u++) {
+#pragma unroll
+            for (int q = 0; q < NP; q++) {
+                k.sx[q] = fma2(w[u][q], dx[u][q], k.sx[q]);
+                k.sy[q] = fma2(w[u][q], dy[u][q], k.sy[q]);
+                k.sz[q] = fma2(w[u][q], dz[u][q], k.sz[q]);
+            }
+            if (ODD) { oax = fmaf(ew[u], ex[u], oax); oay = fmaf(ew[u], ey[u], oay); oaz = fmaf(ew[u], ez[u], oaz); }
         }
     }
+    if (ODD) { k.sx[NP] = pk(oax, keepx); k.sy[NP] = pk(oay, keepy); k.sz[NP] = pk(oaz, keepz); }
 }
 
 template <int S, int U, bool SOFT>
