@@ -40,7 +40,11 @@ def clock_sampler(stop, out, index):
                  nv.nvmlClocksThrottleReasonSwThermalSlowdown: "sw_thermal_slowdown",
                  nv.nvmlClocksThrottleReasonHwThermalSlowdown: "hw_thermal_slowdown",
                  nv.nvmlClocksThrottleReasonHwPowerBrakeSlowdown: "hw_power_brake"}
+        out["ready"].set()
         while not stop.is_set():
+            if not out["go"].is_set():
+                time.sleep(0.001)
+                continue
             out["samples"].append(nv.nvmlDeviceGetClockInfo(h, nv.NVML_CLOCK_SM))
             r = nv.nvmlDeviceGetCurrentClocksThrottleReasons(h)
             for bit, nm in names.items():
@@ -49,6 +53,7 @@ def clock_sampler(stop, out, index):
             time.sleep(0.002)
     except Exception as e:  # noqa: BLE001
         out["error"] = repr(e)
+        out["ready"].set()
 
 
 def oracle_sample(cfg, pos, seconds):
@@ -151,10 +156,12 @@ def main():
     h.export("interactions"); h.export("timings")
     launches0 = int(h.export("counts")[6])
 
-    clk = {"samples": [], "reasons": set()}
+    clk = {"samples": [], "reasons": set(), "ready": threading.Event(), "go": threading.Event()}
     stop = threading.Event()
     th = threading.Thread(target=clock_sampler, args=(stop, clk, local_rank), daemon=True)
     th.start()
+    clk["ready"].wait(30.0)                                     # NVML initialised before the timed region starts
+    clk["go"].set()
     if world > 1:
         dist.barrier()
     torch.cuda.synchronize()
