@@ -529,6 +529,18 @@ void orc_walk_counts(const orc_tree *t, int mode, uint32_t *ncell, uint32_t *npa
     }
 }
 
+/* the same for the groups in gsel only: entry k of each output belongs to group gsel[k] */
+void orc_walk_counts_sel(const orc_tree *t, int mode, int64_t ngsel, const int64_t *gsel,
+                         uint32_t *ncell, uint32_t *npart, uint32_t *nhard)
+{
+#pragma omp parallel for schedule(dynamic, 16)
+    for (int64_t k = 0; k < ngsel; k++) {
+        walk_out w; memset(&w, 0, sizeof w);
+        walk_group(t, mode, gsel[k], &w, 0);
+        ncell[k] = (uint32_t)w.ncells; npart[k] = (uint32_t)w.npart; nhard[k] = (uint32_t)w.nhard;
+    }
+}
+
 int orc_walk_lists(const orc_tree *t, int mode, int64_t g,
                    uint32_t *cells, int64_t cap_cells, int64_t *ncells,
                    uint32_t *parts, uint8_t *hard, int64_t cap_parts, int64_t *nparts)

@@ -91,6 +91,9 @@ int64_t orc_tree_get(const orc_tree *t, int what, void *dst, int64_t bytes);
 
 /* T12-T13: list lengths per group. */
 void orc_walk_counts(const orc_tree *t, int mode, uint32_t *ncell, uint32_t *npart, uint32_t *nhard);
+/* T12-T13 for the ngsel groups listed in gsel: output entry k belongs to group gsel[k]. */
+void orc_walk_counts_sel(const orc_tree *t, int mode, int64_t ngsel, const int64_t *gsel,
+                         uint32_t *ncell, uint32_t *npart, uint32_t *nhard);
 /* list contents for one group: cells = node ids, parts = sorted-order particle indices,
  * hard[k] = 1 if parts[k] is on the hard list. Returns 0, or -1 if a capacity is too small. */
 int orc_walk_lists(const orc_tree *t, int mode, int64_t g,

@@ -49,6 +49,7 @@ def lib():
         L.orc_tree_get.restype = C.c_int64
         L.orc_tree_get.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_int64]
         L.orc_walk_counts.argtypes = [C.c_void_p, C.c_int] + [C.c_void_p] * 3
+        L.orc_walk_counts_sel.argtypes = [C.c_void_p, C.c_int, C.c_int64] + [C.c_void_p] * 4
         L.orc_walk_lists.restype = C.c_int
         L.orc_walk_lists.argtypes = [C.c_void_p, C.c_int, C.c_int64, C.c_void_p, C.c_int64, C.c_void_p,
                                      C.c_void_p, C.c_void_p, C.c_int64, C.c_void_p]
@@ -121,7 +122,13 @@ class Tree:
         assert got == out.nbytes, (name, got, out.nbytes)
         return out[0] if which == "one" and w > 1 else out
 
-    def walk_counts(self, mode: int):
+    def walk_counts(self, mode: int, gsel=None):
+        if gsel is not None:
+            gsel = np.ascontiguousarray(gsel, dtype=np.int64)
+            k = len(gsel)
+            nc = np.zeros(k, np.uint32); npart = np.zeros(k, np.uint32); nh = np.zeros(k, np.uint32)
+            lib().orc_walk_counts_sel(self._h, mode, k, _p(gsel), _p(nc), _p(npart), _p(nh))
+            return nc, npart, nh
         nc = np.zeros(self.ng, np.uint32); npart = np.zeros(self.ng, np.uint32); nh = np.zeros(self.ng, np.uint32)
         lib().orc_walk_counts(self._h, mode, _p(nc), _p(npart), _p(nh))
         return nc, npart, nh

@@ -44,11 +44,13 @@ def compare_tree(h, t, abs_mode=False):
     assert np.array_equal(h.export("ghi")[:, :3], t.get("ghi"))
 
 
-def compare_lists(h, t, mode):
-    nc, npart, nh = t.walk_counts(mode)
-    assert np.array_equal(h.export("ncell"), nc)
-    assert np.array_equal(h.export("npart"), npart)
-    assert np.array_equal(h.export("nhard"), nh)
+def compare_lists(h, t, mode, gsel=None):
+    """list lengths per group (T13), bit-exact; gsel: only those groups (sampled check)."""
+    nc, npart, nh = t.walk_counts(mode, gsel)
+    sel = slice(None) if gsel is None else np.asarray(gsel)
+    assert np.array_equal(h.export("ncell")[sel], nc)
+    assert np.array_equal(h.export("npart")[sel], npart)
+    assert np.array_equal(h.export("nhard")[sel], nh)
 
 
 def acc_errors(a_gpu, a_ref, a_tot_ref):
@@ -60,12 +62,14 @@ def acc_errors(a_gpu, a_ref, a_tot_ref):
     return float(np.sqrt(np.mean(err ** 2))), float(err.max())
 
 
-def check_forces(h, t, split=True, gsel=None):
-    """runs soft (and hard) force on the GPU and compares with the oracle (T14)."""
+def check_forces(h, t, split=True, gsel=None, lists_full=True):
+    """runs soft (and hard) force on the GPU and compares with the oracle (T14).
+    gsel: accelerations only on those groups; lists_full=False: list lengths on gsel only."""
     mode = O.MODE_HYBRID if split else O.MODE_NORMAL
     h.soft_force()
     h.sync()
-    compare_lists(h, t, mode)
+    lsel = None if lists_full else gsel
+    compare_lists(h, t, mode, lsel)
     a_s, a_h, inter = t.forces(mode, gsel)
     gs = h.a_soft.cpu().numpy()[:, :3]; gh = h.a_hard.cpu().numpy()[:, :3]
     if gsel is not None:
@@ -84,7 +88,7 @@ def check_forces(h, t, split=True, gsel=None):
         h.a_hard.zero_()
         h.hard_force()
         h.sync()
-        compare_lists(h, t, O.MODE_HARD)
+        compare_lists(h, t, O.MODE_HARD, lsel)
         gh2 = h.a_hard.cpu().numpy()[:, :3]
         rms, mx = acc_errors(gh2[idx], a_h[idx], tot)
         assert rms < RMS_TOL and mx < MAX_TOL, ("hard-only", rms, mx)
