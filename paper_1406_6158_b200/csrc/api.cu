@@ -25,6 +25,7 @@ Layout plan_workspace(int64_t n)
     L.rs_tiles = (n + RS_TILE - 1) / RS_TILE;
     L.node_tiles = (L.node_cap + RS_TILE - 1) / RS_TILE;
     L.sc_tiles = (n + SC_TILE - 1) / SC_TILE;
+    L.po_tiles = (n + PO_TILE - 1) / PO_TILE;
     size_t off = 0;
     auto take = [&](size_t bytes) { size_t o = off; off = align_up(off + bytes); return o; };
     const size_t N = (size_t)n, NC = (size_t)L.node_cap, GC = (size_t)L.group_cap;
@@ -33,14 +34,14 @@ Layout plan_workspace(int64_t n)
     L.val_a = take(4 * N); L.val_b = take(4 * N);
     L.pos_tmp = take(16 * N); L.vel_tmp = take(16 * N); L.id_tmp = take(4 * N);
     L.rs_status = take(4 * 256 * (size_t)L.rs_tiles * RS_PASSES);
-    L.sc_status = take(8 * 2 * (size_t)L.sc_tiles);
+    L.sc_status = take(8 * (size_t)(L.sc_tiles + L.po_tiles));
     L.dlev = take(N); L.cnt_slot = take(4 * N); L.gflag = take(N);
     L.pre_level = take(NC); L.pre_first = take(4 * NC); L.pre_of_bfs = take(4 * NC); L.bfs_of_pre = take(4 * NC);
     L.node_status = take(4 * 256 * (size_t)L.node_tiles);
     L.level = take(NC); L.first = take(4 * NC); L.count = take(4 * NC); L.child = take(4 * NC);
     L.nchild = take(NC); L.parent = take(4 * NC); L.arrived = take(4 * NC);
     L.nodes = take(sizeof(NodeRec) * NC);
-    L.M64 = take(8 * NC); L.S64 = take(24 * NC); L.C64 = take(24 * NC); L.B2 = take(8 * NC); L.bmax2 = take(8 * NC);
+    L.MS64 = take(32 * NC); L.C64 = take(24 * NC); L.B2 = take(8 * NC); L.bmax2 = take(8 * NC);
     L.leaf_of = take(4 * N);
     L.gfirst = take(4 * GC); L.gcount = take(4 * GC); L.glo = take(16 * GC); L.ghi = take(16 * GC);
     L.ncell = take(4 * GC); L.npart = take(4 * GC); L.nhard = take(4 * GC);
@@ -157,6 +158,13 @@ int hyb_init(hyb_ctx **out, const hyb_params *params, int64_t n, hyb_float4 *d_p
     if (e != cudaSuccess) { delete c; return cuda_fail(nullptr, e, "cudaDeviceGetAttribute"); }
     for (int i = 0; i < 5; i++) {
         e = cudaEventCreate(&c->ev[i]);
+        if (e != cudaSuccess) { delete c; return cuda_fail(nullptr, e, "cudaEventCreate"); }
+    }
+    e = cudaStreamCreateWithFlags(&c->aux, cudaStreamNonBlocking);
+    if (e != cudaSuccess) { delete c; return cuda_fail(nullptr, e, "cudaStreamCreate"); }
+    cudaEvent_t *evs[4] = {&c->ev_sorted, &c->ev_perm, &c->ev_linked, &c->ev_groups};
+    for (int i = 0; i < 4; i++) {
+        e = cudaEventCreateWithFlags(evs[i], cudaEventDisableTiming);
         if (e != cudaSuccess) { delete c; return cuda_fail(nullptr, e, "cudaEventCreate"); }
     }
     c->timing = true;
@@ -336,7 +344,14 @@ int hyb_export(hyb_ctx *ctx, int32_t what, void *host_dst, size_t bytes, size_t 
     case HYB_X_NCELL: src = c->ws + L.ncell; sz = 4 * ng; break;
     case HYB_X_NPART: src = c->ws + L.npart; sz = 4 * ng; break;
     case HYB_X_NHARD: src = c->ws + L.nhard; sz = 4 * ng; break;
-    case HYB_X_M64: src = c->ws + L.M64; sz = 8 * nn; break;
+    case HYB_X_M64:                                                            // strided field of (M, Sx, Sy, Sz)
+        if (bytes < 8 * nn) return fail(c, HYB_ERR_INVALID_ARG, "buffer too small");
+        if (nn) {
+            e = cudaMemcpy2D(host_dst, 8, c->ws + L.MS64, 32, 8, nn, cudaMemcpyDeviceToHost);
+            if (e != cudaSuccess) return cuda_fail(c, e, "hyb_export copy");
+        }
+        if (written) *written = 8 * nn;
+        return HYB_OK;
     case HYB_X_C64: src = c->ws + L.C64; sz = 24 * nn; break;
     case HYB_X_B2: src = c->ws + L.B2; sz = 8 * nn; break;
     case HYB_X_BMAX: {
@@ -410,6 +425,9 @@ void hyb_free(hyb_ctx *ctx)
     Ctx *c = reinterpret_cast<Ctx *>(ctx);
     if (!c) return;
     for (int i = 0; i < 5; i++) if (c->ev[i]) cudaEventDestroy(c->ev[i]);
+    if (c->aux) { cudaStreamSynchronize(c->aux); cudaStreamDestroy(c->aux); }
+    cudaEvent_t evs[4] = {c->ev_sorted, c->ev_perm, c->ev_linked, c->ev_groups};
+    for (int i = 0; i < 4; i++) if (evs[i]) cudaEventDestroy(evs[i]);
     delete c;
 }
 

@@ -30,8 +30,10 @@ constexpr int RS_PASSES = 8;      // 8 x 8 bits >= 63 bits
 
 // single-value scan tiles (octree preorder, group compaction)
 constexpr int SC_THREADS = 256;
-constexpr int SC_IPT = 4;
+constexpr int SC_IPT = 16;
 constexpr int SC_TILE = SC_THREADS * SC_IPT;
+constexpr int PO_IPT = 4;                // octree preorder: heavy per-item work, small tiles
+constexpr int PO_TILE = SC_THREADS * PO_IPT;
 
 // walk kernel geometry
 constexpr int WK_WARPS = 8;              // warps per CTA
@@ -76,19 +78,19 @@ struct Layout {   // byte offsets into the workspace; computed by plan_workspace
     size_t key_orig, key_a, key_b, val_a, val_b;
     size_t pos_tmp, vel_tmp, id_tmp;
     size_t rs_status;           // [RS_PASSES][ntiles][256] u32
-    size_t sc_status;           // [2][nsc_tiles] u64   (preorder scan, group scan)
+    size_t sc_status;           // u64 [po_tiles] (preorder scan) then [sc_tiles] (group scan)
     size_t dlev, cnt_slot;      // int8[n], u32[n]
     size_t gflag;               // u8[n]
     size_t pre_level, pre_first, pre_of_bfs, bfs_of_pre;   // u8, u32, u32, u32 [node_cap]
     size_t node_status;         // [ntiles(node_cap)][256] u32
     size_t level, first, count, child, nchild, parent, arrived;
     size_t nodes;                              // NodeRec[node_cap]
-    size_t M64, S64, C64, B2, bmax2;           // double[nc], [3nc], [3nc], [nc], u64[nc]
+    size_t MS64, C64, B2, bmax2;               // double[4nc] (M, Sx, Sy, Sz), [3nc], [nc], u64[nc]
     size_t leaf_of;             // u32[n]
     size_t gfirst, gcount, glo, ghi, ncell, npart, nhard;   // [group_cap]
     size_t total;
     int64_t n, node_cap, group_cap;
-    int64_t rs_tiles, node_tiles, sc_tiles;
+    int64_t rs_tiles, node_tiles, sc_tiles, po_tiles;
 };
 
 inline int64_t node_capacity(int64_t n) { return 2 * n + 4096; }
@@ -100,6 +102,8 @@ struct Ctx {
     int64_t n;
     int device;
     cudaStream_t stream;
+    cudaStream_t aux;              // library-owned: runs the parts of a build that are off the critical path
+    cudaEvent_t ev_sorted, ev_perm, ev_linked, ev_groups;
     int num_sms;
     hyb_float4 *pos, *vel, *a_soft, *a_hard;
     u32 *id;
@@ -153,14 +157,62 @@ __device__ __forceinline__ u64 lookback_single(u64 *status, u32 tile, u64 aggreg
     if (tile == 0) { st[0] = LB_PREFIX | aggregate; return 0; }
     st[tile] = LB_AGG | aggregate;
     u64 excl = 0;
-    for (long long t = (long long)tile - 1; t >= 0; --t) {
-        u64 s; int spins = 0;
-        do { s = st[t]; } while ((s >> 62) == 0 && ++spins < LB_SPIN_LIMIT);
-        if ((s >> 62) == 0) { atomicOr(dev_status, ST_WAIT_EXPIRED); break; }
-        excl += s & LB_MASK;
-        if ((s >> 62) == 2) break;
+    long long t = (long long)tile - 1;
+    int spins = 0;
+    bool done = false;
+    constexpr int WIN = 16;          // predecessors requested together (divides the round trips)
+    while (!done) {
+        u64 s[WIN];
+#pragma unroll
+        for (int i = 0; i < WIN; i++) s[i] = (t - i >= 0) ? st[t - i] : (2ull << 62);
+#pragma unroll
+        for (int i = 0; i < WIN; i++) {
+            if (done) break;
+            const u64 f = s[i] >> 62;
+            if (f == 0) break;               // not published yet: poll again from here
+            excl += s[i] & LB_MASK;
+            t--;
+            if (f == 2) done = true;
+        }
+        if (!done && ++spins >= LB_SPIN_LIMIT) { atomicOr(dev_status, ST_WAIT_EXPIRED); break; }
     }
     st[tile] = LB_PREFIX | (excl + aggregate);
+    return excl;
+}
+
+// The same with the 32 lanes of one warp each inspecting a different predecessor.  Called by all lanes
+// of ONE warp of the CTA that owns `tile`; every lane returns the exclusive prefix.
+__device__ __forceinline__ u64 lookback_warp(u64 *status, u32 tile, u64 aggregate, u32 *dev_status, int lane)
+{
+    volatile u64 *st = status;
+    if (tile == 0) {
+        if (lane == 0) st[0] = LB_PREFIX | aggregate;
+        return 0;
+    }
+    if (lane == 0) st[tile] = LB_AGG | aggregate;
+    u64 excl = 0;
+    long long t = (long long)tile - 1;
+    int spins = 0;
+    for (;;) {
+        const long long idx = t - lane;
+        const u64 s = idx >= 0 ? st[idx] : (2ull << 62);
+        const u32 f = (u32)(s >> 62);
+        const u32 notready = __ballot_sync(0xFFFFFFFFu, f == 0u), prefix = __ballot_sync(0xFFFFFFFFu, f == 2u);
+        const int lim_nr = notready ? __ffs(notready) - 1 : 32, lim_p = prefix ? __ffs(prefix) - 1 : 32;
+        const bool done = lim_p < lim_nr;
+        const int use = done ? lim_p + 1 : lim_nr;          // lanes 0 .. use-1 contribute
+        u64 v = lane < use ? (s & LB_MASK) : 0ull;
+#pragma unroll
+        for (int off = 16; off; off >>= 1) v += __shfl_xor_sync(0xFFFFFFFFu, v, off);
+        excl += v;
+        if (done) break;
+        t -= use;
+        if (use == 0 && ++spins >= LB_SPIN_LIMIT) {
+            if (lane == 0) atomicOr(dev_status, ST_WAIT_EXPIRED);
+            break;
+        }
+    }
+    if (lane == 0) st[tile] = LB_PREFIX | (excl + aggregate);
     return excl;
 }
 

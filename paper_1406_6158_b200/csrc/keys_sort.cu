@@ -133,7 +133,9 @@ cudaError_t launch_keys_sort_permute(Ctx *c)
     root_cube_kernel<<<1, 1, 0, st>>>(ctl);
     u64 *key_orig = wsptr<u64>(c, L.key_orig), *key_a = wsptr<u64>(c, L.key_a), *key_b = wsptr<u64>(c, L.key_b);
     u32 *val_a = wsptr<u32>(c, L.val_a), *val_b = wsptr<u32>(c, L.val_b);
-    keys_kernel<<<grid, 256, 0, st>>>(reinterpret_cast<const float4 *>(c->pos), n, ctl, key_orig);
+    // few CTAs: every CTA ends with up to 2048 global atomics for its share of the digit histograms
+    const int kgrid = (int)imin64((c->n + 255) / 256, (int64_t)c->num_sms * 2);
+    keys_kernel<<<kgrid, 256, 0, st>>>(reinterpret_cast<const float4 *>(c->pos), n, ctl, key_orig);
     digit_base_kernel<<<RS_PASSES, 256, 0, st>>>(ctl);
 
     u32 *status = wsptr<u32>(c, L.rs_status);
@@ -148,14 +150,20 @@ cudaError_t launch_keys_sort_permute(Ctx *c)
         if (e != cudaSuccess) return e;
         kin = kout; vin = vout;
     }
-    // RS_PASSES is even: sorted keys in key_b, permutation in val_b
+    // RS_PASSES is even: sorted keys in key_b, permutation in val_b.
+    // The re-order of the store runs on the auxiliary stream, next to the octree build (which needs
+    // only the sorted keys); later stages read the permuted positions from pos_tmp.
+    cudaStream_t ax = c->aux;
+    cudaEventRecord(c->ev_sorted, st);
+    cudaStreamWaitEvent(ax, c->ev_sorted, 0);
     float4 *pos_t = wsptr<float4>(c, L.pos_tmp), *vel_t = wsptr<float4>(c, L.vel_tmp);
     u32 *id_t = wsptr<u32>(c, L.id_tmp);
-    permute_kernel<<<grid, 256, 0, st>>>(val_b, n, reinterpret_cast<const float4 *>(c->pos),
+    permute_kernel<<<grid, 256, 0, ax>>>(val_b, n, reinterpret_cast<const float4 *>(c->pos),
                                          reinterpret_cast<const float4 *>(c->vel), c->id, pos_t, vel_t, id_t);
-    cudaMemcpyAsync(c->pos, pos_t, sizeof(float4) * (size_t)n, cudaMemcpyDeviceToDevice, st);
-    cudaMemcpyAsync(c->vel, vel_t, sizeof(float4) * (size_t)n, cudaMemcpyDeviceToDevice, st);
-    cudaMemcpyAsync(c->id, id_t, sizeof(u32) * (size_t)n, cudaMemcpyDeviceToDevice, st);
+    cudaEventRecord(c->ev_perm, ax);
+    cudaMemcpyAsync(c->pos, pos_t, sizeof(float4) * (size_t)n, cudaMemcpyDeviceToDevice, ax);
+    cudaMemcpyAsync(c->vel, vel_t, sizeof(float4) * (size_t)n, cudaMemcpyDeviceToDevice, ax);
+    cudaMemcpyAsync(c->id, id_t, sizeof(u32) * (size_t)n, cudaMemcpyDeviceToDevice, ax);
     return cudaGetLastError();
 }
 

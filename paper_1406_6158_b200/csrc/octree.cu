@@ -9,6 +9,7 @@
 //   bfs      : one stable counting-sort pass by level turns preorder into breadth-first order.
 //   link     : every node finds its range end, children and parent by binary search in the keys.
 //   upsweep  : leaves first, the last child to arrive computes the parent (fixed summation order).
+#include <stdlib.h>
 #include "common.cuh"
 #include "sort.cuh"
 
@@ -28,14 +29,14 @@ __global__ void __launch_bounds__(SC_THREADS) preorder_kernel(
     signed char *__restrict__ dlev, u32 *__restrict__ slot, unsigned char *__restrict__ pre_level,
     u32 *__restrict__ pre_first)
 {
-    __shared__ u64 s_key[SC_TILE + 2 * PO_HALO];
-    __shared__ signed char s_w[SC_TILE + PO_HALO];
+    __shared__ u64 s_key[PO_TILE + 2 * PO_HALO];
+    __shared__ signed char s_w[PO_TILE + PO_HALO];
     __shared__ u32 s_hist[MAXLEVEL + 1];
     __shared__ u32 s_warp[SC_THREADS / 32];
     __shared__ u32 s_tile;
     __shared__ u64 s_prefix;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const u32 ntiles = (n + SC_TILE - 1) / SC_TILE;
+    const u32 ntiles = (n + PO_TILE - 1) / PO_TILE;
     for (;;) {
         __syncthreads();
         if (tid == 0) s_tile = atomicAdd(&ctl->tile_counter[8], 1u);
@@ -43,24 +44,24 @@ __global__ void __launch_bounds__(SC_THREADS) preorder_kernel(
         __syncthreads();
         const u32 tile = s_tile;
         if (tile >= ntiles) break;
-        const long long t0 = (long long)tile * SC_TILE;
-        for (int q = tid; q < SC_TILE + 2 * PO_HALO; q += SC_THREADS) {
+        const long long t0 = (long long)tile * PO_TILE;
+        for (int q = tid; q < PO_TILE + 2 * PO_HALO; q += SC_THREADS) {
             long long g = t0 - PO_HALO + q;
             s_key[q] = (g >= 0 && g < (long long)n) ? key[g] : 0ull;
         }
         __syncthreads();
-        for (int q = tid; q < SC_TILE + PO_HALO; q += SC_THREADS) {       // w(s), s = t0 - HALO + q
+        for (int q = tid; q < PO_TILE + PO_HALO; q += SC_THREADS) {       // w(s), s = t0 - HALO + q
             long long s = t0 - PO_HALO + q;
             int w = -1;
             if (s >= 0 && s + leaf_max < (long long)n) w = lcp_levels(s_key[q], s_key[q + leaf_max]);
             s_w[q] = (signed char)w;
         }
         __syncthreads();
-        int d[SC_IPT], cnt[SC_IPT];
+        int d[PO_IPT], cnt[PO_IPT];
         u32 mysum = 0;
 #pragma unroll
-        for (int k = 0; k < SC_IPT; k++) {
-            const int li = tid * SC_IPT + k;                 // local index in tile
+        for (int k = 0; k < PO_IPT; k++) {
+            const int li = tid * PO_IPT + k;                 // local index in tile
             const long long i = t0 + li;
             d[k] = 0; cnt[k] = 0;
             if (i < (long long)n) {
@@ -84,10 +85,10 @@ __global__ void __launch_bounds__(SC_THREADS) preorder_kernel(
         u32 wbase = 0, tile_total = 0;
 #pragma unroll
         for (int w = 0; w < SC_THREADS / 32; w++) { if (w < warp) wbase += s_warp[w]; tile_total += s_warp[w]; }
-        if (tid == 0) {
-            u64 pre = lookback_single(sc_status, tile, tile_total, &ctl->status);
-            s_prefix = pre;
-            if (tile == ntiles - 1) {
+        if (warp == 0) {
+            const u64 pre = lookback_warp(sc_status, tile, tile_total, &ctl->status, lane);
+            if (lane == 0) s_prefix = pre;
+            if (lane == 0 && tile == ntiles - 1) {
                 u64 tot = pre + tile_total;
                 ctl->nn_total = (u32)min(tot, (u64)0xFFFFFFFFu);
                 ctl->nn = (u32)min(tot, (u64)node_cap);
@@ -97,8 +98,8 @@ __global__ void __launch_bounds__(SC_THREADS) preorder_kernel(
         __syncthreads();
         u64 p = s_prefix + wbase + incl - mysum;
 #pragma unroll
-        for (int k = 0; k < SC_IPT; k++) {
-            const long long i = t0 + tid * SC_IPT + k;
+        for (int k = 0; k < PO_IPT; k++) {
+            const long long i = t0 + tid * PO_IPT + k;
             if (i < (long long)n) {
                 dlev[i] = (signed char)d[k];
                 slot[i] = (u32)min(p, (u64)0xFFFFFFFFu);
@@ -144,7 +145,6 @@ __device__ __forceinline__ u32 lower_bound_key(const u64 *__restrict__ key, u32 
     }
     return lo;
 }
-
 __global__ void __launch_bounds__(256) link_kernel(
     const u64 *__restrict__ key, u32 n, int leaf_max, const DevCtl *__restrict__ ctl,
     const unsigned char *__restrict__ level, const u32 *__restrict__ pre_of_bfs, const u32 *__restrict__ bfs_of_pre,
@@ -195,9 +195,17 @@ struct NodeArrays {
     const unsigned char *nchild, *level;
     u32 *arrived;
     NodeRec *rec;               // A = com_m, B = lo | ropen2, C = hi | 0
-    double *M64, *S64, *C64, *B2;
+    double4 *MS64;              // (M, Sx, Sy, Sz) before the division
+    double *C64, *B2;
     u32 *leaf_of;
 };
+
+__device__ __forceinline__ double4 ldcg_d4(const double4 *p)
+{
+    const double2 *q = reinterpret_cast<const double2 *>(p);
+    const double2 a = __ldcg(q), b = __ldcg(q + 1);
+    return make_double4(a.x, a.y, b.x, b.y);
+}
 
 __device__ __forceinline__ double dist2_rn(double ax, double ay, double az, double bx, double by, double bz)
 {
@@ -220,8 +228,7 @@ __device__ __forceinline__ void finish_node(const NodeArrays &na, u32 b, int lev
     na.rec[b].A = make_float4(__double2float_rn(Cx), __double2float_rn(Cy), __double2float_rn(Cz), __double2float_rn(M));
     na.rec[b].B = make_float4(lo.x, lo.y, lo.z, ropen2);
     na.rec[b].C = make_float4(hi.x, hi.y, hi.z, 0.0f);
-    na.M64[b] = M;
-    na.S64[3 * (size_t)b] = Sx; na.S64[3 * (size_t)b + 1] = Sy; na.S64[3 * (size_t)b + 2] = Sz;
+    na.MS64[b] = make_double4(M, Sx, Sy, Sz);
     na.C64[3 * (size_t)b] = Cx; na.C64[3 * (size_t)b + 1] = Cy; na.C64[3 * (size_t)b + 2] = Cz;
 }
 
@@ -266,34 +273,34 @@ __global__ void __launch_bounds__(128) upsweep_kernel(NodeArrays na, const float
     for (;;) {
         const u32 par = na.parent[cur];
         if (par == NOCHILD) break;
+        const u32 nc = na.nchild[par], c0 = na.child[par];      // topology: requested before the fence
+        const int plev = na.level[par];
         __threadfence();
         const u32 old = atomicAdd(&na.arrived[par], 1u);
-        const u32 nc = na.nchild[par];
         if (old + 1 != nc) break;
         __threadfence();
-        const u32 c0 = na.child[par];
         double M = 0.0, Sx = 0.0, Sy = 0.0, Sz = 0.0;
         float3 lo, hi;
-        for (u32 q = c0; q < c0 + nc; q++) {
-            M = __dadd_rn(M, __ldcg(na.M64 + q));
-            Sx = __dadd_rn(Sx, __ldcg(na.S64 + 3 * (size_t)q));
-            Sy = __dadd_rn(Sy, __ldcg(na.S64 + 3 * (size_t)q + 1));
-            Sz = __dadd_rn(Sz, __ldcg(na.S64 + 3 * (size_t)q + 2));
-            float4 bl = __ldcg(&na.rec[q].B), bh = __ldcg(&na.rec[q].C);
-            if (q == c0) { lo = make_float3(bl.x, bl.y, bl.z); hi = make_float3(bh.x, bh.y, bh.z); }
-            else {
-                lo.x = fminf(lo.x, bl.x); lo.y = fminf(lo.y, bl.y); lo.z = fminf(lo.z, bl.z);
-                hi.x = fmaxf(hi.x, bh.x); hi.y = fmaxf(hi.y, bh.y); hi.z = fmaxf(hi.z, bh.z);
+        {
+            for (u32 q = c0; q < c0 + nc; q++) {
+                const double4 cm = ldcg_d4(na.MS64 + q);
+                M = __dadd_rn(M, cm.x); Sx = __dadd_rn(Sx, cm.y); Sy = __dadd_rn(Sy, cm.z); Sz = __dadd_rn(Sz, cm.w);
+                const float4 bl = __ldcg(&na.rec[q].B), bh = __ldcg(&na.rec[q].C);
+                if (q == c0) { lo = make_float3(bl.x, bl.y, bl.z); hi = make_float3(bh.x, bh.y, bh.z); }
+                else {
+                    lo.x = fminf(lo.x, bl.x); lo.y = fminf(lo.y, bl.y); lo.z = fminf(lo.z, bl.z);
+                    hi.x = fmaxf(hi.x, bh.x); hi.y = fmaxf(hi.y, bh.y); hi.z = fmaxf(hi.z, bh.z);
+                }
             }
         }
         double Cx, Cy, Cz;
-        finish_node(na, par, na.level[par], M, Sx, Sy, Sz, lo, hi, mac, Lf, theta, Cx, Cy, Cz);
+        finish_node(na, par, plev, M, Sx, Sy, Sz, lo, hi, mac, Lf, theta, Cx, Cy, Cz);
         if (mac == HYB_MAC_ABS) {            // parallel-axis sum of the children's B_2 (T10)
             double B2 = 0.0;
             for (u32 q = c0; q < c0 + nc; q++) {
                 double d2 = dist2_rn(__ldcg(na.C64 + 3 * (size_t)q), __ldcg(na.C64 + 3 * (size_t)q + 1),
                                      __ldcg(na.C64 + 3 * (size_t)q + 2), Cx, Cy, Cz);
-                B2 = __dadd_rn(B2, __dadd_rn(__ldcg(na.B2 + q), __dmul_rn(__ldcg(na.M64 + q), d2)));
+                B2 = __dadd_rn(B2, __dadd_rn(__ldcg(na.B2 + q), __dmul_rn(__ldcg(&na.MS64[q].x), d2)));
             }
             na.B2[par] = B2;
         }
@@ -385,7 +392,19 @@ __global__ void __launch_bounds__(SC_THREADS) gscan_kernel(const unsigned char *
         const u32 i0 = tile * SC_TILE + tid * SC_IPT;
         u32 fl[SC_IPT], mysum = 0;
 #pragma unroll
-        for (int k = 0; k < SC_IPT; k++) { fl[k] = (i0 + k < n) ? gflag[i0 + k] : 0u; mysum += fl[k]; }
+        for (int k = 0; k < SC_IPT; k++) fl[k] = 0u;
+        if (i0 + SC_IPT <= n) {                      // 16 flags in one 16-byte load
+            static_assert(SC_IPT == 16, "vector load of the flags assumes 16 items per thread");
+            const uint4 v = *reinterpret_cast<const uint4 *>(gflag + i0);
+            const u32 w[4] = {v.x, v.y, v.z, v.w};
+#pragma unroll
+            for (int k = 0; k < SC_IPT; k++) fl[k] = (w[k >> 2] >> (8 * (k & 3))) & 0xFFu;
+        } else {
+#pragma unroll
+            for (int k = 0; k < SC_IPT; k++) fl[k] = (i0 + k < n) ? gflag[i0 + k] : 0u;
+        }
+#pragma unroll
+        for (int k = 0; k < SC_IPT; k++) mysum += fl[k];
         u32 incl = mysum;
 #pragma unroll
         for (int off = 1; off < 32; off <<= 1) {
@@ -397,10 +416,10 @@ __global__ void __launch_bounds__(SC_THREADS) gscan_kernel(const unsigned char *
         u32 wbase = 0, tile_total = 0;
 #pragma unroll
         for (int w = 0; w < SC_THREADS / 32; w++) { if (w < warp) wbase += s_warp[w]; tile_total += s_warp[w]; }
-        if (tid == 0) {
-            u64 pre = lookback_single(sc_status, tile, tile_total, &ctl->status);
-            s_prefix = pre;
-            if (tile == ntiles - 1) ctl->ng = (u32)(pre + tile_total);
+        if (warp == 0) {
+            const u64 pre = lookback_warp(sc_status, tile, tile_total, &ctl->status, lane);
+            if (lane == 0) s_prefix = pre;
+            if (lane == 0 && tile == ntiles - 1) ctl->ng = (u32)(pre + tile_total);
         }
         __syncthreads();
         u32 g = (u32)s_prefix + wbase + incl - mysum;
@@ -409,24 +428,38 @@ __global__ void __launch_bounds__(SC_THREADS) gscan_kernel(const unsigned char *
     }
 }
 
+// eight lanes per group: each takes every eighth member, then the octet combines by shuffles
 __global__ void __launch_bounds__(256) ginfo_kernel(const DevCtl *__restrict__ ctl, u32 n,
                                                     const float4 *__restrict__ pos, const u32 *__restrict__ gfirst,
                                                     u32 *__restrict__ gcount, float4 *__restrict__ glo,
                                                     float4 *__restrict__ ghi)
 {
     const u32 ng = ctl->ng;
-    for (u32 g = blockIdx.x * blockDim.x + threadIdx.x; g < ng; g += gridDim.x * blockDim.x) {
-        const u32 f = gfirst[g], e = (g + 1 < ng) ? gfirst[g + 1] : n;
-        float4 p = __ldg(pos + f);
-        float3 lo = make_float3(p.x, p.y, p.z), hi = lo;
-        for (u32 j = f + 1; j < e; j++) {
-            p = __ldg(pos + j);
+    const u32 sub = threadIdx.x & 7u;
+    const u32 ngr = (ng + 31u) & ~31u;          // whole warps stay in the loop together (shuffles below)
+    for (u32 g = (blockIdx.x * blockDim.x + threadIdx.x) >> 3; g < ngr; g += (gridDim.x * blockDim.x) >> 3) {
+        const bool live = g < ng;
+        const u32 f = live ? gfirst[g] : 0u, e = live ? ((g + 1 < ng) ? gfirst[g + 1] : n) : 0u;
+        float3 lo = make_float3(INFINITY, INFINITY, INFINITY), hi = make_float3(-INFINITY, -INFINITY, -INFINITY);
+        for (u32 j = f + sub; j < e; j += 8) {
+            const float4 p = __ldg(pos + j);
             lo.x = fminf(lo.x, p.x); lo.y = fminf(lo.y, p.y); lo.z = fminf(lo.z, p.z);
             hi.x = fmaxf(hi.x, p.x); hi.y = fmaxf(hi.y, p.y); hi.z = fmaxf(hi.z, p.z);
         }
-        gcount[g] = e - f;
-        glo[g] = make_float4(lo.x, lo.y, lo.z, 0.0f);
-        ghi[g] = make_float4(hi.x, hi.y, hi.z, 0.0f);
+#pragma unroll
+        for (int off = 4; off; off >>= 1) {
+            lo.x = fminf(lo.x, __shfl_xor_sync(0xFFFFFFFFu, lo.x, off));
+            lo.y = fminf(lo.y, __shfl_xor_sync(0xFFFFFFFFu, lo.y, off));
+            lo.z = fminf(lo.z, __shfl_xor_sync(0xFFFFFFFFu, lo.z, off));
+            hi.x = fmaxf(hi.x, __shfl_xor_sync(0xFFFFFFFFu, hi.x, off));
+            hi.y = fmaxf(hi.y, __shfl_xor_sync(0xFFFFFFFFu, hi.y, off));
+            hi.z = fmaxf(hi.z, __shfl_xor_sync(0xFFFFFFFFu, hi.z, off));
+        }
+        if (live && sub == 0) {
+            gcount[g] = e - f;
+            glo[g] = make_float4(lo.x, lo.y, lo.z, 0.0f);
+            ghi[g] = make_float4(hi.x, hi.y, hi.z, 0.0f);
+        }
     }
 }
 
@@ -444,7 +477,7 @@ cudaError_t launch_build_tree(Ctx *c)
                     offsetof(DevCtl, bbox) - offsetof(DevCtl, bbox_enc), st);
     cudaMemsetAsync(reinterpret_cast<char *>(ctl) + offsetof(DevCtl, bbox_enc), 0xFF, 3 * sizeof(u32), st);
     cudaMemsetAsync(c->ws + L.rs_status, 0, sizeof(u32) * 256 * (size_t)L.rs_tiles * RS_PASSES, st);
-    cudaMemsetAsync(c->ws + L.sc_status, 0, sizeof(u64) * 2 * (size_t)L.sc_tiles, st);
+    cudaMemsetAsync(c->ws + L.sc_status, 0, sizeof(u64) * (size_t)(L.sc_tiles + L.po_tiles), st);
     cudaMemsetAsync(c->ws + L.node_status, 0, sizeof(u32) * 256 * (size_t)L.node_tiles, st);
     cudaMemsetAsync(c->ws + L.gflag, 0, (size_t)n, st);
 
@@ -458,7 +491,8 @@ cudaError_t launch_build_tree(Ctx *c)
     u32 *slot = wsptr<u32>(c, L.cnt_slot);
     unsigned char *pre_level = wsptr<unsigned char>(c, L.pre_level);
     u32 *pre_first = wsptr<u32>(c, L.pre_first);
-    preorder_kernel<<<sc_grid, SC_THREADS, 0, st>>>(key, n, c->p.leaf_max, (u32)L.node_cap, ctl, sc_status, dlev, slot,
+    const int po_grid = (int)imin64(L.po_tiles, (int64_t)c->num_sms * 8);
+    preorder_kernel<<<po_grid, SC_THREADS, 0, st>>>(key, n, c->p.leaf_max, (u32)L.node_cap, ctl, sc_status, dlev, slot,
                                                     pre_level, pre_first);
     level_offset_kernel<<<1, 32, 0, st>>>(ctl);
     unsigned char *level = wsptr<unsigned char>(c, L.level);
@@ -475,31 +509,36 @@ cudaError_t launch_build_tree(Ctx *c)
     NodeRec *rec = wsptr<NodeRec>(c, L.nodes);
     u64 *bmax2 = wsptr<u64>(c, L.bmax2);
     const int node_grid = (int)imin64((L.node_cap + 255) / 256, (int64_t)c->num_sms * 16);
-    link_kernel<<<node_grid, 256, 0, st>>>(key, n, c->p.leaf_max, ctl, level, pre_of_bfs, bfs_of_pre, pre_level,
-                                           pre_first, dlev, slot, first, count, child, nchild, parent, arrived, rec,
-                                           bmax2);
+    link_kernel<<<node_grid, 256, 0, st>>>(key, n, c->p.leaf_max, ctl, level, pre_of_bfs, bfs_of_pre, pre_level, pre_first,
+                                           dlev, slot, first, count, child, nchild, parent, arrived, rec, bmax2);
+    // sink groups need only the topology and the permuted positions: auxiliary stream, next to the upsweep
+    cudaStream_t ax = c->aux;
+    const float4 *pos_t = wsptr<float4>(c, L.pos_tmp);      // == the re-ordered store (copied back on aux)
+    cudaEventRecord(c->ev_linked, st);
+    cudaStreamWaitEvent(ax, c->ev_linked, 0);
+    unsigned char *gflag = wsptr<unsigned char>(c, L.gflag);
+    gmark_kernel<<<(int)((L.node_cap + 255) / 256), 256, 0, ax>>>(ctl, first, count, child, parent, c->p.group_max,
+                                                                  gflag);
+    u32 *gfirst = wsptr<u32>(c, L.gfirst);
+    gscan_kernel<<<sc_grid, SC_THREADS, 0, ax>>>(gflag, n, ctl, sc_status + L.po_tiles, gfirst);
+    ginfo_kernel<<<(int)imin64((c->n + 255) / 256, (int64_t)c->num_sms * 8), 256, 0, ax>>>(
+        ctl, n, pos_t, gfirst, wsptr<u32>(c, L.gcount), wsptr<float4>(c, L.glo), wsptr<float4>(c, L.ghi));
+    cudaEventRecord(c->ev_groups, ax);
+
     NodeArrays na;
     na.first = first; na.count = count; na.child = child; na.parent = parent; na.nchild = nchild; na.level = level;
     na.arrived = arrived;
     na.rec = rec;
-    na.M64 = wsptr<double>(c, L.M64); na.S64 = wsptr<double>(c, L.S64); na.C64 = wsptr<double>(c, L.C64);
+    na.MS64 = wsptr<double4>(c, L.MS64); na.C64 = wsptr<double>(c, L.C64);
     na.B2 = wsptr<double>(c, L.B2); na.leaf_of = wsptr<u32>(c, L.leaf_of);
     const int full_node_grid = (int)((L.node_cap + 127) / 128);
-    upsweep_kernel<<<full_node_grid, 128, 0, st>>>(na, reinterpret_cast<const float4 *>(c->pos), ctl, c->p.mac,
-                                                   c->p.theta);
+    cudaStreamWaitEvent(st, c->ev_perm, 0);
+    upsweep_kernel<<<full_node_grid, 128, 0, st>>>(na, pos_t, ctl, c->p.mac, c->p.theta);
     if (c->p.mac == HYB_MAC_ABS) {
-        bmax_kernel<<<(n + 255) / 256, 256, 0, st>>>(reinterpret_cast<const float4 *>(c->pos), n, na.leaf_of, parent,
-                                                     level, na.C64, bmax2);
+        bmax_kernel<<<(n + 255) / 256, 256, 0, st>>>(pos_t, n, na.leaf_of, parent, level, na.C64, bmax2);
         ropen_abs_kernel<<<(int)((L.node_cap + 255) / 256), 256, 0, st>>>(ctl, bmax2, na.B2, c->p.a_err, rec);
     }
-    unsigned char *gflag = wsptr<unsigned char>(c, L.gflag);
-    gmark_kernel<<<(int)((L.node_cap + 255) / 256), 256, 0, st>>>(ctl, first, count, child, parent, c->p.group_max,
-                                                                  gflag);
-    u32 *gfirst = wsptr<u32>(c, L.gfirst);
-    gscan_kernel<<<sc_grid, SC_THREADS, 0, st>>>(gflag, n, ctl, sc_status + L.sc_tiles, gfirst);
-    ginfo_kernel<<<(int)imin64((c->n + 255) / 256, (int64_t)c->num_sms * 8), 256, 0, st>>>(
-        ctl, n, reinterpret_cast<const float4 *>(c->pos), gfirst, wsptr<u32>(c, L.gcount), wsptr<float4>(c, L.glo),
-        wsptr<float4>(c, L.ghi));
+    cudaStreamWaitEvent(st, c->ev_groups, 0);       // join: groups, and (earlier on aux) the store copied back
     return cudaGetLastError();
 }
 

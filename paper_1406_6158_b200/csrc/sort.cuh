@@ -8,6 +8,7 @@
 
 namespace hyb {
 
+constexpr int LB_WIN = 16;        // look-back window (status words requested together)
 constexpr u32 RS_FLAG_AGG = 1u << 30, RS_FLAG_PREFIX = 2u << 30, RS_VALUE_MASK = (1u << 30) - 1;
 
 struct RadixSmem {
@@ -56,17 +57,31 @@ __global__ void __launch_bounds__(RS_THREADS) radix_pass_kernel(
             key[k] = ok ? kin[idx] : (KeyT)0;
             val[k] = ok ? (vin ? vin[idx] : idx) : 0xFFFFFFFFu;
         }
-        // stable rank of every key among the keys of this warp with the same digit
+        // stable rank of every key among the keys of this warp with the same digit.  The peer masks come
+        // from eight ballots per key (one per digit bit; match.any is far slower when the 32 digits of a
+        // warp are mostly distinct, as they are in the low passes) and are independent across the keys;
+        // only the counter update below is a serial chain.
+        u32 peers[RS_KPT];
 #pragma unroll
         for (int k = 0; k < RS_KPT; k++) {
-            u32 idx = base + k * 32 + lane;
-            bool ok = idx < n;
-            u32 d = ok ? (u32)((key[k] >> shift) & 0xFF) : 256u;
-            u32 peers = __match_any_sync(0xFFFFFFFFu, d);
-            u32 c = ok ? sm.warp_cnt[warp][d] : 0u;
+            const bool ok = base + k * 32 + lane < n;
+            const u32 d = (u32)((key[k] >> shift) & 0xFF);
+            u32 m = __ballot_sync(0xFFFFFFFFu, ok);
+#pragma unroll
+            for (int b = 0; b < 8; b++) {
+                const u32 bal = __ballot_sync(0xFFFFFFFFu, (d >> b) & 1u);
+                m &= ((d >> b) & 1u) ? bal : ~bal;
+            }
+            peers[k] = ok ? m : 0u;
+        }
+#pragma unroll
+        for (int k = 0; k < RS_KPT; k++) {
+            const bool ok = peers[k] != 0u;
+            const u32 d = (u32)((key[k] >> shift) & 0xFF);
+            const u32 c = ok ? sm.warp_cnt[warp][d] : 0u;
             __syncwarp();
-            rank[k] = c + __popc(peers & lt_mask);
-            if (ok && (peers & lt_mask) == 0) sm.warp_cnt[warp][d] = c + __popc(peers);
+            rank[k] = c + __popc(peers[k] & lt_mask);
+            if (ok && (peers[k] & lt_mask) == 0) sm.warp_cnt[warp][d] = c + __popc(peers[k]);
             __syncwarp();
         }
         __syncthreads();
@@ -78,7 +93,9 @@ __global__ void __launch_bounds__(RS_THREADS) radix_pass_kernel(
             sm.warp_cnt[w][tid] = total;
             total += t;
         }
-        // publish + look back (thread d for digit d)
+        // publish + look back (thread d for digit d).  All tiles of a pass are usually resident at once
+        // and publish at about the same time, so a tile may have to walk far back: LB_WIN predecessors
+        // are requested together and consumed in order, which divides the number of round trips.
         u32 excl = 0;
         {
             volatile u32 *st = status;
@@ -86,12 +103,24 @@ __global__ void __launch_bounds__(RS_THREADS) radix_pass_kernel(
             if (tile == 0) st[me] = RS_FLAG_PREFIX | total;
             else {
                 st[me] = RS_FLAG_AGG | total;
-                for (long long t = (long long)tile - 1; t >= 0; --t) {
-                    u32 s; int spins = 0;
-                    do { s = st[(size_t)t * 256 + tid]; } while ((s >> 30) == 0 && ++spins < LB_SPIN_LIMIT);
-                    if ((s >> 30) == 0) { atomicOr(dev_status, ST_WAIT_EXPIRED); break; }
-                    excl += s & RS_VALUE_MASK;
-                    if ((s >> 30) == 2) break;
+                long long t = (long long)tile - 1;
+                int spins = 0;
+                bool done = false;
+                while (!done) {
+                    u32 s[LB_WIN];
+#pragma unroll
+                    for (int i = 0; i < LB_WIN; i++)
+                        s[i] = (t - i >= 0) ? st[(size_t)(t - i) * 256 + tid] : (2u << 30);
+#pragma unroll
+                    for (int i = 0; i < LB_WIN; i++) {
+                        if (done) break;
+                        const u32 f = s[i] >> 30;
+                        if (f == 0) break;                       // not published yet: poll again from here
+                        excl += s[i] & RS_VALUE_MASK;
+                        t--;
+                        if (f == 2) done = true;
+                    }
+                    if (!done && ++spins >= LB_SPIN_LIMIT) { atomicOr(dev_status, ST_WAIT_EXPIRED); break; }
                 }
                 st[me] = RS_FLAG_PREFIX | (excl + total);
             }
