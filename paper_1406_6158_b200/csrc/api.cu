@@ -45,6 +45,7 @@ Layout plan_workspace(int64_t n)
     L.leaf_of = take(4 * N);
     L.gfirst = take(4 * GC); L.gcount = take(4 * GC); L.glo = take(16 * GC); L.ghi = take(16 * GC);
     L.ncell = take(4 * GC); L.npart = take(4 * GC); L.nhard = take(4 * GC);
+    L.splitq = take(4 * 4 * GC);
     L.total = off;
     return L;
 }
@@ -169,6 +170,7 @@ int hyb_init(hyb_ctx **out, const hyb_params *params, int64_t n, hyb_float4 *d_p
     }
     c->timing = true;
     e = cudaMemsetAsync(c->ctl, 0, sizeof(DevCtl), c->stream);
+    if (e == cudaSuccess) e = cudaMemsetAsync(c->ws + L.nhard, 0, 4 * (size_t)L.group_cap, c->stream);
     if (e != cudaSuccess) { delete c; return cuda_fail(nullptr, e, "cudaMemsetAsync"); }
     *out = reinterpret_cast<hyb_ctx *>(c);
     return HYB_OK;

@@ -60,7 +60,8 @@ struct DevCtl {
     u32 digit_base[RS_PASSES * 256];
     u32 node_base[256];
     // ---- walk ----
-    u32 group_counter;
+    u32 group_counter;          // ---- walk work distribution: reset before every launch (2 words)
+    u32 nheavy;                 // sink ranges of split groups (hard walk)
     u64 inter_soft, inter_hard;
 };
 
@@ -88,6 +89,7 @@ struct Layout {   // byte offsets into the workspace; computed by plan_workspace
     size_t MS64, C64, B2, bmax2;               // double[4nc] (M, Sx, Sy, Sz), [3nc], [nc], u64[nc]
     size_t leaf_of;             // u32[n]
     size_t gfirst, gcount, glo, ghi, ncell, npart, nhard;   // [group_cap]
+    size_t splitq;              // u32[4 group_cap]: sink ranges of split groups, processed first (walk.cu)
     size_t total;
     int64_t n, node_cap, group_cap;
     int64_t rs_tiles, node_tiles, sc_tiles, po_tiles;

@@ -29,6 +29,8 @@ struct WalkArgs {
     const u32 *gfirst, *gcount;
     const float4 *glo, *ghi;
     u32 *ncell, *npart, *nhard;
+    const u32 *heavy;             // hard walk: sink ranges of split groups (see split_kernel)
+    const unsigned char *is_split; // hard walk: group is handled as ranges
     float4 *a_soft, *a_hard;
     DevCtl *ctl;
     float G, eps2, rout, kc0, kc1;   // Y = sat(kc0 + kc1 r)
@@ -38,6 +40,8 @@ struct WalkArgs {
 constexpr int WK_SMAX = 4;          // most sinks per lane
 constexpr int WK_PAD_SLACK = 64;    // spare buffer entries for padding to a multiple of P U (<= 16 * 4)
 constexpr u32 FULL = 0xFFFFFFFFu;
+// hard walk: estimated pair count (members x hard-list length) above which a group is cut in 2 / 4 ranges
+constexpr unsigned long long WK_SPLIT2 = 24576ull, WK_SPLIT4 = 65536ull;
 constexpr u32 DESC_MASK = 0x1FFFFFFFu;      // node index bits of a stack descriptor
 
 template <int MODE>
@@ -372,15 +376,36 @@ __global__ void __launch_bounds__(WK_WARPS * 32, SmemLayout<MODE>::ctas_per_sm) 
     const float eps2 = a.eps2, kc0 = a.kc0, kc1 = a.kc1;
     unsigned long long isoft = 0, ihard = 0;
 
-    u32 g = 0;
-    if (lane == 0) g = atomicAdd(&a.ctl->group_counter, 1u);
-    g = __shfl_sync(FULL, g, 0);
+    // Work items come from one atomic counter.  In the hard walk the heaviest sink groups (by the
+    // estimate of split_kernel) have been cut into 2 or 4 sink ranges that are handed out first, so
+    // that the longest items start early and run side by side; then the other groups in Morton order.
+    // Every range walks with the box of the WHOLE group, so its lists are the group's lists (T12-T13);
+    // only the sinks differ.
+    constexpr bool SPLIT = MODE == WALK_HARD;
+    const u32 nheavy = SPLIT ? a.ctl->nheavy : 0u;
+    const u32 nitems = ng + nheavy;
+    u32 item = 0;
+    if (lane == 0) item = atomicAdd(&a.ctl->group_counter, 1u);
+    item = __shfl_sync(FULL, item, 0);
 
-    while (g < ng) {
-        u32 g_next = 0;
-        if (lane == 0) g_next = atomicAdd(&a.ctl->group_counter, 1u);      // consumed at the end of this group
-        const u32 gf = a.gfirst[g];
-        const int n = (int)a.gcount[g];
+    while (item < nitems) {
+        u32 item_next = 0;
+        if (lane == 0) item_next = atomicAdd(&a.ctl->group_counter, 1u);      // consumed at the end of this item
+        u32 g, rsub = 0, nsub = 1;
+        if (SPLIT && item < nheavy) {
+            const u32 it = __ldg(a.heavy + item);
+            g = it & 0x0FFFFFFFu; rsub = (it >> 28) & 3u; nsub = (it >> 30) + 1u;
+        } else {
+            g = item - nheavy;
+            if (SPLIT && a.is_split[g]) {                      // handled as ranges
+                item = __shfl_sync(FULL, item_next, 0);
+                continue;
+            }
+        }
+        const u32 n_all = a.gcount[g];
+        const u32 n_rng = (n_all + nsub - 1u) / nsub;                  // sinks per range
+        const u32 gf = a.gfirst[g] + rsub * n_rng;
+        const int n = (int)(min(n_all, (rsub + 1u) * n_rng) - rsub * n_rng);
         const float4 glo = a.glo[g], ghi = a.ghi[g];
         // sinks per lane: maximise n P / (32 S) over S in {2,3,4}; ties go to the larger S
         int S = 2, A = (n + 1) >> 1, P = 32 / A;
@@ -643,15 +668,38 @@ __global__ void __launch_bounds__(WK_WARPS * 32, SmemLayout<MODE>::ctas_per_sm) 
             }
         }
         if (lane == 0) {
-            a.ncell[g] = ncell; a.npart[g] = npart; a.nhard[g] = nhard;
+            if (rsub == 0) { a.ncell[g] = ncell; a.npart[g] = npart; a.nhard[g] = nhard; }
             if (MODE != WALK_HARD) isoft += (unsigned long long)n * (unsigned long long)(ncell + npart);
             if (MODE != WALK_NORMAL) ihard += (unsigned long long)n * (unsigned long long)nhard;
         }
-        g = __shfl_sync(FULL, g_next, 0);
+        item = __shfl_sync(FULL, item_next, 0);
     }
     if (lane == 0) {
         if (isoft) atomicAdd(&a.ctl->inter_soft, isoft);
         if (ihard) atomicAdd(&a.ctl->inter_hard, ihard);
+    }
+}
+
+// Hard walk scheduling: a group whose hard list was long at the previous walk (n x nhard of the group
+// with the same index -- an estimate that only steers the order of work, never the result) is cut
+// into 2 or 4 sink ranges, which are queued in front of everything else; the walk skips it
+// in the ordinary sequence.
+__global__ void __launch_bounds__(256) split_kernel(DevCtl *ctl, const u32 *__restrict__ gcount,
+                                                    const u32 *__restrict__ nhard, u32 *__restrict__ heavy,
+                                                    unsigned char *__restrict__ is_split, unsigned long long t2, unsigned long long t4)
+{
+    const u32 ng = ctl->ng;
+    for (u32 g = blockIdx.x * blockDim.x + threadIdx.x; g < ng; g += gridDim.x * blockDim.x) {
+        const u32 n = gcount[g], h = nhard[g];
+        const unsigned long long est = (unsigned long long)n * (unsigned long long)h;
+        u32 nsub = 1;
+        if (est >= t4 && n >= 32u) nsub = 4;
+        else if (est >= t2 && n >= 16u) nsub = 2;
+        if (nsub > 1) {
+            const u32 at = atomicAdd(&ctl->nheavy, nsub);
+            for (u32 i = 0; i < nsub; i++) heavy[at + i] = g | (i << 28) | ((nsub - 1u) << 30);
+        }
+        is_split[g] = nsub > 1;
     }
 }
 
@@ -698,7 +746,13 @@ cudaError_t launch_walk(Ctx *c, int mode)
     const float w = c->p.r_out - c->p.r_in;
     a.kc0 = c->p.r_out / w; a.kc1 = -1.0f / w;
     a.zero64 = 0ull;
-    cudaMemsetAsync(&c->ctl->group_counter, 0, sizeof(u32), c->stream);
+    a.heavy = wsptr<u32>(c, L.splitq);
+    a.is_split = wsptr<unsigned char>(c, L.gflag);      // the build's flag array is free between builds
+    cudaMemsetAsync(&c->ctl->group_counter, 0, 2 * sizeof(u32), c->stream);      // counter, nheavy
+    if (mode == WALK_HARD)
+        split_kernel<<<(int)imin64((c->n + 255) / 256, (int64_t)c->num_sms * 4), 256, 0, c->stream>>>(
+            c->ctl, a.gcount, a.nhard, wsptr<u32>(c, L.splitq), wsptr<unsigned char>(c, L.gflag),
+            WK_SPLIT2, WK_SPLIT4);
     if (mode == WALK_HYBRID) return launch_walk_mode<WALK_HYBRID>(c, a);
     if (mode == WALK_HARD) return launch_walk_mode<WALK_HARD>(c, a);
     return launch_walk_mode<WALK_NORMAL>(c, a);
