@@ -145,7 +145,8 @@ def main():
     torch.cuda.set_device(local_rank)
     if world > 1:
         dist.init_process_group("nccl")
-    pos, vel = make_ic(cfg.kind, cfg.n, cfg.seed + rank)       # independent replica per rank
+    from paper_1406_6158_b200.replicas import replica_seed
+    pos, vel = make_ic(cfg.kind, cfg.n, replica_seed(cfg.seed, rank))      # independent replica per rank
     P = HybParams.from_config(cfg)
     dpos = torch.from_numpy(pos).cuda(); dvel = torch.from_numpy(vel).cuda()
     h = Hyb(P, dpos, dvel)
@@ -179,13 +180,8 @@ def main():
     inter = h.export("interactions").astype(np.float64)
     stage = h.export("timings").astype(np.float64)
     launches = int(h.export("counts")[6]) - launches0
-    t = torch.tensor([total_ms], dtype=torch.float64, device="cuda")
-    tot_inter = torch.tensor([inter.sum()], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        dist.all_reduce(tot_inter, op=dist.ReduceOp.SUM)
-    total_ms = float(t.item())
-    value = float(tot_inter.item()) / (total_ms * 1e-3)
+    from paper_1406_6158_b200.replicas import aggregate
+    total_ms, _, value = aggregate(total_ms, float(inter.sum()), device="cuda")     # max over ranks, sum of work
 
     # ---- roofline of the dominant kernel (the fused soft+hard group walk), rank 0's numbers
     K = args.steps
@@ -198,9 +194,12 @@ def main():
     sm_max = clk.get("sm_max_mhz", 1965)
     peak = N_SM * FP32_LANES * 2 * sm_max * 1e6 / 1e12
     traffic = None
-    tpath = os.path.join(ROOT, "profiles", "traffic.json")
+    tpath = os.path.join(ROOT, "profiles", "traffic.csv")      # "kernel,dram_bytes_per_launch" from the ncu --set full capture
     if os.path.exists(tpath):
-        traffic = json.load(open(tpath)).get("walk_hybrid_dram_bytes_per_launch")
+        for line in open(tpath):
+            k, _, v = line.strip().partition(",")
+            if k == "walk_kernel<HYBRID>":
+                traffic = float(v)
     achieved = flops / (soft_ms * 1e-3) / 1e12
     roofline = {"bound": "alu", "kernel": "walk_kernel<HYBRID> (fused soft+hard group walk)", "achieved": achieved,
                 "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak, "traffic": traffic,

@@ -115,7 +115,7 @@ static int do_hard(Ctx *c)
 {
     cudaError_t e = c->p.split ? launch_walk(c, WALK_HARD) : launch_zero_acc(c, c->a_hard);
     if (e != cudaSuccess) return cuda_fail(c, e, "hard walk");
-    c->launches += 1;
+    c->launches += c->p.split ? 2 : 1;          // split_kernel + walk, or the zero fill
     return HYB_OK;
 }
 
