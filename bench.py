@@ -97,6 +97,7 @@ def main():
     ap.add_argument("--cpu-seconds", type=float, default=12.0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer leg (profiling runs)")
+    ap.add_argument("--no-normal", action="store_true", help="skip the normal-tree comparison leg")
     args = ap.parse_args()
 
     rank = int(os.environ.get("RANK", "0"))
@@ -232,6 +233,37 @@ def main():
                "what": "hyb_run_host: upload pos/vel/id, initial tree+forces, one soft cycle, download "
                        "pos/vel/id/a_soft/a_hard; device alloc/free inside"}
 
+    # ---- the same cycle with a plain (unsplit, theta-only) tree at dt_h: n_sub
+    #      builds + n_sub full walks per cycle; reported beside the hybrid to show its compute ratio
+    #      (the paper's R_hybrid of about 0.8 is a multi-process wall-clock ratio on other hardware)
+    normal = None
+    if rank == 0 and not args.no_normal:
+        hn = Hyb(HybParams.from_config(cfg, split=0), torch.from_numpy(pos).cuda(), torch.from_numpy(vel).cuda())
+        hn.step(0)
+        for _ in range(2):
+            hn.step(1)
+        hn.export("interactions"); hn.export("timings")
+        kn = max(2, min(K, 4))
+        evn = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(kn)]
+        for a, b in evn:
+            flush.zero_()
+            a.record(); hn.step(1); b.record()
+        torch.cuda.synchronize()
+        n_ms = sum(a.elapsed_time(b) for a, b in evn) / kn
+        n_inter = hn.export("interactions").astype(np.float64)
+        n_stage = hn.export("timings").astype(np.float64)
+        walk_ms = n_stage[1] / kn / cfg.n_sub                    # one unsplit walk
+        normal = {"ms_per_step": n_ms, "interactions_per_s": float(n_inter.sum()) / kn / (n_ms * 1e-3),
+                  "stages": {"build_ms": n_stage[0] / kn, "walk_ms": n_stage[1] / kn, "integrate_ms": n_stage[3] / kn},
+                  "walk_kernel": {"ms": walk_ms, "interactions_per_s": n_inter[0] / kn / cfg.n_sub / (walk_ms * 1e-3),
+                                  "tflops": FLOP_MONO * n_inter[0] / kn / cfg.n_sub / (walk_ms * 1e-3) / 1e12,
+                                  "frac_of_fp32_peak": FLOP_MONO * n_inter[0] / kn / cfg.n_sub / (walk_ms * 1e-3) / 1e12 / peak},
+                  "t_hybrid_over_t_normal": (total_ms / K) / n_ms,
+                  "hard_walk_over_normal_walk": (stage[2] / K / max(cfg.n_sub - 1, 1)) / walk_ms,
+                  "paper_context": "PAPER.md:182 hard kernel ~40 % of a normal-tree force kernel; PAPER.md:216 total time "
+                                   "80-90 % of a normal tree (HA-PACS: Tesla M2090 + E5-2670, multi-process)"}
+        hn.close()
+
     cpu_baseline = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         cpu_baseline, _ = oracle_sample(cfg, pos, args.cpu_seconds)
@@ -242,7 +274,8 @@ def main():
             "warmup": args.warmup, "ms_per_step": total_ms / K, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f32", "data": "synthetic", "config": config, "stages": stages,
             "interactions_per_step": {"soft": inter[0] / K, "hard": inter[1] / K},
-            "roofline": roofline, "cpu_baseline": cpu_baseline, "e2e": e2e, "gpu_launches": launches,
+            "roofline": roofline, "normal_tree": normal, "cpu_baseline": cpu_baseline, "e2e": e2e,
+            "gpu_launches": launches,
             "clocks": {"sm_mhz": sm_mhz, "sm_max_mhz": sm_max, "reasons": sorted(clk["reasons"]),
                        "samples": len(sm), **({"error": clk["error"]} if "error" in clk else {})}}))
     h.close()

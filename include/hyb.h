@@ -46,7 +46,7 @@ typedef struct hyb_params {
     int32_t leaf_max;  /* n_crit: a cell with more particles is split; 1..64     */
     int32_t group_max; /* sinks that share one traversal (n_vec); leaf_max..64   */
     int32_t mac;       /* HYB_MAC_THETA or HYB_MAC_ABS (Eq. 5-6)                               */
-    int32_t kfunc;     /* HYB_K_PAPER (Eq. 10).  HYB_K_POLY7 is rejected (not built yet)       */
+    int32_t kfunc;     /* HYB_K_PAPER (Eq. 10, the default) or HYB_K_POLY7 (north_star's alternative) */
     int32_t split;     /* 1 = hybrid (Eq. 7-9); 0 = normal tree (K == 0)     */
 } hyb_params;
 

@@ -63,7 +63,7 @@ static bool params_ok(const hyb_params *p, int64_t n, char *msg)
     if (p->mac != HYB_MAC_THETA && p->mac != HYB_MAC_ABS) return bad("unknown mac");
     if (p->mac == HYB_MAC_THETA && !(p->theta >= 0.0f && isfinite(p->theta))) return bad("theta must be finite and >= 0");
     if (p->mac == HYB_MAC_ABS && !(p->a_err > 0.0f && isfinite(p->a_err))) return bad("a_err must be finite and > 0");
-    if (p->kfunc != HYB_K_PAPER) return bad("only HYB_K_PAPER (Eq. 10) is built");
+    if (p->kfunc != HYB_K_PAPER && p->kfunc != HYB_K_POLY7) return bad("unknown kfunc");
     if (p->split != 0 && p->split != 1) return bad("split must be 0 or 1");
     if (p->split == 1 && !(p->r_in >= 0.0f && p->r_out > p->r_in && isfinite(p->r_out))) return bad("need 0 <= r_in < r_out");
     return true;

@@ -151,18 +151,26 @@ __device__ __forceinline__ void mono1(const float4 s, f2 nx, f2 ny, f2 nz, float
     ax = pk(a0, hx); ay = pk(a1, hy); az = pk(a2, hz);
 }
 
-// Eq. 10 with Y clamped to [0,1]: K = t^3 (10 - 15 t + 6 t^2), t = Y^2 (T15)
+// KF = HYB_K_PAPER: Eq. 10 with Y clamped to [0,1]: K = t^3 (10 - 15 t + 6 t^2), t = Y^2 (T15).
+// KF = HYB_K_POLY7 (north_star's alternative, R6): K = 1 - x^4 (35 - 84 x + 70 x^2 - 20 x^3),
+// x = (r - r_in)/(r_out - r_in) = 1 - Y on the clamped range.
+template <int KF>
 __device__ __forceinline__ float kfun(float r, float kc0, float kc1)
 {
-    float Y = __saturatef(fmaf(r, kc1, kc0));
-    float t = Y * Y;
-    float poly = fmaf(fmaf(6.0f, t, -15.0f), t, 10.0f);
+    const float Y = __saturatef(fmaf(r, kc1, kc0));
+    if (KF == HYB_K_POLY7) {
+        const float x = 1.0f - Y, x2 = x * x;
+        const float poly = fmaf(fmaf(fmaf(-20.0f, x, 70.0f), x, -84.0f), x, 35.0f);
+        return fmaf(-(x2 * x2), poly, 1.0f);
+    }
+    const float t = Y * Y;
+    const float poly = fmaf(fmaf(6.0f, t, -15.0f), t, 10.0f);
     return (t * t) * (t * poly);
 }
 
 // K-weighted pair (Eq. 8, 9) for two sinks: hard part K F, and (SOFT) the soft part (1 - K) F.
 // fused: 25 FP32-pipe instruction equivalents + 4 MUFU per pair of interactions; hard only: 21 + 4.
-template <bool SOFT>
+template <bool SOFT, int KF>
 __device__ __forceinline__ void kpair2(const float4 s, f2 nx, f2 ny, f2 nz, float eps2, float kc0, float kc1, f2 &sx,
                                        f2 &sy, f2 &sz, f2 &hx, f2 &hy, f2 &hz)
 {
@@ -176,9 +184,16 @@ __device__ __forceinline__ void kpair2(const float4 s, f2 nx, f2 ny, f2 nz, floa
     const f2 ri = pk(rsqrt_approx(ea), rsqrt_approx(eb));
     const float Ya = __saturatef(fmaf(sqrt_approx(ua), kc1, kc0)), Yb = __saturatef(fmaf(sqrt_approx(ub), kc1, kc0));
     const f2 Y = pk(Ya, Yb);
-    const f2 t = mul2(Y, Y);
-    const f2 poly = fma2(fma2(pk(6.0f, 6.0f), t, pk(-15.0f, -15.0f)), t, pk(10.0f, 10.0f));
-    const f2 K = mul2(mul2(t, t), mul2(t, poly));
+    f2 K;
+    if (KF == HYB_K_POLY7) {
+        const f2 x = fma2(Y, pk(-1.0f, -1.0f), pk(1.0f, 1.0f)), x2 = mul2(x, x);
+        const f2 poly = fma2(fma2(fma2(pk(-20.0f, -20.0f), x, pk(70.0f, 70.0f)), x, pk(-84.0f, -84.0f)), x, pk(35.0f, 35.0f));
+        K = fma2(mul2(mul2(x2, x2), pk(-1.0f, -1.0f)), poly, pk(1.0f, 1.0f));
+    } else {
+        const f2 t = mul2(Y, Y);
+        const f2 poly = fma2(fma2(pk(6.0f, 6.0f), t, pk(-15.0f, -15.0f)), t, pk(10.0f, 10.0f));
+        K = mul2(mul2(t, t), mul2(t, poly));
+    }
     const f2 ri2 = mul2(ri, ri);
     const f2 mr = mul2(pk(s.w, s.w), ri);
     const f2 mr3 = mul2(mr, ri2);
@@ -194,7 +209,7 @@ __device__ __forceinline__ void kpair2(const float4 s, f2 nx, f2 ny, f2 nz, floa
     }
 }
 
-template <bool SOFT>
+template <bool SOFT, int KF>
 __device__ __forceinline__ void kpair1(const float4 s, f2 nx, f2 ny, f2 nz, float eps2, float kc0, float kc1, f2 &sx,
                                        f2 &sy, f2 &sz, f2 &hx, f2 &hy, f2 &hz)
 {
@@ -209,7 +224,7 @@ __device__ __forceinline__ void kpair1(const float4 s, f2 nx, f2 ny, f2 nz, floa
     const float ri2 = ri * ri;
     const float mr = s.w * ri;
     const float mr3 = mr * ri2;
-    const float wh = kfun(r, kc0, kc1) * mr3;
+    const float wh = kfun<KF>(r, kc0, kc1) * mr3;
     float a0, a1, a2, b0, b1, b2;
     upk(hx, a0, b0); upk(hy, a1, b1); upk(hz, a2, b2);
     hx = pk(fmaf(wh, dx, a0), b0); hy = pk(fmaf(wh, dy, a1), b1); hz = pk(fmaf(wh, dz, a2), b2);
@@ -308,7 +323,7 @@ __device__ __forceinline__ void eval_mono(const float4 *buf, int cnt, int part, 
     if (ODD) { k.sx[NP] = pk(oax, keepx); k.sy[NP] = pk(oay, keepy); k.sz[NP] = pk(oaz, keepz); }
 }
 
-template <int S, int U, bool SOFT>
+template <int S, int U, bool SOFT, int KF>
 __device__ __forceinline__ void eval_near(const float4 *buf, int cnt, int part, int P, Sinks &k, float eps2, float kc0,
                                           float kc1)
 {
@@ -323,10 +338,10 @@ __device__ __forceinline__ void eval_near(const float4 *buf, int cnt, int part, 
         for (int u = 0; u < U; u++) {
 #pragma unroll
             for (int q = 0; q < S / 2; q++)
-                kpair2<SOFT>(s[u], k.nx[q], k.ny[q], k.nz[q], eps2, kc0, kc1, k.sx[q], k.sy[q], k.sz[q], k.hx[q], k.hy[q],
+                kpair2<SOFT, KF>(s[u], k.nx[q], k.ny[q], k.nz[q], eps2, kc0, kc1, k.sx[q], k.sy[q], k.sz[q], k.hx[q], k.hy[q],
                              k.hz[q]);
             if (S & 1)
-                kpair1<SOFT>(s[u], k.nx[S / 2], k.ny[S / 2], k.nz[S / 2], eps2, kc0, kc1, k.sx[S / 2], k.sy[S / 2],
+                kpair1<SOFT, KF>(s[u], k.nx[S / 2], k.ny[S / 2], k.nz[S / 2], eps2, kc0, kc1, k.sx[S / 2], k.sy[S / 2],
                              k.sz[S / 2], k.hx[S / 2], k.hy[S / 2], k.hz[S / 2]);
         }
     }
@@ -352,7 +367,7 @@ __device__ __forceinline__ u32 warp_excl_scan(u32 v, int lane, u32 &total)
     return incl - v;
 }
 
-template <int MODE>
+template <int MODE, int KF>
 __global__ void __launch_bounds__(WK_WARPS * 32, SmemLayout<MODE>::ctas_per_sm) walk_kernel(const WalkArgs a)
 {
     using SL = SmemLayout<MODE>;
@@ -460,9 +475,9 @@ __global__ void __launch_bounds__(WK_WARPS * 32, SmemLayout<MODE>::ctas_per_sm) 
                 if (HAS_NEAR && flush_near) {
                     const int cnt = pad_buffer(partbuf, npb, P * 2, dummy, lane);
                     __syncwarp();
-                    if (S == 2) eval_near<2, 2, MODE == WALK_HYBRID>(partbuf, cnt, part, P, sk, eps2, kc0, kc1);
-                    else if (S == 3) eval_near<3, 2, MODE == WALK_HYBRID>(partbuf, cnt, part, P, sk, eps2, kc0, kc1);
-                    else eval_near<4, 2, MODE == WALK_HYBRID>(partbuf, cnt, part, P, sk, eps2, kc0, kc1);
+                    if (S == 2) eval_near<2, 2, MODE == WALK_HYBRID, KF>(partbuf, cnt, part, P, sk, eps2, kc0, kc1);
+                    else if (S == 3) eval_near<3, 2, MODE == WALK_HYBRID, KF>(partbuf, cnt, part, P, sk, eps2, kc0, kc1);
+                    else eval_near<4, 2, MODE == WALK_HYBRID, KF>(partbuf, cnt, part, P, sk, eps2, kc0, kc1);
                     npb = 0; flush_near = false;
                     __syncwarp();
                 }
@@ -716,18 +731,18 @@ cudaError_t launch_zero_acc(Ctx *c, hyb_float4 *a)
     return cudaGetLastError();
 }
 
-template <int MODE>
+template <int MODE, int KF>
 static cudaError_t launch_walk_mode(Ctx *c, const WalkArgs &a)
 {
     using SL = SmemLayout<MODE>;
     const size_t smem = SL::bytes * WK_WARPS;
     static bool attr_set = false;
     if (!attr_set) {
-        cudaError_t e = cudaFuncSetAttribute(walk_kernel<MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        cudaError_t e = cudaFuncSetAttribute(walk_kernel<MODE, KF>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
         attr_set = true;
     }
-    walk_kernel<MODE><<<c->num_sms * SL::ctas_per_sm, WK_WARPS * 32, smem, c->stream>>>(a);
+    walk_kernel<MODE, KF><<<c->num_sms * SL::ctas_per_sm, WK_WARPS * 32, smem, c->stream>>>(a);
     return cudaGetLastError();
 }
 
@@ -753,9 +768,10 @@ cudaError_t launch_walk(Ctx *c, int mode)
         split_kernel<<<(int)imin64((c->n + 255) / 256, (int64_t)c->num_sms * 4), 256, 0, c->stream>>>(
             c->ctl, a.gcount, a.nhard, wsptr<u32>(c, L.splitq), wsptr<unsigned char>(c, L.gflag),
             WK_SPLIT2, WK_SPLIT4);
-    if (mode == WALK_HYBRID) return launch_walk_mode<WALK_HYBRID>(c, a);
-    if (mode == WALK_HARD) return launch_walk_mode<WALK_HARD>(c, a);
-    return launch_walk_mode<WALK_NORMAL>(c, a);
+    const bool poly7 = c->p.kfunc == HYB_K_POLY7;
+    if (mode == WALK_HYBRID) return poly7 ? launch_walk_mode<WALK_HYBRID, HYB_K_POLY7>(c, a) : launch_walk_mode<WALK_HYBRID, HYB_K_PAPER>(c, a);
+    if (mode == WALK_HARD) return poly7 ? launch_walk_mode<WALK_HARD, HYB_K_POLY7>(c, a) : launch_walk_mode<WALK_HARD, HYB_K_PAPER>(c, a);
+    return launch_walk_mode<WALK_NORMAL, HYB_K_PAPER>(c, a);
 }
 
 }  // namespace hyb

@@ -43,7 +43,7 @@ def test_workspace_bytes_and_validation(L):
     assert sizes[-1] < 16 * 2 ** 30                    # 2^24 particles fit comfortably in 180 GB
     good = HybParams.from_config(CONFIGS[0])
     bad = [dict(eps=0.0), dict(n_sub=0), dict(leaf_max=0), dict(group_max=4), dict(group_max=65), dict(mac=2),
-           dict(kfunc=1), dict(split=2), dict(r_in=0.2), dict(theta=-1.0), dict(mac=1, a_err=0.0)]
+           dict(kfunc=2), dict(split=2), dict(r_in=0.2), dict(theta=-1.0), dict(mac=1, a_err=0.0)]
     for kw in bad:
         assert hyb_workspace_bytes(4096, HybParams.from_config(CONFIGS[0], **kw)) == 0, kw
     assert hyb_workspace_bytes(0, good) == 0 and hyb_workspace_bytes(1 << 30, good) == 0

@@ -68,3 +68,26 @@ def test_theta_zero_opens_everything():
     err = np.linalg.norm(tot - at[perm], axis=1) / np.linalg.norm(at[perm], axis=1)
     assert err.max() < 1e-4 and np.sqrt(np.mean(err ** 2)) < 1e-5
     h.close()
+
+
+def test_poly7_changeover_function():
+    """north_star's alternative K (HYB_K_POLY7, R6): same lists, different split of the pair force."""
+    for cfg, seed in ((CONFIGS[0], 0), (CONFIGS[1].with_(n=30011), 9)):
+        pos, vel = make_ic(cfg.kind, cfg.n, seed)
+        res = _run_case(cfg, pos, vel, kfunc=1)
+        res0 = _run_case(cfg, pos, vel, kfunc=0)
+        print(res)
+        assert res["hard"] != res0["hard"]                 # the two changeover functions really differ
+
+
+def test_paper_parameter_recipe():
+    """the paper's own parameter choice: eps = 0.1 N^-0.26, R1 = 1.03 N^-1/3, R2 = 2 R1,
+    absolute MAC with a_err = 2^-8, n = 4."""
+    from workloads import paper_params
+    cfg = paper_params(1 << 16, seed=12)
+    pos, vel = make_ic(cfg.kind, cfg.n, cfg.seed)
+    print(_run_case(cfg, pos, vel))
+    h = make_hyb(cfg, pos, vel)
+    h.step(1); h.sync()
+    assert np.all(np.isfinite(h.pos_m.cpu().numpy()))
+    h.close()
