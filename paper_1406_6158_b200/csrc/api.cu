@@ -253,8 +253,11 @@ int hyb_step(hyb_ctx *ctx, int32_t n_soft_steps)
             cudaEvent_t e0 = c->timing ? ev() : nullptr;
             cudaError_t e;
             // opening kick(s) + drift.  split = 0: the whole force lives in a_soft and is kicked at dt_h.
-            if (split) e = launch_kick_drift(c, k == 0 ? 0.5f * dts : 0.0f, 0.5f * dth, dth);
-            else e = launch_kick_drift(c, 0.5f * dth, 0.0f, dth);
+            // Inside a cycle the closing half kick of one substep and the opening half kick of the next
+            // use the same acceleration, so they are one full kick fused with the drift (k > 0).
+            const float open_c = k == 0 ? 0.5f * dth : dth;
+            if (split) e = launch_kick_drift(c, k == 0 ? 0.5f * dts : 0.0f, open_c, dth);
+            else e = launch_kick_drift(c, open_c, 0.0f, dth);
             if (e != cudaSuccess) return cuda_fail(c, e, "kick_drift");
             cudaEvent_t e1 = c->timing ? ev() : nullptr;
             if ((rc = do_build(c)) != HYB_OK) return rc;
@@ -263,10 +266,13 @@ int hyb_step(hyb_ctx *ctx, int32_t n_soft_steps)
             if (soft_step) rc = do_soft(c); else rc = do_hard(c);
             if (rc != HYB_OK) return rc;
             cudaEvent_t e3 = c->timing ? ev() : nullptr;
-            if (split) e = launch_kick_drift(c, k == nsub - 1 ? 0.5f * dts : 0.0f, 0.5f * dth, 0.0f);
-            else e = launch_kick_drift(c, 0.5f * dth, 0.0f, 0.0f);
-            if (e != cudaSuccess) return cuda_fail(c, e, "kick");
-            c->launches += 2;
+            const bool last = k == nsub - 1;           // the closing half kick of the other substeps is fused above
+            if (last) {
+                if (split) e = launch_kick_drift(c, 0.5f * dts, 0.5f * dth, 0.0f);
+                else e = launch_kick_drift(c, 0.5f * dth, 0.0f, 0.0f);
+                if (e != cudaSuccess) return cuda_fail(c, e, "kick");
+            }
+            c->launches += last ? 2 : 1;
             if (c->timing) {
                 cudaEvent_t e4 = ev();
                 segs.push_back({3, e0, e1}); segs.push_back({0, e1, e2});
