@@ -182,12 +182,12 @@ def main():
     stage = h.export("timings").astype(np.float64)
     launches = int(h.export("counts")[6]) - launches0
     from paper_1406_6158_b200.replicas import aggregate
-    total_ms, _, value = aggregate(total_ms, float(inter.sum()), device="cuda")     # max over ranks, sum of work
+    total_ms, _, value = aggregate(total_ms, float(inter[0] + inter[1]), device="cuda")     # max over ranks, sum of work
 
     # ---- roofline of the dominant kernel (the fused soft+hard group walk), rank 0's numbers
     K = args.steps
     soft_ms = stage[1] / K                                       # one launch per step
-    fused_hard = inter[1] / cfg.n_sub                           # hard pairs evaluated inside the soft-step walk
+    fused_hard = inter[2]                                       # hard pairs evaluated inside the soft-step walks
     mono = inter[0] - fused_hard                                # plain monopole pairs (cells + far particles)
     flops = (FLOP_MONO * mono + FLOP_KFUSED * fused_hard) / K
     sm = sorted(clk["samples"])
@@ -210,7 +210,8 @@ def main():
                 "interactions_per_s": (mono + fused_hard) / K / (soft_ms * 1e-3),
                 "flop_per_pair": {"monopole": FLOP_MONO, "k_fused": FLOP_KFUSED, "k_hard": FLOP_KHARD},
                 "hard_walk": {"interactions_per_s": (inter[1] - fused_hard) / max(stage[2] * 1e-3, 1e-12),
-                              "tflops": FLOP_KHARD * (inter[1] - fused_hard) / max(stage[2] * 1e-3, 1e-12) / 1e12}}
+                              "tflops": FLOP_KHARD * (inter[1] - fused_hard) / max(stage[2] * 1e-3, 1e-12) / 1e12,
+                              "frac": FLOP_KHARD * (inter[1] - fused_hard) / max(stage[2] * 1e-3, 1e-12) / 1e12 / peak}}
     stages = {"build_ms": stage[0] / K, "soft_ms": soft_ms, "hard_ms": stage[2] / K, "integrate_ms": stage[3] / K}
 
     # ---- end to end through the C-ABI with HOST buffers (pinned), copies inside the timed region
@@ -253,7 +254,7 @@ def main():
         n_inter = hn.export("interactions").astype(np.float64)
         n_stage = hn.export("timings").astype(np.float64)
         walk_ms = n_stage[1] / kn / cfg.n_sub                    # one unsplit walk
-        normal = {"ms_per_step": n_ms, "interactions_per_s": float(n_inter.sum()) / kn / (n_ms * 1e-3),
+        normal = {"ms_per_step": n_ms, "interactions_per_s": float(n_inter[0] + n_inter[1]) / kn / (n_ms * 1e-3),
                   "stages": {"build_ms": n_stage[0] / kn, "walk_ms": n_stage[1] / kn, "integrate_ms": n_stage[3] / kn},
                   "walk_kernel": {"ms": walk_ms, "interactions_per_s": n_inter[0] / kn / cfg.n_sub / (walk_ms * 1e-3),
                                   "tflops": FLOP_MONO * n_inter[0] / kn / cfg.n_sub / (walk_ms * 1e-3) / 1e12,

@@ -32,6 +32,7 @@ typedef struct hyb_ctx hyb_ctx; /* opaque; created by hyb_init, destroyed by hyb
 
 enum { HYB_MAC_THETA = 0, HYB_MAC_ABS = 1 };
 enum { HYB_K_PAPER = 0, HYB_K_POLY7 = 1 };
+enum { HYB_GROUP_NODE = 0, HYB_GROUP_SIBLINGS = 1, HYB_GROUP_AUTO = 2 };
 
 /* The paper's statement of the problem. */
 typedef struct hyb_params {
@@ -48,6 +49,12 @@ typedef struct hyb_params {
     int32_t mac;       /* HYB_MAC_THETA or HYB_MAC_ABS (Eq. 5-6)                               */
     int32_t kfunc;     /* HYB_K_PAPER (Eq. 10, the default) or HYB_K_POLY7 (north_star's alternative) */
     int32_t split;     /* 1 = hybrid (Eq. 7-9); 0 = normal tree (K == 0)     */
+    int32_t grouping;  /* sink groups (consecutive sorted sinks share a traversal):
+                          HYB_GROUP_SIBLINGS = runs of consecutive sibling cells of <= group_max particles
+                          in all, HYB_GROUP_NODE = one tree node per group (R17);
+                          HYB_GROUP_AUTO = SIBLINGS, except that hyb_step builds the trees that only a
+                          hard walk uses with NODE (the hard force is a direct sum whatever the groups
+                          are; small groups list fewer particles beyond r_out)                        */
 } hyb_params;
 
 enum {
@@ -88,8 +95,8 @@ enum {
     HYB_X_NCELL = 18,      /* uint32[ng] cell-list length of the last walk                      */
     HYB_X_NPART = 19,      /* uint32[ng] particle-list length of the last walk                  */
     HYB_X_NHARD = 20,      /* uint32[ng] hard-list length of the last walk                      */
-    HYB_X_INTERACTIONS = 21,/* uint64[2] sum over groups of members x (ncell+npart), members x
-                              nhard, accumulated since hyb_init or the last read of this item   */
+    HYB_X_INTERACTIONS = 21,/* uint64[3] since the last read: sum over groups of members x (ncell+npart),
+                              members x nhard (all walks), members x nhard of the fused soft+hard walks */
     HYB_X_TIMINGS = 22,    /* float[8] ms accumulated in hyb_step since the last read:
                               build, soft walk, hard walk, integrate, 0, 0, 0, cycles           */
     HYB_X_BBOX = 23,       /* float[6] lo xyz, hi xyz of the last build                         */

@@ -312,12 +312,32 @@ static void moments(orc_tree *t)
 }
 
 /* ------------------------------------------------------------------ T11 groups */
-/* several sinks share one traversal (n_vec); R17: a sink group is a maximal
- * tree node with count <= group_max; level-21 leaves larger than that are cut into chunks. */
+/* n_vec CONSECUTIVE sorted sinks share one traversal.  R17, two readings:
+ *   grouping 0: a sink group is a maximal tree node with count <= group_max;
+ *   grouping 1: the children of a cell with more than group_max particles are taken in order and
+ *               consecutive children with count <= group_max are packed greedily into runs whose
+ *               total stays <= group_max (a child with more than group_max particles closes the run
+ *               and is treated recursively); a group is such a run -- consecutive sorted sinks as in
+ *               the paper, fuller than single nodes, and still inside one cell.
+ * In both, level-21 leaves larger than group_max are cut into chunks of group_max. */
 static void groups(orc_tree *t)
 {
     int64_t gm = t->p.group_max, ng = 0;
     uint8_t *mark = (uint8_t *)calloc((size_t)t->n, 1);
+    if (t->p.grouping == 1) {             /* T11 (siblings): see the comment above */
+        for (int64_t k = 0; k < t->nn; k++) {
+            uint32_t c = t->count[k], f = t->first[k];
+            if ((int64_t)c <= gm) { if (k == 0) mark[f] = 1; continue; }
+            if (t->child[k] == NOCHILD) { for (uint32_t s = f; s < f + c; s += (uint32_t)gm) mark[s] = 1; continue; }
+            int64_t run = 0; int open = 0;
+            for (uint32_t q = t->child[k]; q < t->child[k] + t->nchild[k]; q++) {
+                int64_t cq = t->count[q];
+                if (cq > gm) { open = 0; run = 0; continue; }
+                if (!open || run + cq > gm) { mark[t->first[q]] = 1; run = 0; open = 1; }
+                run += cq;
+            }
+        }
+    } else
     for (int64_t k = 0; k < t->nn; k++) {
         uint32_t c = t->count[k], f = t->first[k];
         int is_group = (int64_t)c <= gm && (k == 0 || (int64_t)t->count[t->parent[k]] > gm);

@@ -41,6 +41,7 @@ typedef struct {
     int32_t mac;           /* 0 theta, 1 absolute */
     int32_t kfunc;         /* 0 Eq. 10, 1 north_star's 7th-degree polynomial */
     int32_t split;         /* 1 hybrid, 0 normal tree */
+    int32_t grouping;      /* T11: 0 sink group = one tree node, 1 = run of consecutive small siblings (R17) */
 } orc_params;
 
 enum { ORC_MODE_HYBRID = 0, ORC_MODE_HARD = 1, ORC_MODE_NORMAL = 2 };

@@ -18,13 +18,15 @@ class OrcParams(C.Structure):
     _fields_ = [("G", C.c_float), ("eps", C.c_float), ("theta", C.c_float), ("a_err", C.c_float),
                 ("r_in", C.c_float), ("r_out", C.c_float), ("dt_soft", C.c_float),
                 ("n_sub", C.c_int32), ("leaf_max", C.c_int32), ("group_max", C.c_int32),
-                ("mac", C.c_int32), ("kfunc", C.c_int32), ("split", C.c_int32)]
+                ("mac", C.c_int32), ("kfunc", C.c_int32), ("split", C.c_int32), ("grouping", C.c_int32)]
 
 
 def params_from(cfg, **over) -> OrcParams:
     """cfg: any object with the workloads.Config attribute names."""
     d = {f: getattr(cfg, f) for f, _ in OrcParams._fields_}
     d.update(over)
+    if d["grouping"] == 2:       # "auto" is a scheduling choice of hyb_step; a tree built on request uses reading 1
+        d["grouping"] = 1
     return OrcParams(**d)
 
 

@@ -22,7 +22,7 @@ EXPORTS = {
     "ropen2": (11, np.float32, 1, "nn"), "nlo": (12, np.float32, 4, "nn"), "nhi": (13, np.float32, 4, "nn"),
     "gfirst": (14, np.uint32, 1, "ng"), "gcount": (15, np.uint32, 1, "ng"), "glo": (16, np.float32, 4, "ng"),
     "ghi": (17, np.float32, 4, "ng"), "ncell": (18, np.uint32, 1, "ng"), "npart": (19, np.uint32, 1, "ng"),
-    "nhard": (20, np.uint32, 1, "ng"), "interactions": (21, np.uint64, 2, "fixed"),
+    "nhard": (20, np.uint32, 1, "ng"), "interactions": (21, np.uint64, 3, "fixed"),
     "timings": (22, np.float32, 8, "fixed"), "bbox": (23, np.float32, 6, "fixed"), "keys": (24, np.uint64, 1, "n"),
     "M64": (25, np.float64, 1, "nn"), "C64": (26, np.float64, 3, "nn"), "B2": (27, np.float64, 1, "nn"),
     "bmax": (28, np.float64, 1, "nn"),
@@ -39,7 +39,7 @@ class HybParams(C.Structure):
     _fields_ = [("G", C.c_float), ("eps", C.c_float), ("theta", C.c_float), ("a_err", C.c_float),
                 ("r_in", C.c_float), ("r_out", C.c_float), ("dt_soft", C.c_float),
                 ("n_sub", C.c_int32), ("leaf_max", C.c_int32), ("group_max", C.c_int32),
-                ("mac", C.c_int32), ("kfunc", C.c_int32), ("split", C.c_int32)]
+                ("mac", C.c_int32), ("kfunc", C.c_int32), ("split", C.c_int32), ("grouping", C.c_int32)]
 
     @classmethod
     def from_config(cls, cfg, **over):

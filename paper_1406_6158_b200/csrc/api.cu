@@ -65,6 +65,7 @@ static bool params_ok(const hyb_params *p, int64_t n, char *msg)
     if (p->mac == HYB_MAC_ABS && !(p->a_err > 0.0f && isfinite(p->a_err))) return bad("a_err must be finite and > 0");
     if (p->kfunc != HYB_K_PAPER && p->kfunc != HYB_K_POLY7) return bad("unknown kfunc");
     if (p->split != 0 && p->split != 1) return bad("split must be 0 or 1");
+    if (p->grouping != HYB_GROUP_NODE && p->grouping != HYB_GROUP_SIBLINGS && p->grouping != HYB_GROUP_AUTO) return bad("unknown grouping");
     if (p->split == 1 && !(p->r_in >= 0.0f && p->r_out > p->r_in && isfinite(p->r_out))) return bad("need 0 <= r_in < r_out");
     return true;
 }
@@ -91,8 +92,10 @@ static int status_to_error(Ctx *c, u32 st)
     return HYB_OK;
 }
 
-static int do_build(Ctx *c)
+static int do_build(Ctx *c, bool hard_only = false)
 {
+    // HYB_GROUP_AUTO: fuller groups for the soft walk, single nodes when only a hard walk follows
+    c->grouping_now = c->p.grouping == HYB_GROUP_AUTO ? (hard_only ? HYB_GROUP_NODE : HYB_GROUP_SIBLINGS) : c->p.grouping;
     cudaError_t e = launch_build_tree(c);
     if (e != cudaSuccess) return cuda_fail(c, e, "build_tree");
     c->tree_valid = true;
@@ -182,8 +185,8 @@ int hyb_set_params(hyb_ctx *ctx, const hyb_params *params)
     char msg[256];
     if (!c) return fail(nullptr, HYB_ERR_INVALID_ARG, "ctx is NULL");
     if (!params_ok(params, c->n, msg)) return fail(c, HYB_ERR_INVALID_ARG, msg);
-    if (params->leaf_max != c->p.leaf_max || params->group_max != c->p.group_max)
-        return fail(c, HYB_ERR_INVALID_ARG, "leaf_max / group_max cannot change after hyb_init");
+    if (params->leaf_max != c->p.leaf_max || params->group_max != c->p.group_max || params->grouping != c->p.grouping)
+        return fail(c, HYB_ERR_INVALID_ARG, "leaf_max / group_max / grouping cannot change after hyb_init");
     c->p = *params;
     c->tree_valid = false; c->acc_valid = false;
     return HYB_OK;
@@ -260,9 +263,9 @@ int hyb_step(hyb_ctx *ctx, int32_t n_soft_steps)
             else e = launch_kick_drift(c, open_c, 0.0f, dth);
             if (e != cudaSuccess) return cuda_fail(c, e, "kick_drift");
             cudaEvent_t e1 = c->timing ? ev() : nullptr;
-            if ((rc = do_build(c)) != HYB_OK) return rc;
-            cudaEvent_t e2 = c->timing ? ev() : nullptr;
             const bool soft_step = !split || k == nsub - 1;
+            if ((rc = do_build(c, !soft_step)) != HYB_OK) return rc;
+            cudaEvent_t e2 = c->timing ? ev() : nullptr;
             if (soft_step) rc = do_soft(c); else rc = do_hard(c);
             if (rc != HYB_OK) return rc;
             cudaEvent_t e3 = c->timing ? ev() : nullptr;
@@ -315,10 +318,10 @@ int hyb_export(hyb_ctx *ctx, int32_t what, void *host_dst, size_t bytes, size_t 
         if (bytes < sizeof h.bbox) return fail(c, HYB_ERR_INVALID_ARG, "buffer too small");
         memcpy(host_dst, h.bbox, sizeof h.bbox); if (written) *written = sizeof h.bbox; return HYB_OK;
     case HYB_X_INTERACTIONS: {
-        u64 v[2] = {h.inter_soft, h.inter_hard};
+        u64 v[3] = {h.inter_soft, h.inter_hard, h.inter_hard_fused};
         if (bytes < sizeof v) return fail(c, HYB_ERR_INVALID_ARG, "buffer too small");
         memcpy(host_dst, v, sizeof v); if (written) *written = sizeof v;
-        cudaMemset(&c->ctl->inter_soft, 0, 2 * sizeof(u64));
+        cudaMemset(&c->ctl->inter_soft, 0, 3 * sizeof(u64));
         return HYB_OK; }
     case HYB_X_TIMINGS:
         if (bytes < sizeof c->t_acc) return fail(c, HYB_ERR_INVALID_ARG, "buffer too small");
@@ -414,7 +417,11 @@ int hyb_run_host(const hyb_params *params, int64_t n, hyb_float4 *h_pos_m, hyb_f
         cudaMemcpyAsync(h_a_hard, d + o_ah, 16 * N, cudaMemcpyDeviceToHost, st);
         cudaMemcpyAsync(h_id, d + o_id, 4 * N, cudaMemcpyDeviceToHost, st);
         if ((e = cudaStreamSynchronize(st)) != cudaSuccess) { rc = cuda_fail(nullptr, e, "copy back"); break; }
-        if (h_interactions) rc = hyb_export(ctx, HYB_X_INTERACTIONS, h_interactions, 16, nullptr);
+        if (h_interactions) {
+            uint64_t v[3];
+            rc = hyb_export(ctx, HYB_X_INTERACTIONS, v, sizeof v, nullptr);
+            h_interactions[0] = v[0]; h_interactions[1] = v[1];
+        }
     } while (0);
     if (ctx) hyb_free(ctx);
     if (st) cudaStreamDestroy(st);

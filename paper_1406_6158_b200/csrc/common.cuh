@@ -62,7 +62,8 @@ struct DevCtl {
     // ---- walk ----
     u32 group_counter;          // ---- walk work distribution: reset before every launch (2 words)
     u32 nheavy;                 // sink ranges of split groups (hard walk)
-    u64 inter_soft, inter_hard;
+    u32 walk_ng;                // number of groups of the last walk (is its nhard[] comparable?)
+    u64 inter_soft, inter_hard, inter_hard_fused;   // pair counts: soft lists, hard lists (all walks), hard lists of fused walks
 };
 
 // One tree node as the walk reads it: 64 bytes, children of a cell are contiguous (T7).
@@ -112,6 +113,7 @@ struct Ctx {
     char *ws;
     Layout L;
     bool tree_valid, acc_valid;
+    int grouping_now;              // HYB_GROUP_NODE / SIBLINGS of the build being enqueued
     cudaEvent_t ev[5];
     float t_acc[8];
     bool timing;

@@ -361,17 +361,31 @@ __global__ void __launch_bounds__(256) ropen_abs_kernel(const DevCtl *__restrict
 // ------------------------------------------------------------------ a7: groups (T11)
 __global__ void __launch_bounds__(256) gmark_kernel(const DevCtl *__restrict__ ctl, const u32 *__restrict__ first,
                                                     const u32 *__restrict__ count, const u32 *__restrict__ child,
-                                                    const u32 *__restrict__ parent, int group_max,
+                                                    const unsigned char *__restrict__ nchild,
+                                                    const u32 *__restrict__ parent, int group_max, int grouping,
                                                     unsigned char *gflag)
 {
     const u32 nn = ctl->nn;
     const u32 b = blockIdx.x * blockDim.x + threadIdx.x;
     if (b >= nn) return;
     const u32 c = count[b], f = first[b], gm = (u32)group_max;
-    if (c <= gm) {
-        if (b == 0 || count[parent[b]] > gm) gflag[f] = 1;
-    } else if (child[b] == NOCHILD) {
+    if (c > gm && child[b] == NOCHILD) {
         for (u32 s = f; s < f + c; s += gm) gflag[s] = 1;       // level-21 leaf cut into chunks
+    } else if (grouping == HYB_GROUP_NODE) {
+        if (c <= gm && (b == 0 || count[parent[b]] > gm)) gflag[f] = 1;
+    } else if (c <= gm) {
+        if (b == 0) gflag[f] = 1;                               // the whole system is one group
+    } else {
+        // the children in order: consecutive small ones are packed greedily into runs of <= gm sinks
+        u32 run = 0;
+        bool open = false;
+        const u32 c0 = child[b], nc = nchild[b];
+        for (u32 q = c0; q < c0 + nc; q++) {
+            const u32 cq = count[q];
+            if (cq > gm) { open = false; run = 0; continue; }
+            if (!open || run + cq > gm) { gflag[first[q]] = 1; run = 0; open = true; }
+            run += cq;
+        }
     }
 }
 
@@ -517,8 +531,8 @@ cudaError_t launch_build_tree(Ctx *c)
     cudaEventRecord(c->ev_linked, st);
     cudaStreamWaitEvent(ax, c->ev_linked, 0);
     unsigned char *gflag = wsptr<unsigned char>(c, L.gflag);
-    gmark_kernel<<<(int)((L.node_cap + 255) / 256), 256, 0, ax>>>(ctl, first, count, child, parent, c->p.group_max,
-                                                                  gflag);
+    gmark_kernel<<<(int)((L.node_cap + 255) / 256), 256, 0, ax>>>(ctl, first, count, child, nchild, parent,
+                                                                  c->p.group_max, c->grouping_now, gflag);
     u32 *gfirst = wsptr<u32>(c, L.gfirst);
     gscan_kernel<<<sc_grid, SC_THREADS, 0, ax>>>(gflag, n, ctl, sc_status + L.po_tiles, gfirst);
     ginfo_kernel<<<(int)imin64((c->n + 255) / 256, (int64_t)c->num_sms * 8), 256, 0, ax>>>(

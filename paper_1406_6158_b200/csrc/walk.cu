@@ -387,6 +387,7 @@ __global__ void __launch_bounds__(WK_WARPS * 32, SmemLayout<MODE>::ctas_per_sm) 
 
     const u32 lt_mask = (1u << lane) - 1u;
     const u32 ng = a.ctl->ng;
+    if (blockIdx.x == 0 && threadIdx.x == 0) a.ctl->walk_ng = ng;      // read by the next split_kernel
     const float rout2 = __fmul_rn(a.rout, a.rout);
     const float eps2 = a.eps2, kc0 = a.kc0, kc1 = a.kc1;
     unsigned long long isoft = 0, ihard = 0;
@@ -692,6 +693,7 @@ __global__ void __launch_bounds__(WK_WARPS * 32, SmemLayout<MODE>::ctas_per_sm) 
     if (lane == 0) {
         if (isoft) atomicAdd(&a.ctl->inter_soft, isoft);
         if (ihard) atomicAdd(&a.ctl->inter_hard, ihard);
+        if (ihard && MODE == WALK_HYBRID) atomicAdd(&a.ctl->inter_hard_fused, ihard);
     }
 }
 
@@ -703,9 +705,11 @@ __global__ void __launch_bounds__(256) split_kernel(DevCtl *ctl, const u32 *__re
                                                     const u32 *__restrict__ nhard, u32 *__restrict__ heavy,
                                                     unsigned char *__restrict__ is_split, unsigned long long t2, unsigned long long t4)
 {
-    const u32 ng = ctl->ng;
+    const u32 ng = ctl->ng, prev = ctl->walk_ng;
+    // the estimate is only meaningful when the previous walk had about the same groups
+    const bool comparable = (prev > ng ? prev - ng : ng - prev) <= ng / 16u;
     for (u32 g = blockIdx.x * blockDim.x + threadIdx.x; g < ng; g += gridDim.x * blockDim.x) {
-        const u32 n = gcount[g], h = nhard[g];
+        const u32 n = gcount[g], h = comparable ? nhard[g] : 0u;
         const unsigned long long est = (unsigned long long)n * (unsigned long long)h;
         u32 nsub = 1;
         if (est >= t4 && n >= 32u) nsub = 4;

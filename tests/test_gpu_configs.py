@@ -48,6 +48,18 @@ def test_cfg2_full(mac):
     h.close()
 
 
+def test_cfg2_single_node_groups():
+    """the other reading of R17 (one tree node per sink group) at the benchmark size"""
+    cfg = CONFIGS[2]
+    pos, vel = make_ic(cfg.kind, cfg.n, cfg.seed)
+    h = make_hyb(cfg, pos, vel, grouping=0)
+    h.build_tree(); h.sync()
+    t = O.Tree(pos, O.params_from(cfg, grouping=0))
+    compare_tree(h, t)
+    print(check_forces(h, t, gsel=_sample_groups(t.ng, 8192, 8)))
+    h.close()
+
+
 def test_cfg2_normal_tree():
     cfg = CONFIGS[2]
     pos, vel = make_ic(cfg.kind, cfg.n, cfg.seed)

@@ -21,11 +21,12 @@ def _run_case(cfg, pos, vel, **over):
     return res
 
 
+@pytest.mark.parametrize("grouping", [1, 0])
 @pytest.mark.parametrize("mac", [0, 1])
-def test_cfg0_all_stages(mac):
+def test_cfg0_all_stages(mac, grouping):
     cfg = CONFIGS[0]
     pos, vel = make_ic(cfg.kind, cfg.n, cfg.seed)
-    print(_run_case(cfg, pos, vel, mac=mac))
+    print(_run_case(cfg, pos, vel, mac=mac, grouping=grouping))
 
 
 def test_cfg0_normal_tree():
@@ -39,9 +40,10 @@ def test_cfg0_normal_tree():
                                                (1, "cold_sphere", 8, 32), (2, "cold_sphere", 8, 32),
                                                (37, "plummer", 8, 32)])
 def test_ragged_sizes(n, kind, leaf, group):
-    cfg = CONFIGS[1].with_(n=n, kind=kind, leaf_max=leaf, group_max=group)
-    pos, vel = make_ic(kind, n, 17)
-    print(_run_case(cfg, pos, vel))
+    for grouping in (1, 0):
+        cfg = CONFIGS[1].with_(n=n, kind=kind, leaf_max=leaf, group_max=group, grouping=grouping)
+        pos, vel = make_ic(kind, n, 17)
+        print(_run_case(cfg, pos, vel))
 
 
 def test_coincident_points_and_depth_limit():
@@ -54,6 +56,7 @@ def test_coincident_points_and_depth_limit():
     pos[:, 3] = 1.0 / 3000
     vel = np.zeros_like(pos)
     print(_run_case(cfg, pos, vel))
+    print(_run_case(cfg, pos, vel, grouping=0))
 
 
 def test_theta_zero_opens_everything():

@@ -144,18 +144,53 @@ def test_abs_mode_B2_bmax(cfg0, ic0):
     assert len(single) and np.all(ropen2[single] == 0.0)                               # single particle -> r_b = 0
 
 
-def test_groups(tree0, cfg0):
-    gf, gc = tree0.get("gfirst").astype(np.int64), tree0.get("gcount").astype(np.int64)
-    assert gf[0] == 0 and np.array_equal(gf[1:], np.cumsum(gc)[:-1]) and gc.sum() == tree0.n
-    assert gc.max() <= cfg0.group_max and gc.min() >= 1
-    first, count, parent = tree0.get("first"), tree0.get("count"), tree0.get("parent")
-    node_of = {(int(f), int(c)): k for k, (f, c) in enumerate(zip(first, count))}
+def _groups_tile(t, group_max):
+    gf, gc = t.get("gfirst").astype(np.int64), t.get("gcount").astype(np.int64)
+    assert gf[0] == 0 and np.array_equal(gf[1:], np.cumsum(gc)[:-1]) and gc.sum() == t.n
+    assert gc.max() <= group_max and gc.min() >= 1
+    return gf, gc
+
+
+def test_groups_single_nodes(cfg0, ic0):
+    """grouping 0 (R17, first reading): a group is a maximal tree node of <= group_max particles"""
+    t = O.Tree(ic0[0], O.params_from(cfg0, grouping=0))
+    gf, gc = _groups_tile(t, cfg0.group_max)
+    first, count, parent = t.get("first"), t.get("count"), t.get("parent")
     for f, c in zip(gf, gc):
         # several nodes on a one-child chain can share (first,count); any of them works for the parent check
-        ks = [k for k in range(tree0.nn) if first[k] == f and count[k] == c]
+        ks = [k for k in range(t.nn) if first[k] == f and count[k] == c]
         assert ks, "every group is a tree node here (no level-21 chunks in cfg0)"
         top = min(ks)
         assert top == 0 or count[parent[top]] > cfg0.group_max
+
+
+def test_groups(tree0, cfg0):
+    """grouping 1 (the configs' default): greedy runs of consecutive small children of one cell"""
+    assert cfg0.grouping in (1, 2) and tree0.params.grouping == 1
+    gf, gc = _groups_tile(tree0, cfg0.group_max)
+    gm = cfg0.group_max
+    first, count, parent, child, nchild = (tree0.get(k).astype(np.int64) for k in ("first", "count", "parent", "child", "nchild"))
+    # brute force, written differently from the oracle: walk the cells that are too big for one group
+    # and cut their list of children wherever the running total would pass group_max
+    starts = set()
+    big = [k for k in range(tree0.nn) if count[k] > gm]
+    for k in big:
+        assert child[k] != NOCHILD, "no level-21 chunks in cfg0"
+        kids = list(range(child[k], child[k] + nchild[k]))
+        i = 0
+        while i < len(kids):
+            if count[kids[i]] > gm:
+                i += 1
+                continue
+            j, tot = i, 0
+            while j < len(kids) and count[kids[j]] <= gm and tot + count[kids[j]] <= gm:
+                tot += count[kids[j]]; j += 1
+            starts.add(int(first[kids[i]]))
+            i = j
+    assert starts == set(int(f) for f in gf)
+    # fewer and fuller groups than one node per group, and never across the parent cell
+    t0 = O.Tree(tree0.get("pos_sorted"), O.params_from(cfg0, grouping=0))
+    assert tree0.ng < t0.ng and set(int(f) for f in gf) <= set(int(f) for f in t0.get("gfirst"))
     ps = tree0.get("pos_sorted")
     glo, ghi = tree0.get("glo"), tree0.get("ghi")
     for g in range(0, tree0.ng, 17):

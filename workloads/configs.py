@@ -24,6 +24,8 @@ class Config:
     mac: int = 0                 # 0 = theta, 1 = absolute MAC (Eq. 5-6)
     kfunc: int = 0               # 0 = paper Eq. 10
     split: int = 1               # 1 = hybrid, 0 = normal tree
+    grouping: int = 2            # sink groups: 1 = runs of consecutive small sibling cells, 0 = single tree nodes,
+                                 # 2 = 1, except 0 for the trees of hyb_step that only a hard walk uses
 
     def with_(self, **kw) -> "Config":
         return replace(self, **kw)
