@@ -26,6 +26,8 @@ Layout plan_workspace(int64_t n)
     L.node_tiles = (L.node_cap + RS_TILE - 1) / RS_TILE;
     L.sc_tiles = (n + SC_TILE - 1) / SC_TILE;
     L.po_tiles = (n + PO_TILE - 1) / PO_TILE;
+    L.rs_blocks = (L.rs_tiles + LB_WIN - 1) / LB_WIN;
+    L.node_blocks = (L.node_tiles + LB_WIN - 1) / LB_WIN;
     size_t off = 0;
     auto take = [&](size_t bytes) { size_t o = off; off = align_up(off + bytes); return o; };
     const size_t N = (size_t)n, NC = (size_t)L.node_cap, GC = (size_t)L.group_cap;
@@ -33,11 +35,11 @@ Layout plan_workspace(int64_t n)
     L.key_orig = take(8 * N); L.key_a = take(8 * N); L.key_b = take(8 * N);
     L.val_a = take(4 * N); L.val_b = take(4 * N);
     L.pos_tmp = take(16 * N); L.vel_tmp = take(16 * N); L.id_tmp = take(4 * N);
-    L.rs_status = take(4 * 256 * (size_t)L.rs_tiles * RS_PASSES);
+    L.rs_status = take(4 * 256 * (size_t)(L.rs_tiles + L.rs_blocks) * RS_PASSES);
     L.sc_status = take(8 * (size_t)(L.sc_tiles + L.po_tiles));
     L.dlev = take(N); L.cnt_slot = take(4 * N); L.gflag = take(N);
     L.pre_level = take(NC); L.pre_first = take(4 * NC); L.pre_of_bfs = take(4 * NC); L.bfs_of_pre = take(4 * NC);
-    L.node_status = take(4 * 256 * (size_t)L.node_tiles);
+    L.node_status = take(4 * 256 * (size_t)(L.node_tiles + L.node_blocks));
     L.level = take(NC); L.first = take(4 * NC); L.count = take(4 * NC); L.child = take(4 * NC);
     L.nchild = take(NC); L.parent = take(4 * NC); L.arrived = take(4 * NC);
     L.nodes = take(sizeof(NodeRec) * NC);

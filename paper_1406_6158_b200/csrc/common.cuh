@@ -27,6 +27,7 @@ constexpr int RS_THREADS = 256;
 constexpr int RS_KPT = 16;
 constexpr int RS_TILE = RS_THREADS * RS_KPT;
 constexpr int RS_PASSES = 8;      // 8 x 8 bits >= 63 bits
+constexpr int LB_WIN = 16;        // radix look-back: tiles per block = status words requested together
 
 // single-value scan tiles (octree preorder, group compaction)
 constexpr int SC_THREADS = 256;
@@ -79,7 +80,7 @@ struct Layout {   // byte offsets into the workspace; computed by plan_workspace
     size_t ctl;
     size_t key_orig, key_a, key_b, val_a, val_b;
     size_t pos_tmp, vel_tmp, id_tmp;
-    size_t rs_status;           // [RS_PASSES][ntiles][256] u32
+    size_t rs_status;           // [RS_PASSES][rs_tiles + rs_blocks][256] u32 (tile and block look-back statuses)
     size_t sc_status;           // u64 [po_tiles] (preorder scan) then [sc_tiles] (group scan)
     size_t dlev, cnt_slot;      // int8[n], u32[n]
     size_t gflag;               // u8[n]
@@ -94,6 +95,7 @@ struct Layout {   // byte offsets into the workspace; computed by plan_workspace
     size_t total;
     int64_t n, node_cap, group_cap;
     int64_t rs_tiles, node_tiles, sc_tiles, po_tiles;
+    int64_t rs_blocks, node_blocks;      // look-back blocks of LB_WIN tiles
 };
 
 inline int64_t node_capacity(int64_t n) { return 2 * n + 4096; }

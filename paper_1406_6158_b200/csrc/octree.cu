@@ -490,9 +490,9 @@ cudaError_t launch_build_tree(Ctx *c)
     cudaMemsetAsync(reinterpret_cast<char *>(ctl) + offsetof(DevCtl, bbox_enc), 0,
                     offsetof(DevCtl, bbox) - offsetof(DevCtl, bbox_enc), st);
     cudaMemsetAsync(reinterpret_cast<char *>(ctl) + offsetof(DevCtl, bbox_enc), 0xFF, 3 * sizeof(u32), st);
-    cudaMemsetAsync(c->ws + L.rs_status, 0, sizeof(u32) * 256 * (size_t)L.rs_tiles * RS_PASSES, st);
+    cudaMemsetAsync(c->ws + L.rs_status, 0, sizeof(u32) * 256 * (size_t)(L.rs_tiles + L.rs_blocks) * RS_PASSES, st);
     cudaMemsetAsync(c->ws + L.sc_status, 0, sizeof(u64) * (size_t)(L.sc_tiles + L.po_tiles), st);
-    cudaMemsetAsync(c->ws + L.node_status, 0, sizeof(u32) * 256 * (size_t)L.node_tiles, st);
+    cudaMemsetAsync(c->ws + L.node_status, 0, sizeof(u32) * 256 * (size_t)(L.node_tiles + L.node_blocks), st);
     cudaMemsetAsync(c->ws + L.gflag, 0, (size_t)n, st);
 
     cudaError_t e = launch_keys_sort_permute(c);
@@ -513,7 +513,7 @@ cudaError_t launch_build_tree(Ctx *c)
     u32 *pre_of_bfs = wsptr<u32>(c, L.pre_of_bfs), *bfs_of_pre = wsptr<u32>(c, L.bfs_of_pre);
     const int ngrid = (int)imin64(L.node_tiles, (int64_t)c->num_sms * 3);
     e = launch_radix_pass<unsigned char>(pre_level, nullptr, level, pre_of_bfs, bfs_of_pre, 0, &ctl->nn, 0,
-                                         ctl->node_base, wsptr<u32>(c, L.node_status), &ctl->tile_counter[10],
+                                         ctl->node_base, wsptr<u32>(c, L.node_status), (u32)L.node_tiles, &ctl->tile_counter[10],
                                          &ctl->status, ngrid, st);
     if (e != cudaSuccess) return e;
 

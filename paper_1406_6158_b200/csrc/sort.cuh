@@ -8,7 +8,6 @@
 
 namespace hyb {
 
-constexpr int LB_WIN = 16;        // look-back window (status words requested together)
 constexpr u32 RS_FLAG_AGG = 1u << 30, RS_FLAG_PREFIX = 2u << 30, RS_VALUE_MASK = (1u << 30) - 1;
 
 struct RadixSmem {
@@ -28,7 +27,7 @@ template <typename KeyT>
 __global__ void __launch_bounds__(RS_THREADS) radix_pass_kernel(
     const KeyT *__restrict__ kin, const u32 *__restrict__ vin, KeyT *__restrict__ kout, u32 *__restrict__ vout,
     u32 *__restrict__ inv_out, u32 n_host, const u32 *__restrict__ n_dev, int shift,
-    const u32 *__restrict__ digit_base, u32 *status, u32 *tile_counter, u32 *dev_status)
+    const u32 *__restrict__ digit_base, u32 *status, u32 tiles_alloc, u32 *tile_counter, u32 *dev_status)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     RadixSmem &sm = *reinterpret_cast<RadixSmem *>(smem_raw);
@@ -94,36 +93,67 @@ __global__ void __launch_bounds__(RS_THREADS) radix_pass_kernel(
             total += t;
         }
         // publish + look back (thread d for digit d).  All tiles of a pass are usually resident at once
-        // and publish at about the same time, so a tile may have to walk far back: LB_WIN predecessors
-        // are requested together and consumed in order, which divides the number of round trips.
+        // and publish at about the same time, so a plain decoupled look-back would walk back to tile 0
+        // (O(tiles^2) status reads).  Two levels instead: LB_WIN consecutive tiles form a block; a tile
+        // sums the aggregates of the earlier tiles of its block (one round trip); the last tile of a block
+        // publishes the block aggregate and looks back over BLOCK statuses, LB_WIN at a time, then
+        // publishes the block's inclusive prefix, which the tiles of the next block wait for.
         u32 excl = 0;
         {
             volatile u32 *st = status;
-            const size_t me = (size_t)tile * 256 + tid;
-            if (tile == 0) st[me] = RS_FLAG_PREFIX | total;
-            else {
-                st[me] = RS_FLAG_AGG | total;
-                long long t = (long long)tile - 1;
-                int spins = 0;
-                bool done = false;
-                while (!done) {
-                    u32 s[LB_WIN];
+            volatile u32 *bs = status + (size_t)tiles_alloc * 256;
+            const u32 blk = tile / LB_WIN, r = tile % LB_WIN;
+            st[(size_t)tile * 256 + tid] = RS_FLAG_AGG | total;
+            u32 inblk = 0;
+            int spins = 0;
+            if (r > 0) {
+                u32 s[LB_WIN - 1];
+                bool ready;
+                do {
+                    ready = true;
 #pragma unroll
-                    for (int i = 0; i < LB_WIN; i++)
-                        s[i] = (t - i >= 0) ? st[(size_t)(t - i) * 256 + tid] : (2u << 30);
+                    for (int i = 0; i < LB_WIN - 1; i++)
+                        s[i] = ((u32)i < r) ? st[((size_t)blk * LB_WIN + i) * 256 + tid] : (1u << 30);
 #pragma unroll
-                    for (int i = 0; i < LB_WIN; i++) {
-                        if (done) break;
-                        const u32 f = s[i] >> 30;
-                        if (f == 0) break;                       // not published yet: poll again from here
-                        excl += s[i] & RS_VALUE_MASK;
-                        t--;
-                        if (f == 2) done = true;
-                    }
-                    if (!done && ++spins >= LB_SPIN_LIMIT) { atomicOr(dev_status, ST_WAIT_EXPIRED); break; }
-                }
-                st[me] = RS_FLAG_PREFIX | (excl + total);
+                    for (int i = 0; i < LB_WIN - 1; i++) ready = ready && (s[i] >> 30) != 0u;
+                } while (!ready && ++spins < LB_SPIN_LIMIT);
+#pragma unroll
+                for (int i = 0; i < LB_WIN - 1; i++) inblk += ((u32)i < r) ? (s[i] & RS_VALUE_MASK) : 0u;
             }
+            u32 bexcl = 0;
+            const bool leader = r == LB_WIN - 1 || tile == ntiles - 1;
+            if (leader) {
+                const size_t me = (size_t)blk * 256 + tid;
+                if (blk == 0) bs[me] = RS_FLAG_PREFIX | (inblk + total);
+                else {
+                    bs[me] = RS_FLAG_AGG | (inblk + total);
+                    long long t = (long long)blk - 1;
+                    bool done = false;
+                    while (!done) {
+                        u32 s[LB_WIN];
+#pragma unroll
+                        for (int i = 0; i < LB_WIN; i++)
+                            s[i] = (t - i >= 0) ? bs[(size_t)(t - i) * 256 + tid] : (2u << 30);
+#pragma unroll
+                        for (int i = 0; i < LB_WIN; i++) {
+                            if (done) break;
+                            const u32 f = s[i] >> 30;
+                            if (f == 0) break;                   // not published yet: poll again from here
+                            bexcl += s[i] & RS_VALUE_MASK;
+                            t--;
+                            if (f == 2) done = true;
+                        }
+                        if (!done && ++spins >= LB_SPIN_LIMIT) break;
+                    }
+                    bs[me] = RS_FLAG_PREFIX | (bexcl + inblk + total);
+                }
+            } else if (blk > 0) {
+                u32 sv;
+                do { sv = bs[(size_t)(blk - 1) * 256 + tid]; } while ((sv >> 30) != 2u && ++spins < LB_SPIN_LIMIT);
+                bexcl = sv & RS_VALUE_MASK;
+            }
+            if (spins >= LB_SPIN_LIMIT) atomicOr(dev_status, ST_WAIT_EXPIRED);
+            excl = bexcl + inblk;
         }
         // block exclusive scan of the digit totals -> digit_start
         u32 incl = total;
@@ -167,7 +197,7 @@ __global__ void __launch_bounds__(RS_THREADS) radix_pass_kernel(
 
 template <typename KeyT>
 static cudaError_t launch_radix_pass(const KeyT *kin, const u32 *vin, KeyT *kout, u32 *vout, u32 *inv_out, u32 n_host,
-                                     const u32 *n_dev, int shift, const u32 *digit_base, u32 *status,
+                                     const u32 *n_dev, int shift, const u32 *digit_base, u32 *status, u32 tiles_alloc,
                                      u32 *tile_counter, u32 *dev_status, int grid, cudaStream_t st)
 {
     static bool attr_set = false;
@@ -178,8 +208,8 @@ static cudaError_t launch_radix_pass(const KeyT *kin, const u32 *vin, KeyT *kout
         attr_set = true;
     }
     radix_pass_kernel<KeyT><<<grid, RS_THREADS, sizeof(RadixSmem), st>>>(kin, vin, kout, vout, inv_out, n_host, n_dev,
-                                                                         shift, digit_base, status, tile_counter,
-                                                                         dev_status);
+                                                                         shift, digit_base, status, tiles_alloc,
+                                                                         tile_counter, dev_status);
     return cudaGetLastError();
 }
 
