@@ -94,3 +94,58 @@ def test_paper_parameter_recipe():
     h.step(1); h.sync()
     assert np.all(np.isfinite(h.pos_m.cpu().numpy()))
     h.close()
+
+
+def test_error_paths_on_device():
+    """every failure is reported as an error code, never silently (include/hyb.h)"""
+    import torch
+    from paper_1406_6158_b200 import Hyb, HybError, HybParams
+    cfg = CONFIGS[0].with_(n=1000)
+    pos, vel = make_ic(cfg.kind, cfg.n, 4)
+    # force call without a tree
+    h = make_hyb(cfg, pos, vel)
+    with pytest.raises(HybError) as ei:
+        h.hard_force()
+    assert ei.value.code == -5
+    with pytest.raises(HybError) as ei:
+        h.soft_force()
+    assert ei.value.code == -5
+    h.build_tree(); h.soft_force(); h.sync()
+    # parameters that cannot change after init
+    with pytest.raises(HybError) as ei:
+        h.set_params(HybParams.from_config(cfg, leaf_max=4))
+    assert ei.value.code == -1
+    # changing theta invalidates the tree
+    h.set_params(HybParams.from_config(cfg, theta=0.7))
+    with pytest.raises(HybError) as ei:
+        h.soft_force()
+    assert ei.value.code == -5
+    h.close()
+    # non-finite position, negative mass
+    for bad in ("nan", "neg"):
+        p2 = pos.copy()
+        if bad == "nan":
+            p2[17, 1] = np.nan
+        else:
+            p2[5, 3] = -1.0
+        h = make_hyb(cfg, p2, vel)
+        h.build_tree()
+        with pytest.raises(HybError) as ei:
+            h.sync()
+        assert ei.value.code == -3
+        h.close()
+    # misaligned / missing pointers and a workspace that is too small are refused by hyb_init
+    from paper_1406_6158_b200.binding import hyb_workspace_bytes, lib
+    import ctypes as C
+    P = HybParams.from_config(cfg)
+    need = hyb_workspace_bytes(cfg.n, P)
+    dpos = torch.from_numpy(pos).cuda(); dvel = torch.from_numpy(vel).cuda()
+    acc = torch.zeros_like(dpos); ids = torch.arange(cfg.n, dtype=torch.int32, device="cuda")
+    ws = torch.empty(need, dtype=torch.uint8, device="cuda")
+    hnd = C.c_void_p()
+    rc = lib().hyb_init(C.byref(hnd), C.byref(P), cfg.n, dpos.data_ptr(), dvel.data_ptr(), acc.data_ptr(), acc.data_ptr(),
+                        ids.data_ptr(), ws.data_ptr(), need - 1, 0, None)
+    assert rc == -2 and not hnd.value
+    rc = lib().hyb_init(C.byref(hnd), C.byref(P), cfg.n, dpos.data_ptr() + 4, dvel.data_ptr(), acc.data_ptr(), acc.data_ptr(),
+                        ids.data_ptr(), ws.data_ptr(), need, 0, None)
+    assert rc == -1 and not hnd.value
