@@ -98,13 +98,14 @@ static int do_build(Ctx *c, bool hard_only = false)
 {
     // HYB_GROUP_AUTO: fuller groups for the soft walk, single nodes when only a hard walk follows
     c->grouping_now = c->p.grouping == HYB_GROUP_AUTO ? (hard_only ? HYB_GROUP_NODE : HYB_GROUP_SIBLINGS) : c->p.grouping;
+    c->boxes_only = hard_only;
     cudaError_t e = launch_build_tree(c);
     if (e != cudaSuccess) return cuda_fail(c, e, "build_tree");
     c->tree_valid = true;
     c->acc_valid = false;
     // bbox, root cube, keys, digit bases, 8 sort passes, permute | preorder, level offsets, level sort,
     // link, upsweep, group mark / scan / info (+ b_max, r_b in absolute-MAC mode)
-    c->launches += 13 + 8 + (c->p.mac == HYB_MAC_ABS ? 2 : 0);
+    c->launches += 13 + 8 + (c->p.mac == HYB_MAC_ABS && !hard_only ? 2 : 0);
     return HYB_OK;
 }
 

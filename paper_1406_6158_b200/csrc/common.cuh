@@ -116,6 +116,7 @@ struct Ctx {
     Layout L;
     bool tree_valid, acc_valid;
     int grouping_now;              // HYB_GROUP_NODE / SIBLINGS of the build being enqueued
+    bool boxes_only;               // the build being enqueued is read by a hard walk only: no moments
     cudaEvent_t ev[5];
     float t_acc[8];
     bool timing;

@@ -232,6 +232,9 @@ __device__ __forceinline__ void finish_node(const NodeArrays &na, u32 b, int lev
     na.C64[3 * (size_t)b] = Cx; na.C64[3 * (size_t)b + 1] = Cy; na.C64[3 * (size_t)b + 2] = Cz;
 }
 
+// MOMENTS = false: tight boxes only.  hyb_step uses it for the trees that only a hard walk reads (rule
+// (b) and the hard list need the boxes and the topology, not the centres of mass).
+template <bool MOMENTS>
 __global__ void __launch_bounds__(128) upsweep_kernel(NodeArrays na, const float4 *__restrict__ pos,
                                                       const DevCtl *__restrict__ ctl, int mac, float theta)
 {
@@ -247,25 +250,32 @@ __global__ void __launch_bounds__(128) upsweep_kernel(NodeArrays na, const float
         float3 lo = make_float3(p0.x, p0.y, p0.z), hi = lo;
         for (u32 j = f; j < f + c; j++) {
             float4 p = __ldg(pos + j);
-            double m = (double)p.w;
-            M = __dadd_rn(M, m);
-            Sx = __dadd_rn(Sx, __dmul_rn(m, (double)p.x));
-            Sy = __dadd_rn(Sy, __dmul_rn(m, (double)p.y));
-            Sz = __dadd_rn(Sz, __dmul_rn(m, (double)p.z));
+            if (MOMENTS) {
+                double m = (double)p.w;
+                M = __dadd_rn(M, m);
+                Sx = __dadd_rn(Sx, __dmul_rn(m, (double)p.x));
+                Sy = __dadd_rn(Sy, __dmul_rn(m, (double)p.y));
+                Sz = __dadd_rn(Sz, __dmul_rn(m, (double)p.z));
+            }
             lo.x = fminf(lo.x, p.x); lo.y = fminf(lo.y, p.y); lo.z = fminf(lo.z, p.z);
             hi.x = fmaxf(hi.x, p.x); hi.y = fmaxf(hi.y, p.y); hi.z = fmaxf(hi.z, p.z);
-            if (mac == HYB_MAC_ABS) na.leaf_of[j] = b;
+            if (MOMENTS && mac == HYB_MAC_ABS) na.leaf_of[j] = b;
         }
-        double Cx, Cy, Cz;
-        finish_node(na, b, na.level[b], M, Sx, Sy, Sz, lo, hi, mac, Lf, theta, Cx, Cy, Cz);
-        if (mac == HYB_MAC_ABS) {
-            double B2 = 0.0;
-            for (u32 j = f; j < f + c; j++) {
-                float4 p = __ldg(pos + j);
-                double d2 = dist2_rn((double)p.x, (double)p.y, (double)p.z, Cx, Cy, Cz);
-                B2 = __dadd_rn(B2, __dmul_rn((double)p.w, d2));
+        if (!MOMENTS) {
+            na.rec[b].B = make_float4(lo.x, lo.y, lo.z, 0.0f);
+            na.rec[b].C = make_float4(hi.x, hi.y, hi.z, 0.0f);
+        } else {
+            double Cx, Cy, Cz;
+            finish_node(na, b, na.level[b], M, Sx, Sy, Sz, lo, hi, mac, Lf, theta, Cx, Cy, Cz);
+            if (mac == HYB_MAC_ABS) {
+                double B2 = 0.0;
+                for (u32 j = f; j < f + c; j++) {
+                    float4 p = __ldg(pos + j);
+                    double d2 = dist2_rn((double)p.x, (double)p.y, (double)p.z, Cx, Cy, Cz);
+                    B2 = __dadd_rn(B2, __dmul_rn((double)p.w, d2));
+                }
+                na.B2[b] = B2;
             }
-            na.B2[b] = B2;
         }
     }
     // ---- climb: the last child to arrive computes the parent, children in ascending order
@@ -281,28 +291,33 @@ __global__ void __launch_bounds__(128) upsweep_kernel(NodeArrays na, const float
         __threadfence();
         double M = 0.0, Sx = 0.0, Sy = 0.0, Sz = 0.0;
         float3 lo, hi;
-        {
-            for (u32 q = c0; q < c0 + nc; q++) {
+        for (u32 q = c0; q < c0 + nc; q++) {
+            if (MOMENTS) {
                 const double4 cm = ldcg_d4(na.MS64 + q);
                 M = __dadd_rn(M, cm.x); Sx = __dadd_rn(Sx, cm.y); Sy = __dadd_rn(Sy, cm.z); Sz = __dadd_rn(Sz, cm.w);
-                const float4 bl = __ldcg(&na.rec[q].B), bh = __ldcg(&na.rec[q].C);
-                if (q == c0) { lo = make_float3(bl.x, bl.y, bl.z); hi = make_float3(bh.x, bh.y, bh.z); }
-                else {
-                    lo.x = fminf(lo.x, bl.x); lo.y = fminf(lo.y, bl.y); lo.z = fminf(lo.z, bl.z);
-                    hi.x = fmaxf(hi.x, bh.x); hi.y = fmaxf(hi.y, bh.y); hi.z = fmaxf(hi.z, bh.z);
-                }
+            }
+            const float4 bl = __ldcg(&na.rec[q].B), bh = __ldcg(&na.rec[q].C);
+            if (q == c0) { lo = make_float3(bl.x, bl.y, bl.z); hi = make_float3(bh.x, bh.y, bh.z); }
+            else {
+                lo.x = fminf(lo.x, bl.x); lo.y = fminf(lo.y, bl.y); lo.z = fminf(lo.z, bl.z);
+                hi.x = fmaxf(hi.x, bh.x); hi.y = fmaxf(hi.y, bh.y); hi.z = fmaxf(hi.z, bh.z);
             }
         }
-        double Cx, Cy, Cz;
-        finish_node(na, par, plev, M, Sx, Sy, Sz, lo, hi, mac, Lf, theta, Cx, Cy, Cz);
-        if (mac == HYB_MAC_ABS) {            // parallel-axis sum of the children's B_2 (T10)
-            double B2 = 0.0;
-            for (u32 q = c0; q < c0 + nc; q++) {
-                double d2 = dist2_rn(__ldcg(na.C64 + 3 * (size_t)q), __ldcg(na.C64 + 3 * (size_t)q + 1),
-                                     __ldcg(na.C64 + 3 * (size_t)q + 2), Cx, Cy, Cz);
-                B2 = __dadd_rn(B2, __dadd_rn(__ldcg(na.B2 + q), __dmul_rn(__ldcg(&na.MS64[q].x), d2)));
+        if (!MOMENTS) {
+            na.rec[par].B = make_float4(lo.x, lo.y, lo.z, 0.0f);
+            na.rec[par].C = make_float4(hi.x, hi.y, hi.z, 0.0f);
+        } else {
+            double Cx, Cy, Cz;
+            finish_node(na, par, plev, M, Sx, Sy, Sz, lo, hi, mac, Lf, theta, Cx, Cy, Cz);
+            if (mac == HYB_MAC_ABS) {            // parallel-axis sum of the children's B_2 (T10)
+                double B2 = 0.0;
+                for (u32 q = c0; q < c0 + nc; q++) {
+                    double d2 = dist2_rn(__ldcg(na.C64 + 3 * (size_t)q), __ldcg(na.C64 + 3 * (size_t)q + 1),
+                                         __ldcg(na.C64 + 3 * (size_t)q + 2), Cx, Cy, Cz);
+                    B2 = __dadd_rn(B2, __dadd_rn(__ldcg(na.B2 + q), __dmul_rn(__ldcg(&na.MS64[q].x), d2)));
+                }
+                na.B2[par] = B2;
             }
-            na.B2[par] = B2;
         }
         cur = par;
     }
@@ -547,8 +562,9 @@ cudaError_t launch_build_tree(Ctx *c)
     na.B2 = wsptr<double>(c, L.B2); na.leaf_of = wsptr<u32>(c, L.leaf_of);
     const int full_node_grid = (int)((L.node_cap + 127) / 128);
     cudaStreamWaitEvent(st, c->ev_perm, 0);
-    upsweep_kernel<<<full_node_grid, 128, 0, st>>>(na, pos_t, ctl, c->p.mac, c->p.theta);
-    if (c->p.mac == HYB_MAC_ABS) {
+    if (c->boxes_only) upsweep_kernel<false><<<full_node_grid, 128, 0, st>>>(na, pos_t, ctl, c->p.mac, c->p.theta);
+    else upsweep_kernel<true><<<full_node_grid, 128, 0, st>>>(na, pos_t, ctl, c->p.mac, c->p.theta);
+    if (c->p.mac == HYB_MAC_ABS && !c->boxes_only) {
         bmax_kernel<<<(n + 255) / 256, 256, 0, st>>>(pos_t, n, na.leaf_of, parent, level, na.C64, bmax2);
         ropen_abs_kernel<<<(int)((L.node_cap + 255) / 256), 256, 0, st>>>(ctl, bmax2, na.B2, c->p.a_err, rec);
     }
