@@ -48,6 +48,7 @@ Layout plan_workspace(int64_t n)
     L.gfirst = take(4 * GC); L.gcount = take(4 * GC); L.glo = take(16 * GC); L.ghi = take(16 * GC);
     L.ncell = take(4 * GC); L.npart = take(4 * GC); L.nhard = take(4 * GC);
     L.splitq = take(4 * 4 * GC);
+    L.gnode = take(4 * GC); L.ganc = take(4 * GC);
     L.total = off;
     return L;
 }
@@ -105,7 +106,7 @@ static int do_build(Ctx *c, bool hard_only = false)
     c->acc_valid = false;
     // bbox, root cube, keys, digit bases, 8 sort passes, permute | preorder, level offsets, level sort,
     // link, upsweep, group mark / scan / info (+ b_max, r_b in absolute-MAC mode)
-    c->launches += 13 + 8 + (c->p.mac == HYB_MAC_ABS && !hard_only ? 2 : 0);
+    c->launches += 13 + 8 + (c->p.mac == HYB_MAC_ABS && !hard_only ? 2 : 0) + (c->p.split ? 1 : 0);     // + ganc
     return HYB_OK;
 }
 

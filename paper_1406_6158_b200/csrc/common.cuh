@@ -91,6 +91,7 @@ struct Layout {   // byte offsets into the workspace; computed by plan_workspace
     size_t MS64, C64, B2, bmax2;               // double[4nc] (M, Sx, Sy, Sz), [3nc], [nc], u64[nc]
     size_t leaf_of;             // u32[n]
     size_t gfirst, gcount, glo, ghi, ncell, npart, nhard;   // [group_cap]
+    size_t gnode, ganc;         // u32[group_cap]: tree node a group hangs from; start node of its hard walk
     size_t splitq;              // u32[4 group_cap]: sink ranges of split groups, processed first (walk.cu)
     size_t total;
     int64_t n, node_cap, group_cap;

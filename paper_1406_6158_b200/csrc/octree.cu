@@ -378,18 +378,18 @@ __global__ void __launch_bounds__(256) gmark_kernel(const DevCtl *__restrict__ c
                                                     const u32 *__restrict__ count, const u32 *__restrict__ child,
                                                     const unsigned char *__restrict__ nchild,
                                                     const u32 *__restrict__ parent, int group_max, int grouping,
-                                                    unsigned char *gflag)
+                                                    unsigned char *gflag, u32 *__restrict__ gnode_at)
 {
     const u32 nn = ctl->nn;
     const u32 b = blockIdx.x * blockDim.x + threadIdx.x;
     if (b >= nn) return;
     const u32 c = count[b], f = first[b], gm = (u32)group_max;
     if (c > gm && child[b] == NOCHILD) {
-        for (u32 s = f; s < f + c; s += gm) gflag[s] = 1;       // level-21 leaf cut into chunks
+        for (u32 s = f; s < f + c; s += gm) { gflag[s] = 1; gnode_at[s] = b; }     // level-21 leaf cut into chunks
     } else if (grouping == HYB_GROUP_NODE) {
-        if (c <= gm && (b == 0 || count[parent[b]] > gm)) gflag[f] = 1;
+        if (c <= gm && (b == 0 || count[parent[b]] > gm)) { gflag[f] = 1; gnode_at[f] = b; }
     } else if (c <= gm) {
-        if (b == 0) gflag[f] = 1;                               // the whole system is one group
+        if (b == 0) { gflag[f] = 1; gnode_at[f] = b; }          // the whole system is one group
     } else {
         // the children in order: consecutive small ones are packed greedily into runs of <= gm sinks
         u32 run = 0;
@@ -398,14 +398,15 @@ __global__ void __launch_bounds__(256) gmark_kernel(const DevCtl *__restrict__ c
         for (u32 q = c0; q < c0 + nc; q++) {
             const u32 cq = count[q];
             if (cq > gm) { open = false; run = 0; continue; }
-            if (!open || run + cq > gm) { gflag[first[q]] = 1; run = 0; open = true; }
+            if (!open || run + cq > gm) { gflag[first[q]] = 1; gnode_at[first[q]] = b; run = 0; open = true; }
             run += cq;
         }
     }
 }
 
 __global__ void __launch_bounds__(SC_THREADS) gscan_kernel(const unsigned char *__restrict__ gflag, u32 n, DevCtl *ctl,
-                                                           u64 *sc_status, u32 *__restrict__ gfirst)
+                                                           u64 *sc_status, u32 *__restrict__ gfirst,
+                                                           const u32 *__restrict__ gnode_at, u32 *__restrict__ gnode)
 {
     __shared__ u32 s_warp[SC_THREADS / 32];
     __shared__ u32 s_tile;
@@ -453,7 +454,8 @@ __global__ void __launch_bounds__(SC_THREADS) gscan_kernel(const unsigned char *
         __syncthreads();
         u32 g = (u32)s_prefix + wbase + incl - mysum;
 #pragma unroll
-        for (int k = 0; k < SC_IPT; k++) if (fl[k]) gfirst[g++] = i0 + k;
+        for (int k = 0; k < SC_IPT; k++)
+            if (fl[k]) { gfirst[g] = i0 + k; gnode[g] = gnode_at[i0 + k]; g++; }
     }
 }
 
@@ -490,6 +492,44 @@ __global__ void __launch_bounds__(256) ginfo_kernel(const DevCtl *__restrict__ c
             ghi[g] = make_float4(hi.x, hi.y, hi.z, 0.0f);
         }
     }
+}
+
+// Start node of the hard walk of every group (walk.cu): the lowest ancestor of the group's node whose
+// Morton cell contains the group box grown by r_out (plus a margin far above the fp32 rounding of the
+// T12 distance).  A leaf whose tight box comes within r_out of the group box in the fp32 arithmetic of
+// T12 overlaps the grown box, so its cell meets that ancestor's cell; Morton cells are nested or disjoint,
+// hence the leaf lies below the ancestor (or is it) and a walk that starts there finds the same hard list
+// as a walk from the root.
+__device__ __forceinline__ u32 quantise_d(double x, double o, double inv)
+{
+    const double f = floor((x - o) * inv);
+    return f >= 2097151.0 ? 2097151u : (f > 0.0 ? (u32)f : 0u);
+}
+
+__global__ void __launch_bounds__(256) ganc_kernel(const DevCtl *__restrict__ ctl, const u32 *__restrict__ gnode,
+                                                   const float4 *__restrict__ glo, const float4 *__restrict__ ghi,
+                                                   const unsigned char *__restrict__ level, const u32 *__restrict__ parent,
+                                                   float r_out, u32 *__restrict__ ganc)
+{
+    const u32 ng = ctl->ng;
+    const u32 g = blockIdx.x * blockDim.x + threadIdx.x;
+    if (g >= ng) return;
+    const float4 lo = glo[g], hi = ghi[g];
+    const double inv = ctl->inv;
+    int lstar = MAXLEVEL;
+    const float l3[3] = {lo.x, lo.y, lo.z}, h3[3] = {hi.x, hi.y, hi.z};
+#pragma unroll
+    for (int a = 0; a < 3; a++) {
+        const double o = ctl->origin[a];
+        const double R = (double)r_out * (1.0 + 1.0 / 1024.0) +
+                         (fabs((double)l3[a]) + fabs((double)h3[a]) + (double)r_out) * (1.0 / 1048576.0);
+        const u32 qa = quantise_d((double)l3[a] - R, o, inv), qb = quantise_d((double)h3[a] + R, o, inv);
+        const u32 x = qa ^ qb;
+        lstar = min(lstar, x ? __clz((int)x) - 11 : MAXLEVEL);       // common leading bits of the 21
+    }
+    u32 node = gnode[g];
+    while ((int)level[node] > lstar) node = parent[node];
+    ganc[g] = node;
 }
 
 // ------------------------------------------------------------------ host side
@@ -547,11 +587,16 @@ cudaError_t launch_build_tree(Ctx *c)
     cudaStreamWaitEvent(ax, c->ev_linked, 0);
     unsigned char *gflag = wsptr<unsigned char>(c, L.gflag);
     gmark_kernel<<<(int)((L.node_cap + 255) / 256), 256, 0, ax>>>(ctl, first, count, child, nchild, parent,
-                                                                  c->p.group_max, c->grouping_now, gflag);
+                                                                  c->p.group_max, c->grouping_now, gflag, wsptr<u32>(c, L.cnt_slot));
     u32 *gfirst = wsptr<u32>(c, L.gfirst);
-    gscan_kernel<<<sc_grid, SC_THREADS, 0, ax>>>(gflag, n, ctl, sc_status + L.po_tiles, gfirst);
+    gscan_kernel<<<sc_grid, SC_THREADS, 0, ax>>>(gflag, n, ctl, sc_status + L.po_tiles, gfirst, wsptr<u32>(c, L.cnt_slot),
+                                                 wsptr<u32>(c, L.gnode));
     ginfo_kernel<<<(int)imin64((c->n + 255) / 256, (int64_t)c->num_sms * 8), 256, 0, ax>>>(
         ctl, n, pos_t, gfirst, wsptr<u32>(c, L.gcount), wsptr<float4>(c, L.glo), wsptr<float4>(c, L.ghi));
+    if (c->p.split)
+        ganc_kernel<<<(int)((L.group_cap + 255) / 256), 256, 0, ax>>>(ctl, wsptr<u32>(c, L.gnode), wsptr<float4>(c, L.glo),
+                                                                     wsptr<float4>(c, L.ghi), level, parent, c->p.r_out,
+                                                                     wsptr<u32>(c, L.ganc));
     cudaEventRecord(c->ev_groups, ax);
 
     NodeArrays na;

@@ -30,6 +30,7 @@ struct WalkArgs {
     const float4 *glo, *ghi;
     u32 *ncell, *npart, *nhard;
     const u32 *heavy;             // hard walk: sink ranges of split groups (see split_kernel)
+    const u32 *ganc;              // hard walk: start node of every group (octree.cu, ganc_kernel)
     const unsigned char *is_split; // hard walk: group is handled as ranges
     float4 *a_soft, *a_hard;
     DevCtl *ctl;
@@ -458,7 +459,9 @@ __global__ void __launch_bounds__(WK_WARPS * 32, SmemLayout<MODE>::ctas_per_sm) 
         bool slow = false;                // something other than a plain traversal iteration is pending
         int ex_near = 0;                  // pending expansion: target buffer, this lane's leaf, progress
         u32 ex_first = 0, ex_cnt = 0, ex_off = 0, ex_T = 0, ex_done = 0;
-        if (lane == 0) stack[0] = 0u;     // the root alone: "first child" 0, nchild - 1 = 0
+        // the start node alone ("first child" = the node, nchild - 1 = 0): the root, or for a hard walk
+        // the lowest ancestor that holds every leaf within r_out of the group box
+        if (lane == 0) stack[0] = MODE == WALK_HARD ? __ldg(a.ganc + g) : 0u;
         __syncwarp();
 
         for (;;) {
@@ -766,6 +769,7 @@ cudaError_t launch_walk(Ctx *c, int mode)
     a.kc0 = c->p.r_out / w; a.kc1 = -1.0f / w;
     a.zero64 = 0ull;
     a.heavy = wsptr<u32>(c, L.splitq);
+    a.ganc = wsptr<u32>(c, L.ganc);
     a.is_split = wsptr<unsigned char>(c, L.gflag);      // the build's flag array is free between builds
     cudaMemsetAsync(&c->ctl->group_counter, 0, 2 * sizeof(u32), c->stream);      // counter, nheavy
     if (mode == WALK_HARD)
