@@ -82,7 +82,7 @@ struct Layout {   // byte offsets into the workspace; computed by plan_workspace
     size_t pos_tmp, vel_tmp, id_tmp;
     size_t rs_status;           // [RS_PASSES][rs_tiles + rs_blocks][256] u32 (tile and block look-back statuses)
     size_t sc_status;           // u64 [po_tiles] (preorder scan) then [sc_tiles] (group scan)
-    size_t dlev, cnt_slot;      // int8[n], u32[n]
+    size_t cnt_slot;            // u32[n]: node a group hangs from, by first particle (scratch of the group kernels)
     size_t gflag;               // u8[n]
     size_t pre_level, pre_first, pre_of_bfs, bfs_of_pre;   // u8, u32, u32, u32 [node_cap]
     size_t node_status;         // [ntiles(node_cap)][256] u32

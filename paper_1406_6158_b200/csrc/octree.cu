@@ -7,9 +7,10 @@
 //              derived from a sliding window of leaf_max+1 keys.  A scan gives each node its
 //              preorder index.
 //   bfs      : one stable counting-sort pass by level turns preorder into breadth-first order.
-//   link     : every node finds its range end, children and parent by binary search in the keys.
+//   link     : every node finds its range end, children and parent from the two orders (a leaf ends
+//              where the next preorder node starts; sibling runs are consecutive in breadth-first
+//              order); only a cell's range end needs a binary search in the keys.
 //   upsweep  : leaves first, the last child to arrive computes the parent (fixed summation order).
-#include <stdlib.h>
 #include "common.cuh"
 #include "sort.cuh"
 
@@ -26,8 +27,7 @@ constexpr int PO_HALO = 64;
 
 __global__ void __launch_bounds__(SC_THREADS) preorder_kernel(
     const u64 *__restrict__ key, u32 n, int leaf_max, u32 node_cap, DevCtl *ctl, u64 *sc_status,
-    signed char *__restrict__ dlev, u32 *__restrict__ slot, unsigned char *__restrict__ pre_level,
-    u32 *__restrict__ pre_first)
+    unsigned char *__restrict__ pre_level, u32 *__restrict__ pre_first)
 {
     __shared__ u64 s_key[PO_TILE + 2 * PO_HALO];
     __shared__ signed char s_w[PO_TILE + PO_HALO];
@@ -101,8 +101,6 @@ __global__ void __launch_bounds__(SC_THREADS) preorder_kernel(
         for (int k = 0; k < PO_IPT; k++) {
             const long long i = t0 + tid * PO_IPT + k;
             if (i < (long long)n) {
-                dlev[i] = (signed char)d[k];
-                slot[i] = (u32)min(p, (u64)0xFFFFFFFFu);
                 for (int j = 0; j < cnt[k]; j++) {
                     if (p + j < node_cap) {
                         pre_level[p + j] = (unsigned char)(d[k] + 1 + j);
@@ -145,11 +143,15 @@ __device__ __forceinline__ u32 lower_bound_key(const u64 *__restrict__ key, u32 
     }
     return lo;
 }
+// Topology from the two orders.  In preorder a node is followed by its first child (one level deeper) if
+// it has children, else by the next node that starts where it ends; a node is a FIRST child exactly when
+// its preorder predecessor is one level up (its parent).  In breadth-first order the children of a cell
+// are consecutive, so the first child of a sibling run is at most seven steps back and the run ends at
+// most seven steps ahead: a handful of grouped loads instead of binary searches in the keys.
 __global__ void __launch_bounds__(256) link_kernel(
     const u64 *__restrict__ key, u32 n, int leaf_max, const DevCtl *__restrict__ ctl,
     const unsigned char *__restrict__ level, const u32 *__restrict__ pre_of_bfs, const u32 *__restrict__ bfs_of_pre,
     const unsigned char *__restrict__ pre_level, const u32 *__restrict__ pre_first,
-    const signed char *__restrict__ dlev, const u32 *__restrict__ slot,
     u32 *__restrict__ first, u32 *__restrict__ count, u32 *__restrict__ child, unsigned char *__restrict__ nchild,
     u32 *__restrict__ parent, u32 *__restrict__ arrived, NodeRec *__restrict__ rec, u64 *__restrict__ bmax2)
 {
@@ -158,29 +160,44 @@ __global__ void __launch_bounds__(256) link_kernel(
         const u32 p = pre_of_bfs[b];
         const int lev = level[b];
         const u32 f = pre_first[p];
-        const u64 k0 = __ldg(key + f);
-        const int sh = 63 - 3 * lev;
+        const bool has_kids = p + 1 < nn && (int)pre_level[p + 1] == lev + 1;
         u32 end;
         if (lev == 0) end = n;
-        else end = lower_bound_key(key, f, n, ((k0 >> sh) + 1ull) << sh);
+        else if (!has_kids) end = p + 1 < nn ? pre_first[p + 1] : n;     // the next node starts where this one ends
+        else {
+            const u64 k0 = __ldg(key + f);
+            const int sh = 63 - 3 * lev;
+            end = lower_bound_key(key, f, n, ((k0 >> sh) + 1ull) << sh);
+        }
         const u32 c = end - f;
-        const bool internal = (c > (u32)leaf_max) && lev < MAXLEVEL && (p + 1 < nn);
+        const bool internal = has_kids && (c > (u32)leaf_max) && lev < MAXLEVEL;
         u32 ch = NOCHILD, nc = 0;
         if (internal) {
             ch = bfs_of_pre[p + 1];
-            const int shc = sh - 3;
-            u32 pos = f;
-            while (pos < end) {
-                u64 kk = __ldg(key + pos);
-                pos = lower_bound_key(key, pos, end, ((kk >> shc) + 1ull) << shc);
-                nc++;
-            }
+            const u32 lim = ctl->level_offset[lev + 2];                   // end of the children's level
+            u32 pq[7];
+#pragma unroll
+            for (int i = 0; i < 7; i++) pq[i] = ch + 1 + i < lim ? pre_of_bfs[ch + 1 + i] : 0u;
+            bool fst[7];
+#pragma unroll
+            for (int i = 0; i < 7; i++) fst[i] = ch + 1 + i >= lim || (int)pre_level[pq[i] - 1] == lev;
+            nc = 8;
+#pragma unroll
+            for (int i = 6; i >= 0; i--) if (fst[i]) nc = 1 + i;          // the run ends before the next first child
         }
         u32 par = NOCHILD;
         if (lev > 0) {
-            const int shp = sh + 3;
-            u32 pf = (lev == 1) ? 0u : lower_bound_key(key, 0, f + 1, (k0 >> shp) << shp);
-            u32 pp = slot[pf] + (u32)(lev - 1 - ((int)dlev[pf] + 1));
+            const u32 lo = ctl->level_offset[lev];
+            u32 pb[8];
+            pb[0] = p;
+#pragma unroll
+            for (int i = 1; i < 8; i++) pb[i] = (b >= lo + i) ? pre_of_bfs[b - i] : 1u;
+            bool fst[8];
+#pragma unroll
+            for (int i = 0; i < 8; i++) fst[i] = (b >= lo + i) && (int)pre_level[pb[i] - 1] == lev - 1;
+            u32 pp = pb[0] - 1;
+#pragma unroll
+            for (int i = 7; i >= 0; i--) if (fst[i]) pp = pb[i] - 1;      // nearest first child at or before b
             par = bfs_of_pre[pp];
         }
         first[b] = f; count[b] = c; child[b] = ch; nchild[b] = (unsigned char)nc; parent[b] = par;
@@ -556,12 +573,10 @@ cudaError_t launch_build_tree(Ctx *c)
     const u64 *key = wsptr<u64>(c, L.key_b);
     u64 *sc_status = wsptr<u64>(c, L.sc_status);
     const int sc_grid = (int)imin64(L.sc_tiles, (int64_t)c->num_sms * 8);
-    signed char *dlev = wsptr<signed char>(c, L.dlev);
-    u32 *slot = wsptr<u32>(c, L.cnt_slot);
     unsigned char *pre_level = wsptr<unsigned char>(c, L.pre_level);
     u32 *pre_first = wsptr<u32>(c, L.pre_first);
     const int po_grid = (int)imin64(L.po_tiles, (int64_t)c->num_sms * 8);
-    preorder_kernel<<<po_grid, SC_THREADS, 0, st>>>(key, n, c->p.leaf_max, (u32)L.node_cap, ctl, sc_status, dlev, slot,
+    preorder_kernel<<<po_grid, SC_THREADS, 0, st>>>(key, n, c->p.leaf_max, (u32)L.node_cap, ctl, sc_status,
                                                     pre_level, pre_first);
     level_offset_kernel<<<1, 32, 0, st>>>(ctl);
     unsigned char *level = wsptr<unsigned char>(c, L.level);
@@ -579,7 +594,7 @@ cudaError_t launch_build_tree(Ctx *c)
     u64 *bmax2 = wsptr<u64>(c, L.bmax2);
     const int node_grid = (int)imin64((L.node_cap + 255) / 256, (int64_t)c->num_sms * 16);
     link_kernel<<<node_grid, 256, 0, st>>>(key, n, c->p.leaf_max, ctl, level, pre_of_bfs, bfs_of_pre, pre_level, pre_first,
-                                           dlev, slot, first, count, child, nchild, parent, arrived, rec, bmax2);
+                                           first, count, child, nchild, parent, arrived, rec, bmax2);
     // sink groups need only the topology and the permuted positions: auxiliary stream, next to the upsweep
     cudaStream_t ax = c->aux;
     const float4 *pos_t = wsptr<float4>(c, L.pos_tmp);      // == the re-ordered store (copied back on aux)
