@@ -302,10 +302,11 @@ __global__ void __launch_bounds__(128) upsweep_kernel(NodeArrays na, const float
         if (par == NOCHILD) break;
         const u32 nc = na.nchild[par], c0 = na.child[par];      // topology: requested before the fence
         const int plev = na.level[par];
-        __threadfence();
-        const u32 old = atomicAdd(&na.arrived[par], 1u);
+        // arrival counter with release (this node's record is written) / acquire (the siblings' records
+        // are read next) ordering at device scope
+        u32 old;
+        asm volatile("atom.acq_rel.gpu.global.add.u32 %0, [%1], %2;" : "=r"(old) : "l"(na.arrived + par), "r"(1u) : "memory");
         if (old + 1 != nc) break;
-        __threadfence();
         double M = 0.0, Sx = 0.0, Sy = 0.0, Sz = 0.0;
         float3 lo, hi;
         for (u32 q = c0; q < c0 + nc; q++) {
