@@ -57,6 +57,26 @@ struct SmemLayout {                 // per warp
     static constexpr int ctas_per_sm = MODE == WALK_HARD ? 3 : 2;
 };
 
+// sink layout by group size (1..64): x = S sinks per lane, y = A lanes per copy, z = P copies,
+// w = ceil(32768 / A) for the division of a lane index by A
+__constant__ ushort4 c_layout[65];
+
+static void sink_layout(ushort4 *t)
+{
+    for (int n = 0; n <= 64; n++) {
+        if (n == 0) { t[0] = make_ushort4(2, 1, 1, 32768); continue; }
+        // maximise n P / (32 S) over S in {2,3,4}; ties go to the larger S
+        int S = 2, A = (n + 1) >> 1, P = 32 / A;
+        const int A3 = (n + 2) / 3, P3 = 32 / A3, A4 = (n + 3) >> 2, P4 = 32 / A4;
+        int best = 6 * P;
+        if (4 * P3 >= best) { best = 4 * P3; S = 3; A = A3; P = P3; }
+        if (3 * P4 >= best) { S = 4; A = A4; P = P4; }
+        if (P > 16) P = 16;               // groups of one or two sinks: keeps the padding step P U <= 64
+        t[n] = make_ushort4((unsigned short)S, (unsigned short)A, (unsigned short)P,
+                            (unsigned short)((32768 + A - 1) / A));
+    }
+}
+
 // ---- pair kernels ---------------------------------------------------------------------------
 __device__ __forceinline__ float rsqrt_approx(float x)
 {
@@ -424,18 +444,14 @@ __global__ void __launch_bounds__(WK_WARPS * 32, SmemLayout<MODE>::ctas_per_sm) 
         const u32 gf = a.gfirst[g] + rsub * n_rng;
         const int n = (int)(min(n_all, (rsub + 1u) * n_rng) - rsub * n_rng);
         const float4 glo = a.glo[g], ghi = a.ghi[g];
-        // sinks per lane: maximise n P / (32 S) over S in {2,3,4}; ties go to the larger S
-        int S = 2, A = (n + 1) >> 1, P = 32 / A;
-        {
-            const int A3 = (n + 2) / 3, P3 = 32 / A3, A4 = (n + 3) >> 2, P4 = 32 / A4;
-            int best = 6 * P;
-            if (4 * P3 >= best) { best = 4 * P3; S = 3; A = A3; P = P3; }
-            if (3 * P4 >= best) { S = 4; A = A4; P = P4; }
-        }
-        P = min(P, 16);                   // groups of one or two sinks: keeps the padding step P U <= 64
+        // sinks per lane S in {2,3,4}, lanes per copy A = ceil(n / S), copies P: from the table of
+        // sink_layout() (maximises the busy fraction n P / (32 S)); lane / A by a 15-bit reciprocal
+        const ushort4 lay = c_layout[n];
+        const int S = lay.x, A = lay.y, P = lay.z;
         const int US = S == 2 ? 4 : 2;                                // sources per evaluation iteration (monopoles)
-        const int aidx = lane % A;
-        const int part = (lane / A < P) ? lane / A : 0x40000000;     // idle lanes never enter the loops
+        const int copy = (lane * (int)lay.w) >> 15;                   // = lane / A  (lane < 32, A <= 32)
+        const int aidx = lane - copy * A;
+        const int part = copy < P ? copy : 0x40000000;               // idle lanes never enter the loops
         const float4 dummy = make_float4(glo.x, glo.y, glo.z, 0.0f); // zero-mass padding entry
         Sinks sk;
 #pragma unroll
@@ -745,7 +761,11 @@ static cudaError_t launch_walk_mode(Ctx *c, const WalkArgs &a)
     const size_t smem = SL::bytes * WK_WARPS;
     static bool attr_set = false;
     if (!attr_set) {
-        cudaError_t e = cudaFuncSetAttribute(walk_kernel<MODE, KF>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        ushort4 t[65];
+        sink_layout(t);
+        cudaError_t e = cudaMemcpyToSymbol(c_layout, t, sizeof t);
+        if (e != cudaSuccess) return e;
+        e = cudaFuncSetAttribute(walk_kernel<MODE, KF>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
         attr_set = true;
     }
