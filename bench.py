@@ -98,6 +98,8 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer leg (profiling runs)")
     ap.add_argument("--no-normal", action="store_true", help="skip the normal-tree comparison leg")
+    ap.add_argument("--grouping", type=int, default=None, choices=[0, 1, 2],
+                    help="sink groups: 0 single tree nodes, 1 runs of sibling cells, 2 auto (the configs' default)")
     args = ap.parse_args()
 
     rank = int(os.environ.get("RANK", "0"))
@@ -106,9 +108,11 @@ def main():
 
     from workloads import CONFIGS, make_ic
     cfg = CONFIGS[args.config]
+    if args.grouping is not None:
+        cfg = cfg.with_(grouping=args.grouping)
     config = {"workload": f"{cfg.name}: {cfg.kind} N={cfg.n}, eps={cfg.eps}, theta={cfg.theta}, leaf<={cfg.leaf_max}, "
                           f"group<={cfg.group_max}, r_in={cfg.r_in}, r_out={cfg.r_out}, dt_soft=1/{round(1 / cfg.dt_soft)}, "
-                          f"n_sub={cfg.n_sub}, seed {cfg.seed}",
+                          f"n_sub={cfg.n_sub}, grouping={cfg.grouping}, seed {cfg.seed}",
               "step": "one soft cycle: n_sub tree builds + 1 fused soft/hard walk + (n_sub-1) hard walks + kick/drift",
               "l2": "256 MiB L2 flush between timed steps", "replicas": world}
 

@@ -475,19 +475,21 @@ static float dist2_box_box(const orc_tree *t, int64_t g, int64_t k)
 
 /* T13.  Visits the tree for group g; calls back for accepted cells and opened leaves. */
 typedef struct {
-    uint32_t *cells; int64_t ncells, cap_cells;
+    uint32_t *cells; uint8_t *cellhard; int64_t ncells, cap_cells;
     uint32_t *leaves; uint8_t *leafhard; int64_t nleaves, cap_leaves;
     int64_t npart, nhard;
 } walk_out;
 
-static void push_cell(walk_out *w, uint32_t k)
+static void push_cell(walk_out *w, uint32_t k, int hard)
 {
     if (w->cells) {
         if (w->ncells == w->cap_cells) { w->cap_cells = w->cap_cells ? 2 * w->cap_cells : 1024;
-            w->cells = (uint32_t *)realloc(w->cells, 4 * (size_t)w->cap_cells); }
-        w->cells[w->ncells] = k;
+            w->cells = (uint32_t *)realloc(w->cells, 4 * (size_t)w->cap_cells);
+            w->cellhard = (uint8_t *)realloc(w->cellhard, (size_t)w->cap_cells); }
+        w->cells[w->ncells] = k; w->cellhard[w->ncells] = (uint8_t)hard;
     }
     w->ncells++;
+    if (hard) w->nhard += 1;
 }
 static void push_leaf(walk_out *w, uint32_t k, int hard, uint32_t count)
 {
@@ -510,7 +512,7 @@ static void walk_group(const orc_tree *t, int mode, int64_t g, walk_out *w, int 
     uint32_t *stack = (uint32_t *)malloc(4 * (size_t)scap);
     w->ncells = w->nleaves = w->npart = w->nhard = 0;
     if (keep) {
-        if (!w->cells) { w->cap_cells = 1024; w->cells = (uint32_t *)malloc(4 * 1024); }
+        if (!w->cells) { w->cap_cells = 1024; w->cells = (uint32_t *)malloc(4 * 1024); w->cellhard = (uint8_t *)malloc(1024); }
         if (!w->leaves) { w->cap_leaves = 1024; w->leaves = (uint32_t *)malloc(4 * 1024); w->leafhard = (uint8_t *)malloc(1024); }
     }
     stack[sp++] = 0;
@@ -519,15 +521,20 @@ static void walk_group(const orc_tree *t, int mode, int64_t g, walk_out *w, int 
         float d2b = dist2_box_box(t, g, k);
         int near = d2b < rout2;
         int open;
+        /* hard_tree ("we use the tree algorithm ... for both of soft and hard
+         * forces", "we can cut-off the tree traversal for distant cells"): the hard walk applies the
+         * MAC too and an accepted cell within r_out contributes K(r_COM) F_COM; the soft walk is the
+         * plain MAC walk (no rule (b)) whose cells within r_out carry 1 - K(r_COM). */
+        int tree = t->p.hard_tree && mode != ORC_MODE_NORMAL;
         if (mode == ORC_MODE_HARD) {
             if (!near) continue;                                       /* discarded */
-            open = 1;
+            open = tree ? (dist2_box_com(t, g, k) < t->ropen2[k]) : 1;
         } else {
             float d2a = dist2_box_com(t, g, k);
             int mac_open = d2a < t->ropen2[k];
-            open = (mode == ORC_MODE_NORMAL) ? mac_open : (mac_open || near);
+            open = (mode == ORC_MODE_NORMAL || tree) ? mac_open : (mac_open || near);
         }
-        if (!open) { push_cell(w, k); continue; }
+        if (!open) { push_cell(w, k, tree && near); continue; }
         if (t->child[k] == NOCHILD) {
             int hard = (mode == ORC_MODE_NORMAL) ? 0 : near;
             push_leaf(w, k, hard, t->count[k]);
@@ -578,7 +585,7 @@ int orc_walk_lists(const orc_tree *t, int mode, int64_t g,
             for (uint32_t j = t->first[k]; j < t->first[k] + t->count[k]; j++) { parts[q] = j; hard[q] = w.leafhard[l]; q++; }
         }
     }
-    free(w.cells); free(w.leaves); free(w.leafhard);
+    free(w.cells); free(w.cellhard); free(w.leaves); free(w.leafhard);
     return rc;
 }
 
@@ -619,7 +626,14 @@ void orc_forces(const orc_tree *t, int mode, int64_t ngsel, const int64_t *gsel,
                 double dx[3], s, r2;
                 pair(xi, src, eps2, dx, &s, &r2);
                 double ms = (double)src[3] * s;
-                as[0] += ms * dx[0]; as[1] += ms * dx[1]; as[2] += ms * dx[2];
+                if (w.cellhard[c]) {                                   /* hard_tree: K-weighted cell */
+                    double K = orc_K(sqrt(r2), rin, rout, t->p.kfunc);
+                    double wh = K * ms, ws = (1.0 - K) * ms;
+                    ah[0] += wh * dx[0]; ah[1] += wh * dx[1]; ah[2] += wh * dx[2];
+                    if (mode == ORC_MODE_HYBRID) { as[0] += ws * dx[0]; as[1] += ws * dx[1]; as[2] += ws * dx[2]; }
+                } else {
+                    as[0] += ms * dx[0]; as[1] += ms * dx[1]; as[2] += ms * dx[2];
+                }
             }
             for (int64_t l = 0; l < w.nleaves; l++) {                 /* particles */
                 uint32_t k = w.leaves[l];
@@ -649,7 +663,7 @@ void orc_forces(const orc_tree *t, int mode, int64_t ngsel, const int64_t *gsel,
             if (mode != ORC_MODE_NORMAL && a_hard) for (int a = 0; a < 3; a++) a_hard[3 * (size_t)i + a] = G * ah[a];
             if (mode == ORC_MODE_NORMAL && a_hard) for (int a = 0; a < 3; a++) a_hard[3 * (size_t)i + a] = 0.0;
         }
-        free(w.cells); free(w.leaves); free(w.leafhard);
+        free(w.cells); free(w.cellhard); free(w.leaves); free(w.leafhard);
     }
     if (inter_soft) *inter_soft = isoft;
     if (inter_hard) *inter_hard = ihard;

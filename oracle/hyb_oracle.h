@@ -42,6 +42,7 @@ typedef struct {
     int32_t kfunc;         /* 0 Eq. 10, 1 north_star's 7th-degree polynomial */
     int32_t split;         /* 1 hybrid, 0 normal tree */
     int32_t grouping;      /* T11: 0 sink group = one tree node, 1 = run of consecutive small siblings (R17) */
+    int32_t hard_tree;     /* R20: 0 hard force = direct K-weighted sum, 1 = the paper's MAC-approximated hard walk */
 } orc_params;
 
 enum { ORC_MODE_HYBRID = 0, ORC_MODE_HARD = 1, ORC_MODE_NORMAL = 2 };

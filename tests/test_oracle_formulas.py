@@ -70,7 +70,7 @@ def test_rb_is_root_of_salmon_warren_bound():
 
 def _params(**kw):
     d = dict(G=1.0, eps=0.01, theta=0.5, a_err=2.0 ** -8, r_in=0.01, r_out=0.1, dt_soft=0.01, n_sub=4,
-             leaf_max=8, group_max=32, mac=0, kfunc=0, split=1, grouping=1)
+             leaf_max=8, group_max=32, mac=0, kfunc=0, split=1, grouping=1, hard_tree=0)
     d.update(kw)
     return O.OrcParams(**d)
 

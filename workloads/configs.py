@@ -27,6 +27,8 @@ class Config:
     grouping: int = 2            # sink groups: 1 = runs of consecutive small sibling cells, 0 = single tree nodes,
                                  # 2 = 1, except 0 for the trees of hyb_step that only a hard walk uses
 
+    hard_tree: int = 0           # 0 = hard force by direct K-weighted sum (R20), 1 = the paper's MAC-approximated hard walk
+
     def with_(self, **kw) -> "Config":
         return replace(self, **kw)
 
