@@ -68,6 +68,7 @@ static bool params_ok(const hyb_params *p, int64_t n, char *msg)
     if (p->mac == HYB_MAC_ABS && !(p->a_err > 0.0f && isfinite(p->a_err))) return bad("a_err must be finite and > 0");
     if (p->kfunc != HYB_K_PAPER && p->kfunc != HYB_K_POLY7) return bad("unknown kfunc");
     if (p->split != 0 && p->split != 1) return bad("split must be 0 or 1");
+    if (p->hard_tree != 0 && p->hard_tree != 1) return bad("hard_tree must be 0 or 1");
     if (p->grouping != HYB_GROUP_NODE && p->grouping != HYB_GROUP_SIBLINGS && p->grouping != HYB_GROUP_AUTO) return bad("unknown grouping");
     if (p->split == 1 && !(p->r_in >= 0.0f && p->r_out > p->r_in && isfinite(p->r_out))) return bad("need 0 <= r_in < r_out");
     return true;
@@ -99,7 +100,7 @@ static int do_build(Ctx *c, bool hard_only = false)
 {
     // HYB_GROUP_AUTO: fuller groups for the soft walk, single nodes when only a hard walk follows
     c->grouping_now = c->p.grouping == HYB_GROUP_AUTO ? (hard_only ? HYB_GROUP_NODE : HYB_GROUP_SIBLINGS) : c->p.grouping;
-    c->boxes_only = hard_only;
+    c->boxes_only = hard_only && !c->p.hard_tree;      // the tree-approximated hard walk needs the moments
     cudaError_t e = launch_build_tree(c);
     if (e != cudaSuccess) return cuda_fail(c, e, "build_tree");
     c->tree_valid = true;

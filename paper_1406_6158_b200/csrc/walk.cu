@@ -388,7 +388,11 @@ __device__ __forceinline__ u32 warp_excl_scan(u32 v, int lane, u32 &total)
     return incl - v;
 }
 
-template <int MODE, int KF>
+// TREE (hyb_params.hard_tree): the paper-literal hard force.  The MAC is applied in the hard walk too and a
+// cell accepted within r_out of the group box is evaluated like a particle at its centre of mass with
+// the K weights (hard K, soft 1 - K); the soft walk drops rule (b).  TREE = false: every node within
+// r_out is opened, i.e. the hard force is the direct K-weighted sum (R20).
+template <int MODE, int KF, bool TREE>
 __global__ void __launch_bounds__(WK_WARPS * 32, SmemLayout<MODE>::ctas_per_sm) walk_kernel(const WalkArgs a)
 {
     using SL = SmemLayout<MODE>;
@@ -477,7 +481,8 @@ __global__ void __launch_bounds__(WK_WARPS * 32, SmemLayout<MODE>::ctas_per_sm) 
         u32 ex_first = 0, ex_cnt = 0, ex_off = 0, ex_T = 0, ex_done = 0;
         // the start node alone ("first child" = the node, nchild - 1 = 0): the root, or for a hard walk
         // the lowest ancestor that holds every leaf within r_out of the group box
-        if (lane == 0) stack[0] = MODE == WALK_HARD ? __ldg(a.ganc + g) : 0u;
+        // (TREE: from the root -- a cell above that ancestor may be accepted by the MAC)
+        if (lane == 0) stack[0] = (MODE == WALK_HARD && !TREE) ? __ldg(a.ganc + g) : 0u;
         __syncwarp();
 
         for (;;) {
@@ -537,6 +542,7 @@ __global__ void __launch_bounds__(WK_WARPS * 32, SmemLayout<MODE>::ctas_per_sm) 
                     }
                 }
                 if (HAS_MONO && ncb > SL::cell_cap - 64) { flush_mono = true; continue; }
+                if (TREE && HAS_NEAR && npb > SL::part_cap - 64) { flush_near = true; continue; }
                 if (trav_done) {
                     if (HAS_MONO && ncb > 0) { flush_mono = true; continue; }
                     if (HAS_NEAR && npb > 0) { flush_near = true; continue; }
@@ -560,16 +566,16 @@ __global__ void __launch_bounds__(WK_WARPS * 32, SmemLayout<MODE>::ctas_per_sm) 
                     if (have[h]) {
                         const NodeRec *r = a.nodes + ((d & DESC_MASK) + (u32)sub);
                         nB[h] = __ldg(&r->B); nC[h] = __ldg(&r->C); mt[h] = __ldg(&r->meta);
-                        if (MODE != WALK_HARD) nA[h] = __ldg(&r->A);
+                        if (MODE != WALK_HARD || TREE) nA[h] = __ldg(&r->A);
                     }
                 }
             }
             sp -= npop;
             __syncwarp();
-            bool accept[2], open_int[2], leaf_far[2], leaf_near[2];
+            bool accept[2], accept_near[2], open_int[2], leaf_far[2], leaf_near[2];
 #pragma unroll
             for (int h = 0; h < 2; h++) {
-                accept[h] = open_int[h] = leaf_far[h] = leaf_near[h] = false;
+                accept[h] = accept_near[h] = open_int[h] = leaf_far[h] = leaf_near[h] = false;
                 if (have[h]) {
                     // T12: box-box distance (rule (b)), fp32, one rounding per operation
                     float fx = fmaxf(0.0f, fmaxf(__fsub_rn(nB[h].x, ghi.x), __fsub_rn(glo.x, nC[h].x)));
@@ -577,18 +583,20 @@ __global__ void __launch_bounds__(WK_WARPS * 32, SmemLayout<MODE>::ctas_per_sm) 
                     float fz = fmaxf(0.0f, fmaxf(__fsub_rn(nB[h].z, ghi.z), __fsub_rn(glo.z, nC[h].z)));
                     float d2b = __fadd_rn(__fadd_rn(__fmul_rn(fx, fx), __fmul_rn(fy, fy)), __fmul_rn(fz, fz));
                     const bool near = d2b < rout2;
-                    bool open;
-                    if (MODE == WALK_HARD) open = near;
-                    else {
+                    bool open, mac_open = true;
+                    if (MODE != WALK_HARD || TREE) {
                         float ex = fmaxf(0.0f, fmaxf(__fsub_rn(glo.x, nA[h].x), __fsub_rn(nA[h].x, ghi.x)));
                         float ey = fmaxf(0.0f, fmaxf(__fsub_rn(glo.y, nA[h].y), __fsub_rn(nA[h].y, ghi.y)));
                         float ez = fmaxf(0.0f, fmaxf(__fsub_rn(glo.z, nA[h].z), __fsub_rn(nA[h].z, ghi.z)));
                         float d2a = __fadd_rn(__fadd_rn(__fmul_rn(ex, ex), __fmul_rn(ey, ey)), __fmul_rn(ez, ez));
-                        const bool mac_open = d2a < nB[h].w;
-                        open = (MODE == WALK_NORMAL) ? mac_open : (mac_open || near);
+                        mac_open = d2a < nB[h].w;
                     }
+                    if (MODE == WALK_HARD) open = near && mac_open;            // (!near: discarded)
+                    else open = (MODE == WALK_NORMAL || TREE) ? mac_open : (mac_open || near);
                     const bool is_leaf = (mt[h].y & 0x80000000u) != 0;
-                    accept[h] = !open && MODE != WALK_HARD;
+                    const bool acc = !open && (MODE != WALK_HARD || (TREE && near));
+                    accept_near[h] = TREE && acc && near && MODE != WALK_NORMAL;
+                    accept[h] = acc && !accept_near[h];
                     open_int[h] = open && !is_leaf;
                     leaf_near[h] = open && is_leaf && near && MODE != WALK_NORMAL;
                     leaf_far[h] = open && is_leaf && !leaf_near[h];
@@ -612,6 +620,16 @@ __global__ void __launch_bounds__(WK_WARPS * 32, SmemLayout<MODE>::ctas_per_sm) 
                     if (accept[h]) cellbuf[ncb + __popc(bal & lt_mask)] = nA[h];
                     ncb += __popc(bal);
                     ncell += __popc(bal);
+                }
+            }
+            // TREE: cells accepted within r_out -> K-weighted buffer (counted as cells and as hard-list entries)
+            if (TREE && HAS_NEAR) {
+#pragma unroll
+                for (int h = 0; h < 2; h++) {
+                    const u32 bal = __ballot_sync(FULL, accept_near[h]);
+                    if (accept_near[h]) partbuf[npb + __popc(bal & lt_mask)] = nA[h];
+                    npb += __popc(bal);
+                    ncell += __popc(bal); nhard += __popc(bal);
                 }
             }
             // opened leaves -> queues
@@ -642,7 +660,8 @@ __global__ void __launch_bounds__(WK_WARPS * 32, SmemLayout<MODE>::ctas_per_sm) 
             }
             __syncwarp();
             trav_done = sp == 0;
-            slow = trav_done || nlq0 >= 32 || nlq1 >= 32 || (HAS_MONO && ncb > SL::cell_cap - 64);
+            slow = trav_done || nlq0 >= 32 || nlq1 >= 32 || (HAS_MONO && ncb > SL::cell_cap - 64) ||
+                   (TREE && HAS_NEAR && npb > SL::part_cap - 64);
         }
         __syncwarp();
         if (overflow && lane == 0) atomicOr(&a.ctl->status, ST_STACK_OVERFLOW);
@@ -754,7 +773,7 @@ cudaError_t launch_zero_acc(Ctx *c, hyb_float4 *a)
     return cudaGetLastError();
 }
 
-template <int MODE, int KF>
+template <int MODE, int KF, bool TREE>
 static cudaError_t launch_walk_mode(Ctx *c, const WalkArgs &a)
 {
     using SL = SmemLayout<MODE>;
@@ -765,11 +784,11 @@ static cudaError_t launch_walk_mode(Ctx *c, const WalkArgs &a)
         sink_layout(t);
         cudaError_t e = cudaMemcpyToSymbol(c_layout, t, sizeof t);
         if (e != cudaSuccess) return e;
-        e = cudaFuncSetAttribute(walk_kernel<MODE, KF>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        e = cudaFuncSetAttribute(walk_kernel<MODE, KF, TREE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
         attr_set = true;
     }
-    walk_kernel<MODE, KF><<<c->num_sms * SL::ctas_per_sm, WK_WARPS * 32, smem, c->stream>>>(a);
+    walk_kernel<MODE, KF, TREE><<<c->num_sms * SL::ctas_per_sm, WK_WARPS * 32, smem, c->stream>>>(a);
     return cudaGetLastError();
 }
 
@@ -796,10 +815,14 @@ cudaError_t launch_walk(Ctx *c, int mode)
         split_kernel<<<(int)imin64((c->n + 255) / 256, (int64_t)c->num_sms * 4), 256, 0, c->stream>>>(
             c->ctl, a.gcount, a.nhard, wsptr<u32>(c, L.splitq), wsptr<unsigned char>(c, L.gflag),
             WK_SPLIT2, WK_SPLIT4);
-    const bool poly7 = c->p.kfunc == HYB_K_POLY7;
-    if (mode == WALK_HYBRID) return poly7 ? launch_walk_mode<WALK_HYBRID, HYB_K_POLY7>(c, a) : launch_walk_mode<WALK_HYBRID, HYB_K_PAPER>(c, a);
-    if (mode == WALK_HARD) return poly7 ? launch_walk_mode<WALK_HARD, HYB_K_POLY7>(c, a) : launch_walk_mode<WALK_HARD, HYB_K_PAPER>(c, a);
-    return launch_walk_mode<WALK_NORMAL, HYB_K_PAPER>(c, a);
+    const bool poly7 = c->p.kfunc == HYB_K_POLY7, tree = c->p.hard_tree != 0;
+    if (mode == WALK_NORMAL) return launch_walk_mode<WALK_NORMAL, HYB_K_PAPER, false>(c, a);
+    if (mode == WALK_HYBRID) {
+        if (tree) return poly7 ? launch_walk_mode<WALK_HYBRID, HYB_K_POLY7, true>(c, a) : launch_walk_mode<WALK_HYBRID, HYB_K_PAPER, true>(c, a);
+        return poly7 ? launch_walk_mode<WALK_HYBRID, HYB_K_POLY7, false>(c, a) : launch_walk_mode<WALK_HYBRID, HYB_K_PAPER, false>(c, a);
+    }
+    if (tree) return poly7 ? launch_walk_mode<WALK_HARD, HYB_K_POLY7, true>(c, a) : launch_walk_mode<WALK_HARD, HYB_K_PAPER, true>(c, a);
+    return poly7 ? launch_walk_mode<WALK_HARD, HYB_K_POLY7, false>(c, a) : launch_walk_mode<WALK_HARD, HYB_K_PAPER, false>(c, a);
 }
 
 }  // namespace hyb

@@ -60,6 +60,18 @@ def test_cfg2_single_node_groups():
     h.close()
 
 
+def test_cfg2_paper_literal_hard_walk():
+    """hard_tree = 1 at the benchmark size: lists in full, accelerations on a sample of groups"""
+    cfg = CONFIGS[2]
+    pos, vel = make_ic(cfg.kind, cfg.n, cfg.seed)
+    h = make_hyb(cfg, pos, vel, hard_tree=1)
+    h.build_tree(); h.sync()
+    t = O.Tree(pos, O.params_from(cfg, hard_tree=1))
+    compare_tree(h, t)
+    print(check_forces(h, t, gsel=_sample_groups(t.ng, 4096, 9)))
+    h.close()
+
+
 def test_cfg2_normal_tree():
     cfg = CONFIGS[2]
     pos, vel = make_ic(cfg.kind, cfg.n, cfg.seed)

@@ -149,3 +149,18 @@ def test_error_paths_on_device():
     rc = lib().hyb_init(C.byref(hnd), C.byref(P), cfg.n, dpos.data_ptr() + 4, dvel.data_ptr(), acc.data_ptr(), acc.data_ptr(),
                         ids.data_ptr(), ws.data_ptr(), need, 0, None)
     assert rc == -1 and not hnd.value
+
+
+@pytest.mark.parametrize("kfunc", [0, 1])
+def test_paper_literal_hard_walk(kfunc):
+    """hard_tree = 1: MAC-approximated hard force, K-weighted cells"""
+    for cfg, seed in ((CONFIGS[0].with_(r_out=0.25, r_in=0.02, theta=0.6), 0), (CONFIGS[1].with_(n=40013, r_out=0.15), 9),
+                      (CONFIGS[0].with_(n=777, theta=0.0), 3)):
+        pos, vel = make_ic(cfg.kind, cfg.n, seed)
+        print(_run_case(cfg, pos, vel, hard_tree=1, kfunc=kfunc))
+    cfg = CONFIGS[0].with_(hard_tree=1, r_out=0.2)
+    pos, vel = make_ic(cfg.kind, cfg.n, 5)
+    h = make_hyb(cfg, pos, vel)
+    h.step(2); h.sync()
+    assert np.all(np.isfinite(h.pos_m.cpu().numpy()))
+    h.close()
