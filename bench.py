@@ -98,6 +98,10 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer leg (profiling runs)")
     ap.add_argument("--no-normal", action="store_true", help="skip the normal-tree comparison leg")
+    ap.add_argument("--paper-n", type=int, default=None,
+                    help="instead of --config: the paper's own recipe (PAPER.md:172-174) for a Plummer model of N particles")
+    ap.add_argument("--hard-tree", type=int, default=None, choices=[0, 1],
+                    help="1: the paper's MAC-approximated hard walk instead of the direct hard sum (DESIGN.md R20)")
     ap.add_argument("--grouping", type=int, default=None, choices=[0, 1, 2],
                     help="sink groups: 0 single tree nodes, 1 runs of sibling cells, 2 auto (the configs' default)")
     args = ap.parse_args()
@@ -108,11 +112,16 @@ def main():
 
     from workloads import CONFIGS, make_ic
     cfg = CONFIGS[args.config]
+    if args.paper_n is not None:
+        from workloads import paper_params
+        cfg = paper_params(args.paper_n, seed=7)
     if args.grouping is not None:
         cfg = cfg.with_(grouping=args.grouping)
+    if args.hard_tree is not None:
+        cfg = cfg.with_(hard_tree=args.hard_tree)
     config = {"workload": f"{cfg.name}: {cfg.kind} N={cfg.n}, eps={cfg.eps}, theta={cfg.theta}, leaf<={cfg.leaf_max}, "
                           f"group<={cfg.group_max}, r_in={cfg.r_in}, r_out={cfg.r_out}, dt_soft=1/{round(1 / cfg.dt_soft)}, "
-                          f"n_sub={cfg.n_sub}, grouping={cfg.grouping}, seed {cfg.seed}",
+                          f"n_sub={cfg.n_sub}, grouping={cfg.grouping}, hard_tree={cfg.hard_tree}, seed {cfg.seed}",
               "step": "one soft cycle: n_sub tree builds + 1 fused soft/hard walk + (n_sub-1) hard walks + kick/drift",
               "l2": "256 MiB L2 flush between timed steps", "replicas": world}
 
