@@ -37,7 +37,7 @@ Layout plan_workspace(int64_t n)
     L.pos_tmp = take(16 * N); L.vel_tmp = take(16 * N); L.id_tmp = take(4 * N);
     L.rs_status = take(4 * 256 * (size_t)(L.rs_tiles + L.rs_blocks) * RS_PASSES);
     L.sc_status = take(8 * (size_t)(L.sc_tiles + L.po_tiles));
-    L.cnt_slot = take(4 * N); L.gflag = take(N);
+    L.gnode_at = take(4 * N); L.gflag = take(N);
     L.pre_level = take(NC); L.pre_first = take(4 * NC); L.pre_of_bfs = take(4 * NC); L.bfs_of_pre = take(4 * NC);
     L.node_status = take(4 * 256 * (size_t)(L.node_tiles + L.node_blocks));
     L.level = take(NC); L.first = take(4 * NC); L.count = take(4 * NC); L.child = take(4 * NC);

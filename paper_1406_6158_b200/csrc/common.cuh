@@ -82,7 +82,7 @@ struct Layout {   // byte offsets into the workspace; computed by plan_workspace
     size_t pos_tmp, vel_tmp, id_tmp;
     size_t rs_status;           // [RS_PASSES][rs_tiles + rs_blocks][256] u32 (tile and block look-back statuses)
     size_t sc_status;           // u64 [po_tiles] (preorder scan) then [sc_tiles] (group scan)
-    size_t cnt_slot;            // u32[n]: node a group hangs from, by first particle (scratch of the group kernels)
+    size_t gnode_at;            // u32[n]: node a group hangs from, by first particle (scratch of the group kernels)
     size_t gflag;               // u8[n]
     size_t pre_level, pre_first, pre_of_bfs, bfs_of_pre;   // u8, u32, u32, u32 [node_cap]
     size_t node_status;         // [ntiles(node_cap)][256] u32
@@ -156,40 +156,10 @@ __device__ __forceinline__ u64 ld_volatile_u64(const u64 *p)
 }
 
 // Decoupled look-back over one value per tile (status word: bits 63..62 flag, low 62 bits value).
-// Called by ONE thread of the CTA that owns `tile`; returns the exclusive prefix of earlier tiles.
 constexpr u64 LB_AGG = 1ull << 62, LB_PREFIX = 2ull << 62, LB_MASK = (1ull << 62) - 1;
 constexpr int LB_SPIN_LIMIT = 1 << 22;
-__device__ __forceinline__ u64 lookback_single(u64 *status, u32 tile, u64 aggregate, u32 *dev_status)
-{
-    volatile u64 *st = status;
-    if (tile == 0) { st[0] = LB_PREFIX | aggregate; return 0; }
-    st[tile] = LB_AGG | aggregate;
-    u64 excl = 0;
-    long long t = (long long)tile - 1;
-    int spins = 0;
-    bool done = false;
-    constexpr int WIN = 16;          // predecessors requested together (divides the round trips)
-    while (!done) {
-        u64 s[WIN];
-#pragma unroll
-        for (int i = 0; i < WIN; i++) s[i] = (t - i >= 0) ? st[t - i] : (2ull << 62);
-#pragma unroll
-        for (int i = 0; i < WIN; i++) {
-            if (done) break;
-            const u64 f = s[i] >> 62;
-            if (f == 0) break;               // not published yet: poll again from here
-            excl += s[i] & LB_MASK;
-            t--;
-            if (f == 2) done = true;
-        }
-        if (!done && ++spins >= LB_SPIN_LIMIT) { atomicOr(dev_status, ST_WAIT_EXPIRED); break; }
-    }
-    st[tile] = LB_PREFIX | (excl + aggregate);
-    return excl;
-}
-
-// The same with the 32 lanes of one warp each inspecting a different predecessor.  Called by all lanes
-// of ONE warp of the CTA that owns `tile`; every lane returns the exclusive prefix.
+// The 32 lanes of one warp each inspect a different predecessor.  Called by all lanes of ONE warp of the
+// CTA that owns `tile`; every lane returns the exclusive prefix of the earlier tiles.
 __device__ __forceinline__ u64 lookback_warp(u64 *status, u32 tile, u64 aggregate, u32 *dev_status, int lane)
 {
     volatile u64 *st = status;
