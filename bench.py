@@ -226,6 +226,24 @@ def main():
                               "tflops": FLOP_KHARD * (inter[1] - fused_hard) / max(stage[2] * 1e-3, 1e-12) / 1e12,
                               "frac": FLOP_KHARD * (inter[1] - fused_hard) / max(stage[2] * 1e-3, 1e-12) / 1e12 / peak}}
     stages = {"build_ms": stage[0] / K, "soft_ms": soft_ms, "hard_ms": stage[2] / K, "integrate_ms": stage[3] / K}
+    # ---- HBM-bound stages: algorithmic bytes over the measured time, against the measured copy peak
+    peaks_path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    hbm_peak, hbm_src = 6650.0, "fallback 6.65 TB/s (B200_PROFILING.md)"
+    if os.path.exists(peaks_path):
+        hbm_peak, hbm_src = float(json.load(open(peaks_path))["hbm_gbs"]), "MEASURED_PEAKS.json hbm_gbs"
+    nodes_per_particle = 0.4
+    build_bytes = {"bbox": 16, "keys": 16 + 12, "radix_sort": 8 * (12 + 12), "permute": 4 + 36 + 36,
+                   "octree": 16 + nodes_per_particle * 24, "upsweep": 16 + nodes_per_particle * (64 + 56), "groups": 8}
+    bpp_build = sum(build_bytes.values())
+    bpp_integrate = (96 + (cfg.n_sub - 1) * 80 + 64) if cfg.split else cfg.n_sub * (64 + 64)
+    gbs_build = bpp_build * cfg.n * cfg.n_sub / (stages["build_ms"] * 1e-3) / 1e9
+    gbs_int = bpp_integrate * cfg.n / (stages["integrate_ms"] * 1e-3) / 1e9
+    hbm_stages = {"peak_gbs": hbm_peak, "peak_source": hbm_src,
+                  "build": {"bytes_per_particle": bpp_build, "by_stage": build_bytes, "achieved_gbs": gbs_build,
+                            "frac": gbs_build / hbm_peak, "radix_sort_share_of_bytes": build_bytes["radix_sort"] / bpp_build},
+                  "integrate": {"bytes_per_particle_per_cycle": bpp_integrate, "achieved_gbs": gbs_int, "frac": gbs_int / hbm_peak},
+                  "note": "N = 2^20 fits the 126 MB L2 and these stages are latency-bound (about 30 dependent kernels per "
+                          "build), so the achieved figure is far below the copy peak; see profiles/r01_profile.md"}
 
     # ---- end to end through the C-ABI with HOST buffers (pinned), copies inside the timed region
     e2e = None
@@ -288,7 +306,7 @@ def main():
             "warmup": args.warmup, "ms_per_step": total_ms / K, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f32", "data": "synthetic", "config": config, "stages": stages,
             "interactions_per_step": {"soft": inter[0] / K, "hard": inter[1] / K},
-            "roofline": roofline, "normal_tree": normal, "cpu_baseline": cpu_baseline, "e2e": e2e,
+            "roofline": roofline, "hbm_stages": hbm_stages, "normal_tree": normal, "cpu_baseline": cpu_baseline, "e2e": e2e,
             "gpu_launches": launches,
             "clocks": {"sm_mhz": sm_mhz, "sm_max_mhz": sm_max, "reasons": sorted(clk["reasons"]),
                        "samples": len(sm), **({"error": clk["error"]} if "error" in clk else {})}}))
