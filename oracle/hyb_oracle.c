@@ -589,6 +589,71 @@ int orc_walk_lists(const orc_tree *t, int mode, int64_t g,
     return rc;
 }
 
+/* ------------------------------------------------------------------ virtual-domain LET counts */
+/* SURVEY.md 8(f) rank 3.  The box is cut into P cuboid domains (the caller's
+ * boxes, half-open [lo, hi) per axis).  For domain j the tree is walked as process j's neighbours
+ * would walk their local trees to fill j's locally essential tree: a node wholly inside D_j is local;
+ * otherwise it is opened when r_ib < r_b (Eq. 14; r_ib = distance from its centre of mass to D_j, r_b
+ * the opening radius of T10) or when part of it lies inside D_j, else it is sent as ONE cell; an
+ * opened leaf sends its particles that lie outside D_j.  N_soft counts what is sent.  The hard LET
+ * (Eq. 15) follows the same walk but drops every node with r_ib >= R_2 + b_max and every particle
+ * farther than R_2 from D_j; N_hard counts what is left.  Decisions in fp32, one rounding per
+ * operation, like T12.  out[3 j .. 3 j + 2] = N_local, N_soft, N_hard. */
+void orc_let_count(const orc_tree *t, int64_t ndom, const float *boxes, uint64_t *out)
+{
+    float R2 = t->p.r_out, R22 = R2 * R2;
+#pragma omp parallel for schedule(dynamic, 1)
+    for (int64_t j = 0; j < ndom; j++) {
+        const float *lo = boxes + 6 * j, *hi = lo + 3;
+        uint64_t nloc = 0, nsoft = 0, nhard = 0;
+        int64_t scap = 1024, sp = 0;
+        uint32_t *stack = (uint32_t *)malloc(4 * (size_t)scap);
+        stack[sp++] = 0u | 0x80000000u;                            /* bit 31: still on the hard walk */
+        while (sp > 0) {
+            uint32_t ent = stack[--sp], k = ent & 0x7FFFFFFFu;
+            int alive = (ent >> 31) != 0;
+            int inside = 1, touches = 1;
+            float e[3];
+            for (int a = 0; a < 3; a++) {
+                float nl = t->nlo[3 * (size_t)k + a], nh = t->nhi[3 * (size_t)k + a], c = t->com_m[4 * (size_t)k + a];
+                inside = inside && nl >= lo[a] && nh < hi[a];
+                touches = touches && nh >= lo[a] && nl < hi[a];
+                float u = lo[a] - c, w = c - hi[a];
+                e[a] = fmax0(u, w);
+            }
+            if (inside) { nloc += t->count[k]; continue; }
+            float xx = e[0] * e[0], yy = e[1] * e[1], zz = e[2] * e[2];
+            float s2 = xx + yy, r2 = s2 + zz;
+            float cut = R2 + (float)t->bmax[k], cut2 = cut * cut;
+            int hard = alive && r2 < cut2;                         /* Eq. 15 */
+            int open = r2 < t->ropen2[k] || touches;               /* Eq. 14 */
+            if (!open) { nsoft++; nhard += (uint64_t)hard; continue; }
+            if (t->child[k] == NOCHILD) {
+                for (uint32_t q = t->first[k]; q < t->first[k] + t->count[k]; q++) {
+                    const float *x = t->pos_s + 4 * (size_t)q;
+                    int in = 1; float d[3];
+                    for (int a = 0; a < 3; a++) {
+                        in = in && x[a] >= lo[a] && x[a] < hi[a];
+                        float u = lo[a] - x[a], w = x[a] - hi[a];
+                        d[a] = fmax0(u, w);
+                    }
+                    if (in) { nloc++; continue; }
+                    float px = d[0] * d[0], py = d[1] * d[1], pz = d[2] * d[2];
+                    float ps = px + py, d2 = ps + pz;
+                    nsoft++;
+                    if (hard && d2 < R22) nhard++;
+                }
+                continue;
+            }
+            if (sp + 8 > scap) { scap *= 2; stack = (uint32_t *)realloc(stack, 4 * (size_t)scap); }
+            for (int q = (int)t->nchild[k] - 1; q >= 0; q--)
+                stack[sp++] = (t->child[k] + (uint32_t)q) | (hard ? 0x80000000u : 0u);
+        }
+        free(stack);
+        out[3 * j] = nloc; out[3 * j + 1] = nsoft; out[3 * j + 2] = nhard;
+    }
+}
+
 /* ------------------------------------------------------------------ T14 forces */
 /* PAPER.md:35 Eq. 2 (R2: m_j is the source mass); Eq. 7-9 (R3) split by K; "we get
  * the force of a sink particle by summing forces from source cells and particles".  Cells are

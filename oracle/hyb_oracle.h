@@ -102,6 +102,11 @@ int orc_walk_lists(const orc_tree *t, int mode, int64_t g,
                    uint32_t *cells, int64_t cap_cells, int64_t *ncells,
                    uint32_t *parts, uint8_t *hard, int64_t cap_parts, int64_t *nparts);
 
+/* Virtual-domain LET counts (Eq. 14-15): boxes = ndom x
+ * (lo xyz, hi xyz) floats, half-open; needs a tree built with mac = 1 (r_b and b_max per node).
+ * out[3 j ..] = N_local, N_soft, N_hard of domain j. */
+void orc_let_count(const orc_tree *t, int64_t ndom, const float *boxes, uint64_t *out);
+
 /* T14: accelerations in SORTED order, double[3n] each.  If ngsel > 0 only the groups in gsel
  * are evaluated (other entries untouched).  interactions (optional) receives
  * sum over evaluated groups of members x (ncell + npart) resp. members x nhard. */

@@ -52,6 +52,7 @@ def lib():
         L.orc_tree_get.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_int64]
         L.orc_walk_counts.argtypes = [C.c_void_p, C.c_int] + [C.c_void_p] * 3
         L.orc_walk_counts_sel.argtypes = [C.c_void_p, C.c_int, C.c_int64] + [C.c_void_p] * 4
+        L.orc_let_count.argtypes = [C.c_void_p, C.c_int64, C.c_void_p, C.c_void_p]
         L.orc_walk_lists.restype = C.c_int
         L.orc_walk_lists.argtypes = [C.c_void_p, C.c_int, C.c_int64, C.c_void_p, C.c_int64, C.c_void_p,
                                      C.c_void_p, C.c_void_p, C.c_int64, C.c_void_p]
@@ -143,6 +144,13 @@ class Tree:
                                   C.byref(npart))
         assert rc == 0
         return cells[:ncell.value].copy(), parts[:npart.value].copy(), hard[:npart.value].astype(bool)
+
+    def let_count(self, boxes: np.ndarray) -> np.ndarray:
+        """boxes float32 [P,6] (lo xyz, hi xyz) -> uint64 [P,3] = N_local, N_soft, N_hard per domain"""
+        boxes = np.ascontiguousarray(boxes, dtype=np.float32)
+        out = np.zeros((boxes.shape[0], 3), np.uint64)
+        lib().orc_let_count(self._h, boxes.shape[0], _p(boxes), _p(out))
+        return out
 
     def forces(self, mode: int, gsel=None):
         """-> a_soft, a_hard float64 [n,3] in SORTED order, interactions (soft, hard)."""
