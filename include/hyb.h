@@ -178,6 +178,17 @@ int hyb_run_host(const hyb_params *params, int64_t n, hyb_float4 *h_pos_m, hyb_f
                  hyb_float4 *h_a_soft, hyb_float4 *h_a_hard, uint32_t *h_id, int32_t n_soft_steps,
                  int device, uint64_t *h_interactions);
 
+/* Virtual-domain LET counts (Eq. 14-15; Fig. 4: N_soft, N_hard).  The paper's processes
+ * exchange locally essential trees; on one GPU nothing is exchanged, but for any set of ndom virtual
+ * domains (h_boxes: HOST float[6 ndom] = lo xyz, hi xyz, half-open, +-INFINITY allowed) the size of what
+ * domain j would have to receive can be counted from the tree: a node wholly inside the domain is local;
+ * otherwise it is sent as one cell unless r_ib < r_b (Eq. 14) or part of it is inside, in which case it
+ * is opened (an opened leaf sends its particles outside the domain); the hard LET drops nodes with
+ * r_ib >= R_2 + b_max (Eq. 15) and particles farther than R_2.  h_counts: HOST uint64[3 ndom] =
+ * N_local, N_soft, N_hard per domain.  Needs a valid tree built with HYB_MAC_ABS; synchronises.
+ * Errors: INVALID_ARG (theta-MAC tree, empty box), NO_TREE, CAPACITY_OVERFLOW (traversal stack). */
+int hyb_let_count(hyb_ctx *ctx, int32_t ndom, const float *h_boxes, uint64_t *h_counts);
+
 /* Message for the last error on this context ("" if none).  ctx may be NULL (returns the
  * message of the last failed hyb_init / hyb_run_host on this thread). */
 const char *hyb_last_error(const hyb_ctx *ctx);

@@ -76,6 +76,8 @@ def lib():
         L.hyb_export.argtypes = [vp, C.c_int32, vp, C.c_size_t, C.POINTER(C.c_size_t)]
         L.hyb_run_host.restype = C.c_int
         L.hyb_run_host.argtypes = [C.POINTER(HybParams), C.c_int64, vp, vp, vp, vp, vp, C.c_int32, C.c_int, vp]
+        L.hyb_let_count.restype = C.c_int
+        L.hyb_let_count.argtypes = [vp, C.c_int32, vp, vp]
         L.hyb_last_error.restype = C.c_char_p
         L.hyb_last_error.argtypes = [vp]
         L.hyb_free.restype = None
@@ -151,6 +153,13 @@ class Hyb:
 
     def step(self, n_soft_steps: int = 1):
         self._check(lib().hyb_step(self._h, n_soft_steps))
+
+    def let_count(self, boxes: np.ndarray) -> np.ndarray:
+        """boxes float32 [P,6] (lo xyz, hi xyz) -> uint64 [P,3] = N_local, N_soft, N_hard per virtual domain"""
+        boxes = np.ascontiguousarray(boxes, dtype=np.float32)
+        out = np.zeros((boxes.shape[0], 3), np.uint64)
+        self._check(lib().hyb_let_count(self._h, boxes.shape[0], C.c_void_p(boxes.ctypes.data), C.c_void_p(out.ctypes.data)))
+        return out
 
     def sync(self):
         self._check(lib().hyb_sync(self._h))

@@ -434,6 +434,32 @@ int hyb_run_host(const hyb_params *params, int64_t n, hyb_float4 *h_pos_m, hyb_f
     return rc;
 }
 
+int hyb_let_count(hyb_ctx *ctx, int32_t ndom, const float *h_boxes, uint64_t *h_counts)
+{
+    Ctx *c = reinterpret_cast<Ctx *>(ctx);
+    if (!c) return fail(nullptr, HYB_ERR_INVALID_ARG, "ctx is NULL");
+    if (ndom < 1 || !h_boxes || !h_counts) return fail(c, HYB_ERR_INVALID_ARG, "need ndom >= 1 and two host pointers");
+    if (!c->tree_valid) return fail(c, HYB_ERR_NO_TREE, "no tree for the current positions");
+    if (c->p.mac != HYB_MAC_ABS) return fail(c, HYB_ERR_INVALID_ARG, "hyb_let_count needs HYB_MAC_ABS (r_b and b_max per node)");
+    for (int32_t i = 0; i < ndom; i++)
+        for (int a = 0; a < 3; a++)
+            if (!(h_boxes[6 * i + a] < h_boxes[6 * i + 3 + a])) return fail(c, HYB_ERR_INVALID_ARG, "a domain box is empty or NaN");
+    cudaSetDevice(c->device);
+    char *d = nullptr;
+    const size_t bb = sizeof(float) * 6 * (size_t)ndom, ob = sizeof(uint64_t) * 3 * (size_t)ndom;
+    cudaError_t e = cudaMalloc(&d, ((bb + 255) & ~(size_t)255) + ob);
+    if (e != cudaSuccess) return cuda_fail(c, e, "cudaMalloc");
+    unsigned long long *d_out = reinterpret_cast<unsigned long long *>(d + ((bb + 255) & ~(size_t)255));
+    int rc = HYB_OK;
+    e = cudaMemcpyAsync(d, h_boxes, bb, cudaMemcpyHostToDevice, c->stream);
+    if (e == cudaSuccess) e = launch_let_count(c, ndom, reinterpret_cast<const float *>(d), d_out);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(h_counts, d_out, ob, cudaMemcpyDeviceToHost, c->stream);
+    if (e != cudaSuccess) rc = cuda_fail(c, e, "hyb_let_count");
+    else { c->launches += 1; rc = hyb_sync(ctx); }
+    cudaFree(d);
+    return rc;
+}
+
 const char *hyb_last_error(const hyb_ctx *ctx)
 {
     const Ctx *c = reinterpret_cast<const Ctx *>(ctx);

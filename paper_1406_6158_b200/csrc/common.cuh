@@ -135,6 +135,7 @@ cudaError_t launch_build_tree(Ctx *c);
 cudaError_t launch_walk(Ctx *c, int mode);
 cudaError_t launch_kick_drift(Ctx *c, float c_soft, float c_hard, float dt_drift);
 cudaError_t launch_zero_acc(Ctx *c, hyb_float4 *a);
+cudaError_t launch_let_count(Ctx *c, int ndom, const float *d_boxes, unsigned long long *d_out);
 
 // ---- device helpers ------------------------------------------------------------------
 __device__ __forceinline__ u32 enc_float(float f)
