@@ -5,8 +5,8 @@
 // the hard force the walk additionally drops what is farther than R_2 + b_max from the domain (Eq. 15).
 // On one GPU there is nothing to exchange, but the sizes of those trees -- the paper's N_soft and N_hard
 // -- can be COUNTED from the global tree for any set of virtual domains.  One warp walks the tree for one
-// domain; a lane tests one node per iteration.  Decisions in fp32 with one rounding per operation, the
-// same sequence as the oracle's orc_let_count.
+// domain; a lane tests one node per iteration.  Decisions in fp32 with one rounding per operation (the
+// sequence include/hyb.h states for hyb_let_count).
 #include "common.cuh"
 
 namespace hyb {
