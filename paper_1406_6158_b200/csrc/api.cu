@@ -35,11 +35,15 @@ Layout plan_workspace(int64_t n)
     L.key_orig = take(8 * N); L.key_a = take(8 * N); L.key_b = take(8 * N);
     L.val_a = take(4 * N); L.val_b = take(4 * N);
     L.pos_tmp = take(16 * N); L.vel_tmp = take(16 * N); L.id_tmp = take(4 * N);
+    // cleared at the start of every build by ONE memset: [zero_begin, zero_end)
     L.rs_status = take(4 * 256 * (size_t)(L.rs_tiles + L.rs_blocks) * RS_PASSES);
+    L.zero_begin = L.rs_status;
     L.sc_status = take(8 * (size_t)(L.sc_tiles + L.po_tiles));
-    L.gnode_at = take(4 * N); L.gflag = take(N);
-    L.pre_level = take(NC); L.pre_first = take(4 * NC); L.pre_of_bfs = take(4 * NC); L.bfs_of_pre = take(4 * NC);
     L.node_status = take(4 * 256 * (size_t)(L.node_tiles + L.node_blocks));
+    L.gflag = take(N);
+    L.zero_end = off;
+    L.gnode_at = take(4 * N);
+    L.pre_level = take(NC); L.pre_first = take(4 * NC); L.pre_of_bfs = take(4 * NC); L.bfs_of_pre = take(4 * NC);
     L.level = take(NC); L.first = take(4 * NC); L.count = take(4 * NC); L.child = take(4 * NC);
     L.nchild = take(NC); L.parent = take(4 * NC); L.arrived = take(4 * NC);
     L.nodes = take(sizeof(NodeRec) * NC);
@@ -105,9 +109,9 @@ static int do_build(Ctx *c, bool hard_only = false)
     if (e != cudaSuccess) return cuda_fail(c, e, "build_tree");
     c->tree_valid = true;
     c->acc_valid = false;
-    // bbox, root cube, keys, digit bases, 8 sort passes, permute | preorder, level offsets, level sort,
+    // bbox (+ root cube), keys, digit bases, 8 sort passes, permute | preorder (+ level offsets), level sort,
     // link, upsweep, group mark / scan / info (+ b_max, r_b in absolute-MAC mode)
-    c->launches += 13 + 8 + (c->p.mac == HYB_MAC_ABS && !hard_only ? 2 : 0) + (c->p.split ? 1 : 0);     // + ganc
+    c->launches += 12 + 7 + (c->p.mac == HYB_MAC_ABS && !hard_only ? 2 : 0) + (c->p.split ? 1 : 0);     // + ganc
     return HYB_OK;
 }
 

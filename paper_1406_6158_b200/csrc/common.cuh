@@ -93,6 +93,7 @@ struct Layout {   // byte offsets into the workspace; computed by plan_workspace
     size_t gfirst, gcount, glo, ghi, ncell, npart, nhard;   // [group_cap]
     size_t gnode, ganc;         // u32[group_cap]: tree node a group hangs from; start node of its hard walk
     size_t splitq;              // u32[4 group_cap]: sink ranges of split groups, processed first (walk.cu)
+    size_t zero_begin, zero_end; // look-back statuses and group flags: cleared by one memset per build
     size_t total;
     int64_t n, node_cap, group_cap;
     int64_t rs_tiles, node_tiles, sc_tiles, po_tiles;

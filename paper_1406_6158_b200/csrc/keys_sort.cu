@@ -6,6 +6,24 @@
 namespace hyb {
 
 // ------------------------------------------------------------------ a1: bounding box (T1, T2)
+// T3: root cube.  One thread (of the last CTA of bbox_kernel to finish).
+__device__ void root_cube(DevCtl *ctl)
+{
+    double L = 0.0;
+    for (int a = 0; a < 3; a++) {
+        float lo = dec_float(ld_volatile_u32(&ctl->bbox_enc[a])), hi = dec_float(ld_volatile_u32(&ctl->bbox_enc[3 + a]));
+        ctl->bbox[a] = lo; ctl->bbox[3 + a] = hi;
+        double e = __dsub_rn((double)hi, (double)lo);
+        if (e > L) L = e;
+        ctl->origin[a] = (double)lo;
+    }
+    if (!(L > 0.0) || !isfinite(L)) L = 1.0;
+    ctl->L = L;
+    ctl->inv = __ddiv_rn(2097152.0, L);
+    ctl->Lf = __double2float_rn(L);
+}
+
+
 __global__ void __launch_bounds__(256) bbox_kernel(const float4 *__restrict__ pos, u32 n, DevCtl *ctl)
 {
     float lo[3] = {INFINITY, INFINITY, INFINITY}, hi[3] = {-INFINITY, -INFINITY, -INFINITY};
@@ -31,23 +49,13 @@ __global__ void __launch_bounds__(256) bbox_kernel(const float4 *__restrict__ po
     __syncthreads();
     if (threadIdx.x < 3) atomicMin(&ctl->bbox_enc[threadIdx.x], s_enc[threadIdx.x]);
     else if (threadIdx.x < 6) atomicMax(&ctl->bbox_enc[threadIdx.x], s_enc[threadIdx.x]);
-}
-
-// T3: root cube.  One thread.
-__global__ void root_cube_kernel(DevCtl *ctl)
-{
-    double L = 0.0;
-    for (int a = 0; a < 3; a++) {
-        float lo = dec_float(ctl->bbox_enc[a]), hi = dec_float(ctl->bbox_enc[3 + a]);
-        ctl->bbox[a] = lo; ctl->bbox[3 + a] = hi;
-        double e = __dsub_rn((double)hi, (double)lo);
-        if (e > L) L = e;
-        ctl->origin[a] = (double)lo;
+    // the last CTA to get here sees every CTA's contribution and derives the root cube
+    __threadfence();
+    __syncthreads();
+    if (threadIdx.x == 0 && atomicAdd(&ctl->tile_counter[11], 1u) == gridDim.x - 1) {
+        __threadfence();
+        root_cube(ctl);
     }
-    if (!(L > 0.0) || !isfinite(L)) L = 1.0;
-    ctl->L = L;
-    ctl->inv = __ddiv_rn(2097152.0, L);
-    ctl->Lf = __double2float_rn(L);
 }
 
 // ------------------------------------------------------------------ a2: keys (T4, T5)
@@ -130,7 +138,6 @@ cudaError_t launch_keys_sort_permute(Ctx *c)
     const int grid = (int)imin64((c->n + 255) / 256, (int64_t)c->num_sms * 8);
 
     bbox_kernel<<<grid, 256, 0, st>>>(reinterpret_cast<const float4 *>(c->pos), n, ctl);
-    root_cube_kernel<<<1, 1, 0, st>>>(ctl);
     u64 *key_orig = wsptr<u64>(c, L.key_orig), *key_a = wsptr<u64>(c, L.key_a), *key_b = wsptr<u64>(c, L.key_b);
     u32 *val_a = wsptr<u32>(c, L.val_a), *val_b = wsptr<u32>(c, L.val_b);
     // few CTAs: every CTA ends with up to 2048 global atomics for its share of the digit histograms

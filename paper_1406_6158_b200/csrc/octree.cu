@@ -23,6 +23,27 @@ __device__ __forceinline__ int lcp_levels(u64 a, u64 b)
 }
 
 // ------------------------------------------------------------------ a5: preorder emission
+// level_offset and the counting-sort bases (clamped to the node pool).  One thread of the last CTA of
+// preorder_kernel to finish (every CTA has added its share of node_hist by then).
+__device__ void level_offsets(DevCtl *ctl)
+{
+    {
+        // node pool overflow: the counting-sort bases would point past the pool, so drop the tree
+        // (nn = 0 makes every later stage a no-op); the status bit reports the failure.
+        if (ld_volatile_u32(&ctl->status) & ST_NODE_OVERFLOW) ctl->nn = 0;
+        const u32 nn = ld_volatile_u32(&ctl->nn);
+        u32 run = 0;
+        for (int l = 0; l <= MAXLEVEL; l++) {
+            ctl->level_offset[l] = min(run, nn);
+            ctl->node_base[l] = run;
+            run += ld_volatile_u32(&ctl->node_hist[l]);
+        }
+        ctl->level_offset[MAXLEVEL + 1] = min(run, nn);
+        for (int l = MAXLEVEL + 1; l < 256; l++) ctl->node_base[l] = run;
+    }
+}
+
+
 constexpr int PO_HALO = 64;
 
 __global__ void __launch_bounds__(SC_THREADS) preorder_kernel(
@@ -114,23 +135,12 @@ __global__ void __launch_bounds__(SC_THREADS) preorder_kernel(
         __syncthreads();
         if (tid <= MAXLEVEL && s_hist[tid]) atomicAdd(&ctl->node_hist[tid], s_hist[tid]);
     }
-}
-
-// level_offset and the counting-sort bases (clamped to the node pool).  One warp.
-__global__ void level_offset_kernel(DevCtl *ctl)
-{
-    if (threadIdx.x == 0) {
-        // node pool overflow: the counting-sort bases would point past the pool, so drop the tree
-        // (nn = 0 makes every later stage a no-op); the status bit reports the failure.
-        if (ctl->status & ST_NODE_OVERFLOW) ctl->nn = 0;
-        u32 run = 0;
-        for (int l = 0; l <= MAXLEVEL; l++) {
-            ctl->level_offset[l] = min(run, ctl->nn);
-            ctl->node_base[l] = run;
-            run += ctl->node_hist[l];
-        }
-        ctl->level_offset[MAXLEVEL + 1] = min(run, ctl->nn);
-        for (int l = MAXLEVEL + 1; l < 256; l++) ctl->node_base[l] = run;
+    // the last CTA to leave sees the complete level histogram and the node count
+    __threadfence();
+    __syncthreads();
+    if (tid == 0 && atomicAdd(&ctl->tile_counter[12], 1u) == gridDim.x - 1) {
+        __threadfence();
+        level_offsets(ctl);
     }
 }
 
@@ -563,10 +573,7 @@ cudaError_t launch_build_tree(Ctx *c)
     cudaMemsetAsync(reinterpret_cast<char *>(ctl) + offsetof(DevCtl, bbox_enc), 0,
                     offsetof(DevCtl, bbox) - offsetof(DevCtl, bbox_enc), st);
     cudaMemsetAsync(reinterpret_cast<char *>(ctl) + offsetof(DevCtl, bbox_enc), 0xFF, 3 * sizeof(u32), st);
-    cudaMemsetAsync(c->ws + L.rs_status, 0, sizeof(u32) * 256 * (size_t)(L.rs_tiles + L.rs_blocks) * RS_PASSES, st);
-    cudaMemsetAsync(c->ws + L.sc_status, 0, sizeof(u64) * (size_t)(L.sc_tiles + L.po_tiles), st);
-    cudaMemsetAsync(c->ws + L.node_status, 0, sizeof(u32) * 256 * (size_t)(L.node_tiles + L.node_blocks), st);
-    cudaMemsetAsync(c->ws + L.gflag, 0, (size_t)n, st);
+    cudaMemsetAsync(c->ws + L.zero_begin, 0, L.zero_end - L.zero_begin, st);     // look-back statuses, group flags
 
     cudaError_t e = launch_keys_sort_permute(c);
     if (e != cudaSuccess) return e;
@@ -579,7 +586,6 @@ cudaError_t launch_build_tree(Ctx *c)
     const int po_grid = (int)imin64(L.po_tiles, (int64_t)c->num_sms * 8);
     preorder_kernel<<<po_grid, SC_THREADS, 0, st>>>(key, n, c->p.leaf_max, (u32)L.node_cap, ctl, sc_status,
                                                     pre_level, pre_first);
-    level_offset_kernel<<<1, 32, 0, st>>>(ctl);
     unsigned char *level = wsptr<unsigned char>(c, L.level);
     u32 *pre_of_bfs = wsptr<u32>(c, L.pre_of_bfs), *bfs_of_pre = wsptr<u32>(c, L.bfs_of_pre);
     const int ngrid = (int)imin64(L.node_tiles, (int64_t)c->num_sms * 3);
