@@ -53,8 +53,9 @@ typedef struct hyb_params {
                           HYB_GROUP_SIBLINGS = runs of consecutive sibling cells of <= group_max particles
                           in all, HYB_GROUP_NODE = one tree node per group (R17);
                           HYB_GROUP_AUTO = SIBLINGS, except that hyb_step builds the trees that only a
-                          hard walk uses with NODE (the hard force is a direct sum whatever the groups
-                          are; small groups list fewer particles beyond r_out)                        */
+                          hard walk uses with runs of at most group_max / 2 sinks (the hard force is a
+                          direct sum whatever the groups are; smaller groups list fewer particles beyond
+                          r_out)                                                                        */
     int32_t hard_tree; /* 0 = the hard force is the direct K-weighted sum over every particle of the leaves
                           within r_out (R20); 1 = the paper's hard walk: the
                           MAC applies there too, a cell accepted within r_out contributes K(r_COM) F_COM and

@@ -117,6 +117,7 @@ struct Ctx {
     char *ws;
     Layout L;
     bool tree_valid, acc_valid;
+    int group_max_now;
     int grouping_now;              // HYB_GROUP_NODE / SIBLINGS of the build being enqueued
     bool boxes_only;               // the build being enqueued is read by a hard walk only: no moments
     cudaEvent_t ev[5];

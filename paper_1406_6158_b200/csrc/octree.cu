@@ -609,7 +609,7 @@ cudaError_t launch_build_tree(Ctx *c)
     cudaStreamWaitEvent(ax, c->ev_linked, 0);
     unsigned char *gflag = wsptr<unsigned char>(c, L.gflag);
     gmark_kernel<<<(int)((L.node_cap + 255) / 256), 256, 0, ax>>>(ctl, first, count, child, nchild, parent,
-                                                                  c->p.group_max, c->grouping_now, gflag, wsptr<u32>(c, L.gnode_at));
+                                                                  c->group_max_now, c->grouping_now, gflag, wsptr<u32>(c, L.gnode_at));
     u32 *gfirst = wsptr<u32>(c, L.gfirst);
     gscan_kernel<<<sc_grid, SC_THREADS, 0, ax>>>(gflag, n, ctl, sc_status + L.po_tiles, gfirst, wsptr<u32>(c, L.gnode_at),
                                                  wsptr<u32>(c, L.gnode));

@@ -25,7 +25,7 @@ class Config:
     kfunc: int = 0               # 0 = paper Eq. 10
     split: int = 1               # 1 = hybrid, 0 = normal tree
     grouping: int = 2            # sink groups: 1 = runs of consecutive small sibling cells, 0 = single tree nodes,
-                                 # 2 = 1, except 0 for the trees of hyb_step that only a hard walk uses
+                                 # 2 = 1, with runs of at most group_max / 2 for the trees of hyb_step that only a hard walk uses
 
     hard_tree: int = 0           # 0 = hard force by direct K-weighted sum (R20), 1 = the paper's MAC-approximated hard walk
 
