@@ -100,6 +100,8 @@ def main():
     ap.add_argument("--no-normal", action="store_true", help="skip the normal-tree comparison leg")
     ap.add_argument("--paper-n", type=int, default=None,
                     help="instead of --config: the paper's own recipe (PAPER.md:172-174) for a Plummer model of N particles")
+    ap.add_argument("--hard-refit", type=int, default=None, choices=[0, 1],
+                    help="1: hard-only substeps refit the boxes instead of rebuilding the tree (not the paper's procedure)")
     ap.add_argument("--hard-tree", type=int, default=None, choices=[0, 1],
                     help="1: the paper's MAC-approximated hard walk instead of the direct hard sum (DESIGN.md R20)")
     ap.add_argument("--grouping", type=int, default=None, choices=[0, 1, 2],
@@ -119,9 +121,11 @@ def main():
         cfg = cfg.with_(grouping=args.grouping)
     if args.hard_tree is not None:
         cfg = cfg.with_(hard_tree=args.hard_tree)
+    if args.hard_refit is not None:
+        cfg = cfg.with_(hard_refit=args.hard_refit)
     config = {"workload": f"{cfg.name}: {cfg.kind} N={cfg.n}, eps={cfg.eps}, theta={cfg.theta}, leaf<={cfg.leaf_max}, "
                           f"group<={cfg.group_max}, r_in={cfg.r_in}, r_out={cfg.r_out}, dt_soft=1/{round(1 / cfg.dt_soft)}, "
-                          f"n_sub={cfg.n_sub}, grouping={cfg.grouping}, hard_tree={cfg.hard_tree}, seed {cfg.seed}",
+                          f"n_sub={cfg.n_sub}, grouping={cfg.grouping}, hard_tree={cfg.hard_tree}, hard_refit={cfg.hard_refit}, seed {cfg.seed}",
               "step": "one soft cycle: n_sub tree builds + 1 fused soft/hard walk + (n_sub-1) hard walks + kick/drift",
               "l2": "256 MiB L2 flush between timed steps", "replicas": world}
 
@@ -296,6 +300,29 @@ def main():
                                    "80-90 % of a normal tree (HA-PACS: Tesla M2090 + E5-2670, multi-process)"}
         hn.close()
 
+    # ---- variant, not the headline: hard-only substeps refit the tight boxes instead of rebuilding the tree
+    #      (R21: the paper rebuilds; the hard force is the same direct sum either way)
+    refit = None
+    if rank == 0 and not args.no_normal and cfg.split and not cfg.hard_tree and not cfg.hard_refit and cfg.n_sub > 1:
+        hr = Hyb(HybParams.from_config(cfg, hard_refit=1), torch.from_numpy(pos).cuda(), torch.from_numpy(vel).cuda())
+        hr.step(0)
+        for _ in range(2):
+            hr.step(1)
+        hr.export("interactions"); hr.export("timings")
+        kr = max(2, min(K, 4))
+        evr = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(kr)]
+        for a, b in evr:
+            flush.zero_()
+            a.record(); hr.step(1); b.record()
+        torch.cuda.synchronize()
+        r_ms = sum(a.elapsed_time(b) for a, b in evr) / kr
+        r_stage = hr.export("timings").astype(np.float64)
+        refit = {"ms_per_step": r_ms, "stages": {"build_or_refit_ms": r_stage[0] / kr, "soft_ms": r_stage[1] / kr,
+                                                 "hard_ms": r_stage[2] / kr, "integrate_ms": r_stage[3] / kr},
+                 "ratio_to_rebuild": r_ms / (total_ms / K),
+                 "what": "hard_refit = 1: one tree build per soft step, n_sub - 1 box refits; same forces up to fp32 summation order"}
+        hr.close()
+
     cpu_baseline = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         cpu_baseline, _ = oracle_sample(cfg, pos, args.cpu_seconds)
@@ -306,7 +333,7 @@ def main():
             "warmup": args.warmup, "ms_per_step": total_ms / K, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f32", "data": "synthetic", "config": config, "stages": stages,
             "interactions_per_step": {"soft": inter[0] / K, "hard": inter[1] / K},
-            "roofline": roofline, "hbm_stages": hbm_stages, "normal_tree": normal, "cpu_baseline": cpu_baseline, "e2e": e2e,
+            "roofline": roofline, "hbm_stages": hbm_stages, "normal_tree": normal, "hard_refit_variant": refit, "cpu_baseline": cpu_baseline, "e2e": e2e,
             "gpu_launches": launches,
             "clocks": {"sm_mhz": sm_mhz, "sm_max_mhz": sm_max, "reasons": sorted(clk["reasons"]),
                        "samples": len(sm), **({"error": clk["error"]} if "error" in clk else {})}}))

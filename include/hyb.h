@@ -60,6 +60,11 @@ typedef struct hyb_params {
                           within r_out (R20); 1 = the paper's hard walk: the
                           MAC applies there too, a cell accepted within r_out contributes K(r_COM) F_COM and
                           (1 - K(r_COM)) F_COM to the soft force, and the soft walk drops rule (b)        */
+    int32_t hard_refit;/* hyb_step only, needs split = 1 and hard_tree = 0.  0 = the tree is rebuilt before
+                          every force evaluation, as the paper does (R21).  1 = it is
+                          rebuilt at soft steps only; the hard-only substeps keep the store order and the
+                          topology and refit the tight boxes (see hyb_refit_tree): the hard force is the same
+                          direct sum, only the order of the fp32 additions differs                          */
 } hyb_params;
 
 enum {
@@ -143,6 +148,14 @@ int hyb_set_params(hyb_ctx *ctx, const hyb_params *params);
  * linear octree, centre-of-mass / opening-radius upsweep
  * and sink groups for the current positions.  Asynchronous. */
 int hyb_build_tree(hyb_ctx *ctx);
+
+/* After the positions have moved a little since the last hyb_build_tree (same store order): recompute the
+ * tight boxes of all nodes and sink groups for the current positions, keeping the topology.  The result
+ * serves hyb_hard_force with hard_tree = 0 only (a direct K-weighted sum over everything within r_out does
+ * not depend on which hierarchy of tight boxes finds the neighbours); hyb_soft_force and hyb_let_count
+ * return HYB_ERR_NO_TREE until the next hyb_build_tree.  Asynchronous.
+ * Errors: NO_TREE (nothing to refit), INVALID_ARG (split = 0 or hard_tree = 1). */
+int hyb_refit_tree(hyb_ctx *ctx);
 
 /* Step a8 (+a9 at a soft-step).  split = 1: one fused group walk that writes d_a_soft
  * (cells accepted by the MAC as monopoles, plus (1-K)-weighted neighbours, Eq. 9)

@@ -39,7 +39,7 @@ class HybParams(C.Structure):
     _fields_ = [("G", C.c_float), ("eps", C.c_float), ("theta", C.c_float), ("a_err", C.c_float),
                 ("r_in", C.c_float), ("r_out", C.c_float), ("dt_soft", C.c_float),
                 ("n_sub", C.c_int32), ("leaf_max", C.c_int32), ("group_max", C.c_int32),
-                ("mac", C.c_int32), ("kfunc", C.c_int32), ("split", C.c_int32), ("grouping", C.c_int32), ("hard_tree", C.c_int32)]
+                ("mac", C.c_int32), ("kfunc", C.c_int32), ("split", C.c_int32), ("grouping", C.c_int32), ("hard_tree", C.c_int32), ("hard_refit", C.c_int32)]
 
     @classmethod
     def from_config(cls, cfg, **over):
@@ -65,7 +65,7 @@ def lib():
         L.hyb_init.restype = C.c_int
         L.hyb_init.argtypes = [C.POINTER(vp), C.POINTER(HybParams), C.c_int64, vp, vp, vp, vp, vp, vp, C.c_size_t,
                                C.c_int, vp]
-        for name in ("hyb_build_tree", "hyb_soft_force", "hyb_hard_force", "hyb_sync"):
+        for name in ("hyb_build_tree", "hyb_refit_tree", "hyb_soft_force", "hyb_hard_force", "hyb_sync"):
             getattr(L, name).restype = C.c_int
             getattr(L, name).argtypes = [vp]
         L.hyb_set_params.restype = C.c_int
@@ -144,6 +144,9 @@ class Hyb:
 
     def build_tree(self):
         self._check(lib().hyb_build_tree(self._h))
+
+    def refit_tree(self):
+        self._check(lib().hyb_refit_tree(self._h))
 
     def soft_force(self):
         self._check(lib().hyb_soft_force(self._h))

@@ -73,6 +73,8 @@ static bool params_ok(const hyb_params *p, int64_t n, char *msg)
     if (p->kfunc != HYB_K_PAPER && p->kfunc != HYB_K_POLY7) return bad("unknown kfunc");
     if (p->split != 0 && p->split != 1) return bad("split must be 0 or 1");
     if (p->hard_tree != 0 && p->hard_tree != 1) return bad("hard_tree must be 0 or 1");
+    if (p->hard_refit != 0 && p->hard_refit != 1) return bad("hard_refit must be 0 or 1");
+    if (p->hard_refit == 1 && (p->split != 1 || p->hard_tree != 0)) return bad("hard_refit needs split = 1 and hard_tree = 0");
     if (p->grouping != HYB_GROUP_NODE && p->grouping != HYB_GROUP_SIBLINGS && p->grouping != HYB_GROUP_AUTO) return bad("unknown grouping");
     if (p->split == 1 && !(p->r_in >= 0.0f && p->r_out > p->r_in && isfinite(p->r_out))) return bad("need 0 <= r_in < r_out");
     return true;
@@ -112,10 +114,32 @@ static int do_build(Ctx *c, bool hard_only = false)
     cudaError_t e = launch_build_tree(c);
     if (e != cudaSuccess) return cuda_fail(c, e, "build_tree");
     c->tree_valid = true;
+    c->tree_refit = false;
     c->acc_valid = false;
     // bbox (+ root cube), keys, digit bases, 8 sort passes, permute | preorder (+ level offsets), level sort,
     // link, upsweep, group mark / scan / info (+ b_max, r_b in absolute-MAC mode)
     c->launches += 12 + 7 + (c->p.mac == HYB_MAC_ABS && !hard_only ? 2 : 0) + (c->p.split ? 1 : 0);     // + ganc
+    return HYB_OK;
+}
+
+// hard-only substep with hard_refit: boxes of the existing topology for the drifted positions; the first
+// one of a cycle also forms the (smaller) sink groups of the hard walks
+static int do_refit(Ctx *c, bool regroup)
+{
+    cudaError_t e = cudaSuccess;
+    if (regroup) {
+        c->grouping_now = c->p.grouping == HYB_GROUP_AUTO ? HYB_GROUP_SIBLINGS : c->p.grouping;
+        c->group_max_now = c->p.group_max;
+        if (c->p.grouping == HYB_GROUP_AUTO)
+            c->group_max_now = c->p.group_max / 2 > c->p.leaf_max ? c->p.group_max / 2 : c->p.leaf_max;
+        e = launch_regroup(c);
+        c->launches += 3;
+    }
+    if (e == cudaSuccess) e = launch_refit_tree(c);
+    if (e != cudaSuccess) return cuda_fail(c, e, "refit_tree");
+    c->launches += 2;
+    c->tree_refit = true;
+    c->acc_valid = false;
     return HYB_OK;
 }
 
@@ -213,11 +237,21 @@ int hyb_build_tree(hyb_ctx *ctx)
     return do_build(c);
 }
 
+int hyb_refit_tree(hyb_ctx *ctx)
+{
+    Ctx *c = reinterpret_cast<Ctx *>(ctx);
+    if (!c) return fail(nullptr, HYB_ERR_INVALID_ARG, "ctx is NULL");
+    if (!c->tree_valid) return fail(c, HYB_ERR_NO_TREE, "nothing to refit: call hyb_build_tree first");
+    if (c->p.split != 1 || c->p.hard_tree != 0) return fail(c, HYB_ERR_INVALID_ARG, "a refitted tree serves the direct hard force only (split = 1, hard_tree = 0)");
+    cudaSetDevice(c->device);
+    return do_refit(c, false);
+}
+
 int hyb_soft_force(hyb_ctx *ctx)
 {
     Ctx *c = reinterpret_cast<Ctx *>(ctx);
     if (!c) return fail(nullptr, HYB_ERR_INVALID_ARG, "ctx is NULL");
-    if (!c->tree_valid) return fail(c, HYB_ERR_NO_TREE, "no tree for the current positions");
+    if (!c->tree_valid || c->tree_refit) return fail(c, HYB_ERR_NO_TREE, "no tree for the current positions");
     cudaSetDevice(c->device);
     int rc = do_soft(c);
     if (rc == HYB_OK) c->acc_valid = true;
@@ -255,7 +289,7 @@ int hyb_step(hyb_ctx *ctx, int32_t n_soft_steps)
     const int nsub = c->p.n_sub;
     const float dts = c->p.dt_soft, dth = dts / (float)nsub;
     int rc;
-    if (!c->acc_valid) {
+    if (!c->acc_valid || (c->p.hard_refit && (!c->tree_valid || c->tree_refit))) {
         if ((rc = do_build(c)) != HYB_OK) return rc;
         if ((rc = do_soft(c)) != HYB_OK) return rc;
         c->acc_valid = true;
@@ -277,7 +311,9 @@ int hyb_step(hyb_ctx *ctx, int32_t n_soft_steps)
             if (e != cudaSuccess) return cuda_fail(c, e, "kick_drift");
             cudaEvent_t e1 = c->timing ? ev() : nullptr;
             const bool soft_step = !split || k == nsub - 1;
-            if ((rc = do_build(c, !soft_step)) != HYB_OK) return rc;
+            if (!soft_step && c->p.hard_refit) rc = do_refit(c, k == 0 && c->p.grouping == HYB_GROUP_AUTO);
+            else rc = do_build(c, !soft_step);
+            if (rc != HYB_OK) return rc;
             cudaEvent_t e2 = c->timing ? ev() : nullptr;
             if (soft_step) rc = do_soft(c); else rc = do_hard(c);
             if (rc != HYB_OK) return rc;
@@ -447,7 +483,7 @@ int hyb_let_count(hyb_ctx *ctx, int32_t ndom, const float *h_boxes, uint64_t *h_
     Ctx *c = reinterpret_cast<Ctx *>(ctx);
     if (!c) return fail(nullptr, HYB_ERR_INVALID_ARG, "ctx is NULL");
     if (ndom < 1 || !h_boxes || !h_counts) return fail(c, HYB_ERR_INVALID_ARG, "need ndom >= 1 and two host pointers");
-    if (!c->tree_valid) return fail(c, HYB_ERR_NO_TREE, "no tree for the current positions");
+    if (!c->tree_valid || c->tree_refit) return fail(c, HYB_ERR_NO_TREE, "no tree for the current positions");
     if (c->p.mac != HYB_MAC_ABS) return fail(c, HYB_ERR_INVALID_ARG, "hyb_let_count needs HYB_MAC_ABS (r_b and b_max per node)");
     for (int32_t i = 0; i < ndom; i++)
         for (int a = 0; a < 3; a++)

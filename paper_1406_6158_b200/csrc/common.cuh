@@ -117,6 +117,7 @@ struct Ctx {
     char *ws;
     Layout L;
     bool tree_valid, acc_valid;
+    bool tree_refit;               // the tree's boxes were refitted after a drift: valid for the direct hard walk only
     int group_max_now;
     int grouping_now;              // HYB_GROUP_NODE / SIBLINGS of the build being enqueued
     bool boxes_only;               // the build being enqueued is read by a hard walk only: no moments
@@ -134,6 +135,8 @@ static inline T *wsptr(const Ctx *c, size_t off) { return reinterpret_cast<T *>(
 
 // stage launchers (each enqueues on c->stream and returns the last CUDA error)
 cudaError_t launch_build_tree(Ctx *c);
+cudaError_t launch_regroup(Ctx *c);        // sink groups again (group_max_now / grouping_now) on the existing topology
+cudaError_t launch_refit_tree(Ctx *c);     // tight boxes of nodes and groups for the current positions, same topology
 cudaError_t launch_walk(Ctx *c, int mode);
 cudaError_t launch_kick_drift(Ctx *c, float c_soft, float c_hard, float dt_drift);
 cudaError_t launch_zero_acc(Ctx *c, hyb_float4 *a);

@@ -639,4 +639,53 @@ cudaError_t launch_build_tree(Ctx *c)
     return cudaGetLastError();
 }
 
+// ------------------------------------------------------------------ refit (hyb_params.hard_refit)
+// Between two soft steps the particles move by a small fraction of r_out.  The hard force is a direct
+// K-weighted sum over everything within r_out, so it does not need the canonical tree of the new
+// positions: any hierarchy of TIGHT boxes finds the same neighbours.  A refit keeps the store order and
+// the topology of the last full build and recomputes the tight boxes of the nodes (boxes-only upsweep)
+// and of the sink groups.  (The Morton cells no longer hold their particles exactly, so the walk starts
+// at the root instead of ganc.)
+cudaError_t launch_regroup(Ctx *c)
+{
+    const Layout &L = c->L;
+    const u32 n = (u32)c->n;
+    cudaStream_t st = c->stream;
+    DevCtl *ctl = c->ctl;
+    cudaMemsetAsync(c->ws + L.gflag, 0, (size_t)n, st);
+    cudaMemsetAsync(c->ws + L.sc_status + sizeof(u64) * (size_t)L.po_tiles, 0, sizeof(u64) * (size_t)L.sc_tiles, st);
+    cudaMemsetAsync(&ctl->tile_counter[9], 0, sizeof(u32), st);
+    unsigned char *gflag = wsptr<unsigned char>(c, L.gflag);
+    gmark_kernel<<<(int)((L.node_cap + 255) / 256), 256, 0, st>>>(
+        ctl, wsptr<u32>(c, L.first), wsptr<u32>(c, L.count), wsptr<u32>(c, L.child), wsptr<unsigned char>(c, L.nchild),
+        wsptr<u32>(c, L.parent), c->group_max_now, c->grouping_now, gflag, wsptr<u32>(c, L.gnode_at));
+    const int sc_grid = (int)imin64(L.sc_tiles, (int64_t)c->num_sms * 8);
+    gscan_kernel<<<sc_grid, SC_THREADS, 0, st>>>(gflag, n, ctl, wsptr<u64>(c, L.sc_status) + L.po_tiles, wsptr<u32>(c, L.gfirst),
+                                                 wsptr<u32>(c, L.gnode_at), wsptr<u32>(c, L.gnode));
+    ginfo_kernel<<<(int)imin64((c->n + 255) / 256, (int64_t)c->num_sms * 8), 256, 0, st>>>(
+        ctl, n, reinterpret_cast<const float4 *>(c->pos), wsptr<u32>(c, L.gfirst), wsptr<u32>(c, L.gcount),
+        wsptr<float4>(c, L.glo), wsptr<float4>(c, L.ghi));
+    return cudaGetLastError();
+}
+
+cudaError_t launch_refit_tree(Ctx *c)
+{
+    const Layout &L = c->L;
+    cudaStream_t st = c->stream;
+    cudaMemsetAsync(c->ws + L.arrived, 0, sizeof(u32) * (size_t)L.node_cap, st);
+    NodeArrays na;
+    na.first = wsptr<u32>(c, L.first); na.count = wsptr<u32>(c, L.count); na.child = wsptr<u32>(c, L.child);
+    na.parent = wsptr<u32>(c, L.parent); na.nchild = wsptr<unsigned char>(c, L.nchild);
+    na.level = wsptr<unsigned char>(c, L.level); na.arrived = wsptr<u32>(c, L.arrived);
+    na.rec = wsptr<NodeRec>(c, L.nodes);
+    na.MS64 = wsptr<double4>(c, L.MS64); na.C64 = wsptr<double>(c, L.C64);
+    na.B2 = wsptr<double>(c, L.B2); na.leaf_of = wsptr<u32>(c, L.leaf_of);
+    upsweep_kernel<false><<<(int)((L.node_cap + 127) / 128), 128, 0, st>>>(na, reinterpret_cast<const float4 *>(c->pos), c->ctl,
+                                                                           c->p.mac, c->p.theta);
+    ginfo_kernel<<<(int)imin64((c->n + 255) / 256, (int64_t)c->num_sms * 8), 256, 0, st>>>(
+        c->ctl, (u32)c->n, reinterpret_cast<const float4 *>(c->pos), wsptr<u32>(c, L.gfirst), wsptr<u32>(c, L.gcount),
+        wsptr<float4>(c, L.glo), wsptr<float4>(c, L.ghi));
+    return cudaGetLastError();
+}
+
 }  // namespace hyb

@@ -482,7 +482,7 @@ __global__ void __launch_bounds__(WK_WARPS * 32, SmemLayout<MODE>::ctas_per_sm) 
         // the start node alone ("first child" = the node, nchild - 1 = 0): the root, or for a hard walk
         // the lowest ancestor that holds every leaf within r_out of the group box
         // (TREE: from the root -- a cell above that ancestor may be accepted by the MAC)
-        if (lane == 0) stack[0] = (MODE == WALK_HARD && !TREE) ? __ldg(a.ganc + g) : 0u;
+        if (lane == 0) stack[0] = (MODE == WALK_HARD && !TREE && a.ganc) ? __ldg(a.ganc + g) : 0u;
         __syncwarp();
 
         for (;;) {
@@ -808,7 +808,7 @@ cudaError_t launch_walk(Ctx *c, int mode)
     a.kc0 = c->p.r_out / w; a.kc1 = -1.0f / w;
     a.zero64 = 0ull;
     a.heavy = wsptr<u32>(c, L.splitq);
-    a.ganc = wsptr<u32>(c, L.ganc);
+    a.ganc = c->tree_refit ? nullptr : wsptr<u32>(c, L.ganc);      // refitted boxes: the Morton cells are stale
     a.is_split = wsptr<unsigned char>(c, L.gflag);      // the build's flag array is free between builds
     cudaMemsetAsync(&c->ctl->group_counter, 0, 2 * sizeof(u32), c->stream);      // counter, nheavy
     if (mode == WALK_HARD)

@@ -29,6 +29,8 @@ class Config:
 
     hard_tree: int = 0           # 0 = hard force by direct K-weighted sum (R20), 1 = the paper's MAC-approximated hard walk
 
+    hard_refit: int = 0          # 0 = tree rebuilt before every force evaluation (paper), 1 = hard-only substeps refit the boxes
+
     def with_(self, **kw) -> "Config":
         return replace(self, **kw)
 
