@@ -83,13 +83,14 @@ def test_cfg2_normal_tree():
     h.close()
 
 
-def test_cfg3_full_tree_sampled_forces():
+@pytest.mark.parametrize("mac", [0, 1])
+def test_cfg3_full_tree_sampled_forces(mac):
     cfg = CONFIGS[3]
     pos, vel = make_ic(cfg.kind, cfg.n, cfg.seed)
-    h = make_hyb(cfg, pos, vel)
+    h = make_hyb(cfg, pos, vel, mac=mac)
     h.build_tree(); h.sync()
-    t = O.Tree(pos, O.params_from(cfg))
-    compare_tree(h, t)
+    t = O.Tree(pos, O.params_from(cfg, mac=mac))
+    compare_tree(h, t, abs_mode=mac == 1)
     print(check_forces(h, t, gsel=_sample_groups(t.ng, 8192, 6)))
     h.close()
 
@@ -127,6 +128,19 @@ def test_cfg4_sweep():
             print(over, res)
             first = False
             del t
+    h.close()
+
+
+def test_cfg4_absolute_mac():
+    """the paper's own opening criterion (Eq. 5-6, a_err = 2^-8) at N = 2^24, centre sweep point"""
+    cfg = CONFIGS[4].with_(mac=1)
+    pos, vel = make_ic(cfg.kind, cfg.n, cfg.seed)
+    h = make_hyb(cfg, pos, vel)
+    h.build_tree(); h.sync()
+    t = O.Tree(pos, O.params_from(cfg))
+    compare_tree(h, t, abs_mode=True)
+    gsel = _sample_groups(t.ng, 4096, 13)
+    print(check_forces(h, t, gsel=gsel[::4], lists_full=False))
     h.close()
 
 
