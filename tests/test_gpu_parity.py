@@ -164,3 +164,44 @@ def test_paper_literal_hard_walk(kfunc):
     h.step(2); h.sync()
     assert np.all(np.isfinite(h.pos_m.cpu().numpy()))
     h.close()
+
+
+@pytest.mark.parametrize("case", ["one_point", "zero_masses", "collinear", "far_offset", "two_clumps"])
+def test_degenerate_inputs(case):
+    """the degenerate inputs the method has: a zero-size root cube, massless particles and cells, a tree that
+    is a chain, coordinates with few significant bits left for the separations, an almost empty root cube"""
+    rng = np.random.default_rng(7)
+    n = 700
+    pos = np.zeros((n, 4), np.float32)
+    pos[:, 3] = 1.0 / n
+    if case == "one_point":
+        pos[:, :3] = np.float32(0.25)
+    elif case == "zero_masses":
+        pos[:, :3] = rng.normal(size=(n, 3))
+        pos[::3, 3] = 0.0
+        pos[300:340, 3] = 0.0                      # whole leaves without mass: COM falls back to the box corner (T9)
+    elif case == "collinear":
+        pos[:, 0] = np.sort(rng.uniform(-1, 1, n)); pos[:, 1] = 0.5; pos[:, 2] = -0.25
+    elif case == "far_offset":
+        pos[:, :3] = 1000.0 + 0.05 * rng.normal(size=(n, 3))
+    else:
+        pos[: n // 2, :3] = 1e-3 * rng.normal(size=(n // 2, 3))
+        pos[n // 2:, :3] = 50.0 + 1e-3 * rng.normal(size=(n - n // 2, 3))
+    vel = np.zeros_like(pos)
+    cfg = CONFIGS[0].with_(n=n, r_in=0.002, r_out=0.02) if case in ("far_offset", "two_clumps") else CONFIGS[0].with_(n=n)
+    for mac in (0, 1):
+        print(case, mac, _run_case(cfg, pos, vel, mac=mac))
+
+
+def test_bitwise_reproducible():
+    """work is handed out by atomic counters, but every sum has a fixed order: two runs agree bit for bit"""
+    cfg = CONFIGS[1].with_(n=60013)
+    pos, vel = make_ic(cfg.kind, cfg.n, 77)
+    outs = []
+    for _ in range(2):
+        h = make_hyb(cfg, pos, vel)
+        h.step(2); h.sync()
+        outs.append([t.cpu().numpy().copy() for t in (h.pos_m, h.vel, h.a_soft, h.a_hard, h.ids)])
+        h.close()
+    for a, b in zip(*outs):
+        assert np.array_equal(a, b)
