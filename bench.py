@@ -267,7 +267,7 @@ def main():
         e2e = {"value": e_int / e_t, "unit": "interactions/s", "h2d_bytes_per_step": 36 * n,
                "d2h_bytes_per_step": 68 * n, "ms_per_call": 1e3 * e_t / 3,
                "what": "hyb_run_host: upload pos/vel/id, initial tree+forces, one soft cycle, download "
-                       "pos/vel/id/a_soft/a_hard; device alloc/free inside"}
+                       "pos/vel/id/a_soft/a_hard; the device buffer is kept between calls (2 untimed calls first)"}
 
     # ---- the same cycle with a plain (unsplit, theta-only) tree at dt_h: n_sub
     #      builds + n_sub full walks per cycle; reported beside the hybrid to show its compute ratio

@@ -186,11 +186,15 @@ int hyb_export(hyb_ctx *ctx, int32_t what, void *host_dst, size_t bytes, size_t 
 
 /* End-to-end convenience for HOST buffers: allocates device memory, copies the particles in,
  * runs hyb_step(n_soft_steps) (n_soft_steps = 0: one build + soft-step evaluation only), copies
- * positions, velocities, ids and both accelerations back, frees everything.  Every pointer is a
- * HOST pointer to n elements; h_interactions (optional) receives uint64[2] as HYB_X_INTERACTIONS. */
+ * positions, velocities, ids and both accelerations back.  The device buffer and its stream are kept for
+ * the next call on the same device (freed by hyb_run_host_release, or replaced when a larger n comes);
+ * concurrent calls are serialised.  Every pointer is a HOST pointer to n elements; h_interactions (optional) receives uint64[2] as HYB_X_INTERACTIONS. */
 int hyb_run_host(const hyb_params *params, int64_t n, hyb_float4 *h_pos_m, hyb_float4 *h_vel,
                  hyb_float4 *h_a_soft, hyb_float4 *h_a_hard, uint32_t *h_id, int32_t n_soft_steps,
                  int device, uint64_t *h_interactions);
+
+/* Frees what hyb_run_host keeps between calls (nothing else holds device memory in this library). */
+void hyb_run_host_release(void);
 
 /* Virtual-domain LET counts (Eq. 14-15; Fig. 4: N_soft, N_hard).  The paper's processes
  * exchange locally essential trees; on one GPU nothing is exchanged, but for any set of ndom virtual

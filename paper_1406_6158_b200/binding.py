@@ -78,6 +78,8 @@ def lib():
         L.hyb_run_host.argtypes = [C.POINTER(HybParams), C.c_int64, vp, vp, vp, vp, vp, C.c_int32, C.c_int, vp]
         L.hyb_let_count.restype = C.c_int
         L.hyb_let_count.argtypes = [vp, C.c_int32, vp, vp]
+        L.hyb_run_host_release.restype = None
+        L.hyb_run_host_release.argtypes = []
         L.hyb_last_error.restype = C.c_char_p
         L.hyb_last_error.argtypes = [vp]
         L.hyb_free.restype = None
@@ -103,6 +105,10 @@ def hyb_run_host(params: HybParams, pos_m: np.ndarray, vel: np.ndarray, ids: np.
     if rc != 0:
         raise HybError(rc, lib().hyb_last_error(None).decode())
     return a_soft, a_hard, inter
+
+
+def hyb_run_host_release() -> None:
+    lib().hyb_run_host_release()
 
 
 class Hyb:

@@ -4,6 +4,7 @@
 #include <stddef.h>
 #include <string.h>
 
+#include <mutex>
 #include <new>
 #include <vector>
 
@@ -162,6 +163,15 @@ static int do_hard(Ctx *c)
 }  // namespace hyb
 
 using namespace hyb;
+
+// device buffer and stream kept between hyb_run_host calls
+static struct { char *ptr; size_t bytes; int device; cudaStream_t st; } g_host = {nullptr, 0, -1, nullptr};
+static std::mutex g_host_mutex;
+static void release_host_cache()
+{
+    if (g_host.ptr) { cudaSetDevice(g_host.device); if (g_host.st) { cudaStreamSynchronize(g_host.st); cudaStreamDestroy(g_host.st); } cudaFree(g_host.ptr); }
+    g_host.ptr = nullptr; g_host.bytes = 0; g_host.device = -1; g_host.st = nullptr;
+}
 
 extern "C" {
 
@@ -441,16 +451,23 @@ int hyb_run_host(const hyb_params *params, int64_t n, hyb_float4 *h_pos_m, hyb_f
     cudaError_t e = cudaSetDevice(device);
     if (e != cudaSuccess) return cuda_fail(nullptr, e, "cudaSetDevice");
     const size_t ws_bytes = plan_workspace(n).total, N = (size_t)n;
-    char *d = nullptr;
     const size_t o_pos = 0, o_vel = 16 * N, o_as = 32 * N, o_ah = 48 * N, o_id = 64 * N;
     const size_t o_ws = (68 * N + 255) & ~(size_t)255;
-    e = cudaMalloc(&d, o_ws + ws_bytes);
-    if (e != cudaSuccess) return cuda_fail(nullptr, e, "cudaMalloc");
-    cudaStream_t st = nullptr;
+    // the device buffer and the stream are kept for the next call (hyb_run_host_release frees them):
+    // cudaMalloc / cudaFree of half a gigabyte cost more than the copies of a million particles
+    std::lock_guard<std::mutex> lock(g_host_mutex);
+    if (g_host.ptr && (g_host.device != device || g_host.bytes < o_ws + ws_bytes)) release_host_cache();
+    if (!g_host.ptr) {
+        e = cudaMalloc(&g_host.ptr, o_ws + ws_bytes);
+        if (e != cudaSuccess) { g_host.ptr = nullptr; return cuda_fail(nullptr, e, "cudaMalloc"); }
+        g_host.bytes = o_ws + ws_bytes; g_host.device = device;
+        if ((e = cudaStreamCreate(&g_host.st)) != cudaSuccess) { release_host_cache(); return cuda_fail(nullptr, e, "cudaStreamCreate"); }
+    }
+    char *d = g_host.ptr;
+    cudaStream_t st = g_host.st;
     int rc = HYB_OK;
     hyb_ctx *ctx = nullptr;
     do {
-        if ((e = cudaStreamCreate(&st)) != cudaSuccess) { rc = cuda_fail(nullptr, e, "cudaStreamCreate"); break; }
         cudaMemcpyAsync(d + o_pos, h_pos_m, 16 * N, cudaMemcpyHostToDevice, st);
         cudaMemcpyAsync(d + o_vel, h_vel, 16 * N, cudaMemcpyHostToDevice, st);
         cudaMemcpyAsync(d + o_id, h_id, 4 * N, cudaMemcpyHostToDevice, st);
@@ -473,9 +490,14 @@ int hyb_run_host(const hyb_params *params, int64_t n, hyb_float4 *h_pos_m, hyb_f
         }
     } while (0);
     if (ctx) hyb_free(ctx);
-    if (st) cudaStreamDestroy(st);
-    cudaFree(d);
+    if (rc != HYB_OK) release_host_cache();
     return rc;
+}
+
+void hyb_run_host_release(void)
+{
+    std::lock_guard<std::mutex> lock(g_host_mutex);
+    release_host_cache();
 }
 
 int hyb_let_count(hyb_ctx *ctx, int32_t ndom, const float *h_boxes, uint64_t *h_counts)
