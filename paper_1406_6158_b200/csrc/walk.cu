@@ -452,7 +452,7 @@ __global__ void __launch_bounds__(WK_WARPS * 32, SmemLayout<MODE>::ctas_per_sm) 
         // sink_layout() (maximises the busy fraction n P / (32 S)); lane / A by a 15-bit reciprocal
         const ushort4 lay = c_layout[n];
         const int S = lay.x, A = lay.y, P = lay.z;
-        const int US = S == 2 ? 4 : 2;                                // sources per evaluation iteration (monopoles)
+        const int US = 4;                                             // sources per evaluation iteration (monopoles)
         const int copy = (lane * (int)lay.w) >> 15;                   // = lane / A  (lane < 32, A <= 32)
         const int aidx = lane - copy * A;
         const int part = copy < P ? copy : 0x40000000;               // idle lanes never enter the loops
@@ -492,8 +492,8 @@ __global__ void __launch_bounds__(WK_WARPS * 32, SmemLayout<MODE>::ctas_per_sm) 
                     const int cnt = pad_buffer(cellbuf, ncb, P * US, dummy, lane);
                     __syncwarp();
                     if (S == 2) eval_mono<2, 4>(cellbuf, cnt, part, P, sk, eps2);
-                    else if (S == 3) eval_mono<3, 2>(cellbuf, cnt, part, P, sk, eps2);
-                    else eval_mono<4, 2>(cellbuf, cnt, part, P, sk, eps2);
+                    else if (S == 3) eval_mono<3, 4>(cellbuf, cnt, part, P, sk, eps2);
+                    else eval_mono<4, 4>(cellbuf, cnt, part, P, sk, eps2);
                     ncb = 0; flush_mono = false;
                     __syncwarp();
                 }
