@@ -498,11 +498,11 @@ __global__ void __launch_bounds__(WK_WARPS * 32, SmemLayout<MODE>::ctas_per_sm) 
                     __syncwarp();
                 }
                 if (HAS_NEAR && flush_near) {
-                    const int cnt = pad_buffer(partbuf, npb, P * 2, dummy, lane);
+                    const int cnt = pad_buffer(partbuf, npb, P * 4, dummy, lane);
                     __syncwarp();
-                    if (S == 2) eval_near<2, 2, MODE == WALK_HYBRID, KF>(partbuf, cnt, part, P, sk, eps2, kc0, kc1);
-                    else if (S == 3) eval_near<3, 2, MODE == WALK_HYBRID, KF>(partbuf, cnt, part, P, sk, eps2, kc0, kc1);
-                    else eval_near<4, 2, MODE == WALK_HYBRID, KF>(partbuf, cnt, part, P, sk, eps2, kc0, kc1);
+                    if (S == 2) eval_near<2, 4, MODE == WALK_HYBRID, KF>(partbuf, cnt, part, P, sk, eps2, kc0, kc1);
+                    else if (S == 3) eval_near<3, 4, MODE == WALK_HYBRID, KF>(partbuf, cnt, part, P, sk, eps2, kc0, kc1);
+                    else eval_near<4, 4, MODE == WALK_HYBRID, KF>(partbuf, cnt, part, P, sk, eps2, kc0, kc1);
                     npb = 0; flush_near = false;
                     __syncwarp();
                 }
