@@ -207,6 +207,16 @@ void hyb_run_host_release(void);
  * Errors: INVALID_ARG (theta-MAC tree, empty box), NO_TREE, CAPACITY_OVERFLOW (traversal stack). */
 int hyb_let_count(hyb_ctx *ctx, int32_t ndom, const float *h_boxes, uint64_t *h_counts);
 
+/* Total-energy diagnostic ("error in total energy of the system that is the sum of kinetic
+ * and potential energy") for the particles as they are in d_pos_m / d_vel now:
+ *   h_energy[0] = T = sum_i 1/2 m_i |v_i|^2
+ *   h_energy[1] = W = - G sum_{i<j} m_i m_j / sqrt(r_ij^2 + eps^2)   (potential of the unsplit force, Eq. 1-2)
+ * h_energy: HOST double[2].  W is a direct sum over all n (n - 1) / 2 pairs on the device (fp32 pair terms,
+ * fp64 accumulation, fixed summation order: repeated calls return the same bits); cost grows as n^2 (a
+ * fraction of a second at n = 2^20).  Needs no tree, changes nothing, synchronises.  With eps = 0 two
+ * coincident particles give W = -inf.  Errors: INVALID_ARG (NULL pointer), CUDA. */
+int hyb_energy(hyb_ctx *ctx, double *h_energy);
+
 /* Message for the last error on this context ("" if none).  ctx may be NULL (returns the
  * message of the last failed hyb_init / hyb_run_host on this thread). */
 const char *hyb_last_error(const hyb_ctx *ctx);

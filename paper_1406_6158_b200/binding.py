@@ -76,6 +76,8 @@ def lib():
         L.hyb_export.argtypes = [vp, C.c_int32, vp, C.c_size_t, C.POINTER(C.c_size_t)]
         L.hyb_run_host.restype = C.c_int
         L.hyb_run_host.argtypes = [C.POINTER(HybParams), C.c_int64, vp, vp, vp, vp, vp, C.c_int32, C.c_int, vp]
+        L.hyb_energy.restype = C.c_int
+        L.hyb_energy.argtypes = [vp, vp]
         L.hyb_let_count.restype = C.c_int
         L.hyb_let_count.argtypes = [vp, C.c_int32, vp, vp]
         L.hyb_run_host_release.restype = None
@@ -169,6 +171,12 @@ class Hyb:
         out = np.zeros((boxes.shape[0], 3), np.uint64)
         self._check(lib().hyb_let_count(self._h, boxes.shape[0], C.c_void_p(boxes.ctypes.data), C.c_void_p(out.ctypes.data)))
         return out
+
+    def energy(self):
+        """(T, W): kinetic and unsplit softened potential energy of the current state, fp64, summed on the device"""
+        out = np.zeros(2, np.float64)
+        self._check(lib().hyb_energy(self._h, C.c_void_p(out.ctypes.data)))
+        return float(out[0]), float(out[1])
 
     def sync(self):
         self._check(lib().hyb_sync(self._h))

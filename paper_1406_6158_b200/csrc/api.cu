@@ -526,6 +526,26 @@ int hyb_let_count(hyb_ctx *ctx, int32_t ndom, const float *h_boxes, uint64_t *h_
     return rc;
 }
 
+int hyb_energy(hyb_ctx *ctx, double *h_energy)
+{
+    Ctx *c = reinterpret_cast<Ctx *>(ctx);
+    if (!c) return fail(nullptr, HYB_ERR_INVALID_ARG, "ctx is NULL");
+    if (!h_energy) return fail(c, HYB_ERR_INVALID_ARG, "h_energy is NULL");
+    cudaSetDevice(c->device);
+    u32 ni, nj, nk;
+    const size_t nd = energy_scratch_doubles(c, &ni, &nj, &nk);
+    double *d = nullptr;
+    cudaError_t e = cudaMalloc(&d, nd * sizeof(double));
+    if (e != cudaSuccess) return cuda_fail(c, e, "cudaMalloc");
+    int rc = HYB_OK;
+    e = launch_energy(c, d, ni, nj, nk);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(h_energy, d, 2 * sizeof(double), cudaMemcpyDeviceToHost, c->stream);
+    if (e != cudaSuccess) rc = cuda_fail(c, e, "hyb_energy");
+    else { c->launches += 3; rc = hyb_sync(ctx); }
+    cudaFree(d);
+    return rc;
+}
+
 const char *hyb_last_error(const hyb_ctx *ctx)
 {
     const Ctx *c = reinterpret_cast<const Ctx *>(ctx);

@@ -141,6 +141,8 @@ cudaError_t launch_walk(Ctx *c, int mode);
 cudaError_t launch_kick_drift(Ctx *c, float c_soft, float c_hard, float dt_drift);
 cudaError_t launch_zero_acc(Ctx *c, hyb_float4 *a);
 cudaError_t launch_let_count(Ctx *c, int ndom, const float *d_boxes, unsigned long long *d_out);
+size_t energy_scratch_doubles(const Ctx *c, u32 *ni, u32 *nj, u32 *nk);
+cudaError_t launch_energy(Ctx *c, double *d_scratch, u32 ni, u32 nj, u32 nk);
 
 // ---- device helpers ------------------------------------------------------------------
 __device__ __forceinline__ u32 enc_float(float f)
