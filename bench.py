@@ -254,12 +254,13 @@ def main():
     if rank == 0 and not args.no_e2e:
         hp = torch.from_numpy(pos).pin_memory(); hv = torch.from_numpy(vel).pin_memory()
         hid = torch.arange(cfg.n, dtype=torch.int32).pin_memory()
+        has = torch.empty(cfg.n, 4).pin_memory(); hah = torch.empty(cfg.n, 4).pin_memory()      # results
         p0, v0 = hp.clone(), hv.clone()
         e_int, e_t = 0.0, 0.0
         for i in range(2 + 3):
             hp.copy_(p0); hv.copy_(v0)
             t0 = time.perf_counter()
-            _, _, it = hyb_run_host(P, hp.numpy(), hv.numpy(), hid.numpy(), 1, local_rank)
+            _, _, it = hyb_run_host(P, hp.numpy(), hv.numpy(), hid.numpy(), 1, local_rank, has.numpy(), hah.numpy())
             dt = time.perf_counter() - t0
             if i >= 2:
                 e_int += float(it.sum()); e_t += dt
@@ -267,7 +268,7 @@ def main():
         e2e = {"value": e_int / e_t, "unit": "interactions/s", "h2d_bytes_per_step": 36 * n,
                "d2h_bytes_per_step": 68 * n, "ms_per_call": 1e3 * e_t / 3,
                "what": "hyb_run_host: upload pos/vel/id, initial tree+forces, one soft cycle, download "
-                       "pos/vel/id/a_soft/a_hard; the device buffer is kept between calls (2 untimed calls first)"}
+                       "pos/vel/id/a_soft/a_hard; all host buffers pinned; the device buffer is kept between calls (2 untimed calls first)"}
 
     # ---- the same cycle with a plain (unsplit, theta-only) tree at dt_h: n_sub
     #      builds + n_sub full walks per cycle; reported beside the hybrid to show its compute ratio

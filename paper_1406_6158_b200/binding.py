@@ -95,11 +95,17 @@ def hyb_workspace_bytes(n: int, params: HybParams) -> int:
 
 
 def hyb_run_host(params: HybParams, pos_m: np.ndarray, vel: np.ndarray, ids: np.ndarray, n_soft_steps: int,
-                 device: int = 0):
+                 device: int = 0, a_soft: np.ndarray | None = None, a_hard: np.ndarray | None = None):
     """End-to-end call on HOST (NumPy / pinned torch) buffers; updates pos_m, vel, ids in place and
-    returns (a_soft, a_hard, interactions)."""
+    returns (a_soft, a_hard, interactions).  a_soft / a_hard: optional float32 [n,4] result buffers (pass
+    pinned ones to keep the download off the pageable-memory path); allocated here when omitted."""
     n = pos_m.shape[0]
-    a_soft = np.empty((n, 4), np.float32); a_hard = np.empty((n, 4), np.float32)
+    if a_soft is None:
+        a_soft = np.empty((n, 4), np.float32)
+    if a_hard is None:
+        a_hard = np.empty((n, 4), np.float32)
+    for a in (a_soft, a_hard):
+        assert a.dtype == np.float32 and a.shape == (n, 4) and a.flags.c_contiguous
     inter = np.zeros(2, np.uint64)
     p = lambda a: C.c_void_p(a.ctypes.data)  # noqa: E731
     rc = lib().hyb_run_host(C.byref(params), n, p(pos_m), p(vel), p(a_soft), p(a_hard), p(ids), n_soft_steps, device,
