@@ -67,6 +67,34 @@ struct DevCtl {
     u64 inter_soft, inter_hard, inter_hard_fused;   // pair counts: soft lists, hard lists (all walks), hard lists of fused walks
 };
 
+// Programmatic dependent launch, used between the passes of the radix sort (sort.cuh).  A kernel
+// launched with launch_pdl may become resident while the previous kernel of the stream is still running; it
+// starts with pdl_begin(), which waits until that kernel has completed and its writes are visible, and only
+// then lets the next launch_pdl kernel of the stream start early.  This hides the launch and
+// CTA-scheduling latency between short dependent kernels.  Rules: nothing is read from global memory before
+// pdl_begin(); and what the kernel reads through the non-coherent path (const __restrict__, __ldg) must not
+// have been read by the previous kernel at addresses that kernel also wrote (a stale L1 line could survive:
+// the previous kernel ran on the same SMs after this one's launch).  A radix pass only writes what the next
+// pass reads, so it qualifies; the other kernels of the build read and write shared control words and are
+// launched the ordinary way (pdl_begin() then returns at once).
+__device__ __forceinline__ void pdl_begin()
+{
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+}
+
+template <typename... Exp, typename... Act>
+static inline cudaError_t launch_pdl(void (*kern)(Exp...), dim3 grid, dim3 block, size_t smem, cudaStream_t st, Act &&...args)
+{
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = st;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at; cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, kern, static_cast<Exp>(args)...);
+}
+
 // One tree node as the walk reads it: 64 bytes, children of a cell are contiguous (T7).
 struct __align__(16) NodeRec {
     float4 A;        // centre of mass, mass (T9)

@@ -31,6 +31,7 @@ __global__ void __launch_bounds__(RS_THREADS) radix_pass_kernel(
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     RadixSmem &sm = *reinterpret_cast<RadixSmem *>(smem_raw);
+    pdl_begin();
     const u32 n = n_dev ? *n_dev : n_host;
     const u32 ntiles = (n + RS_TILE - 1) / RS_TILE;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -207,10 +208,8 @@ static cudaError_t launch_radix_pass(const KeyT *kin, const u32 *vin, KeyT *kout
         if (e != cudaSuccess) return e;
         attr_set = true;
     }
-    radix_pass_kernel<KeyT><<<grid, RS_THREADS, sizeof(RadixSmem), st>>>(kin, vin, kout, vout, inv_out, n_host, n_dev,
-                                                                         shift, digit_base, status, tiles_alloc,
-                                                                         tile_counter, dev_status);
-    return cudaGetLastError();
+    return launch_pdl(radix_pass_kernel<KeyT>, dim3((unsigned)grid), dim3(RS_THREADS), sizeof(RadixSmem), st, kin, vin, kout, vout,
+                      inv_out, n_host, n_dev, shift, digit_base, status, tiles_alloc, tile_counter, dev_status);
 }
 
 }  // namespace hyb
