@@ -32,11 +32,11 @@ Layout plan_workspace(int64_t n)
     size_t off = 0;
     auto take = [&](size_t bytes) { size_t o = off; off = align_up(off + bytes); return o; };
     const size_t N = (size_t)n, NC = (size_t)L.node_cap, GC = (size_t)L.group_cap;
-    L.ctl = take(sizeof(DevCtl));
     L.key_orig = take(8 * N); L.key_a = take(8 * N); L.key_b = take(8 * N);
     L.val_a = take(4 * N); L.val_b = take(4 * N);
     L.pos_tmp = take(16 * N); L.vel_tmp = take(16 * N); L.id_tmp = take(4 * N);
-    // cleared at the start of every build by ONE memset: [zero_begin, zero_end)
+    // cleared at the start of every build by ONE memset: the tail of the control block and [zero_begin, zero_end)
+    L.ctl = take(sizeof(DevCtl));
     L.rs_status = take(4 * 256 * (size_t)(L.rs_tiles + L.rs_blocks) * RS_PASSES);
     L.zero_begin = L.rs_status;
     L.sc_status = take(8 * (size_t)(L.sc_tiles + L.po_tiles));

@@ -43,17 +43,13 @@ constexpr int WK_PART_CAP = 192;         // K-weighted (near) particle buffer en
 
 enum WalkMode { WALK_HYBRID = 0, WALK_HARD = 1, WALK_NORMAL = 2 };
 
-// Device control block: lives at the start of the caller's workspace.
+// Device control block.  It sits in the workspace right in front of the look-back statuses, and its last
+// block of fields is what a build starts from zero: ONE memset per build clears from bbox_enc to the end of
+// the status arrays (Layout::zero_end).
 struct DevCtl {
     u32 status;
     u32 nn, ng;
     u32 level_offset[MAXLEVEL + 2];
-    // ---- reset at the start of every build (see reset_build_state) ----
-    u32 bbox_enc[6];            // order-preserving encodings: min xyz, max xyz
-    u32 digit_hist[RS_PASSES * 256];
-    u32 node_hist[256];
-    u32 tile_counter[16];       // dynamic tile ids, one slot per lookback kernel instance
-    u32 nn_total;               // un-clamped node count
     // ---- derived ----
     float bbox[6];
     double L, inv, origin[3];
@@ -61,10 +57,17 @@ struct DevCtl {
     u32 digit_base[RS_PASSES * 256];
     u32 node_base[256];
     // ---- walk ----
-    u32 group_counter;          // ---- walk work distribution: reset before every launch (2 words)
-    u32 nheavy;                 // sink ranges of split groups (hard walk)
+    // work distribution: launch k uses slot k & 1 and clears the other slot for launch k + 1 (no memset)
+    u32 group_counter[2];
+    u32 nheavy[2];              // sink ranges of split groups (hard walk)
     u32 walk_ng;                // number of groups of the last walk (is its nhard[] comparable?)
     u64 inter_soft, inter_hard, inter_hard_fused;   // pair counts: soft lists, hard lists (all walks), hard lists of fused walks
+    // ---- zero at the start of every build (keep last) ----
+    u32 bbox_enc[6];            // order-preserving encodings: ~min xyz, max xyz (atomicMax from 0 for both)
+    u32 digit_hist[RS_PASSES * 256];
+    u32 node_hist[256];
+    u32 tile_counter[16];       // dynamic tile ids, one slot per lookback kernel instance
+    u32 nn_total;               // un-clamped node count
 };
 
 // Programmatic dependent launch, used between the passes of the radix sort (sort.cuh).  A kernel
@@ -133,6 +136,7 @@ inline int64_t imin64(int64_t a, int64_t b) { return a < b ? a : b; }
 Layout plan_workspace(int64_t n);
 
 struct Ctx {
+    u32 walk_par = 0;           // slot of the walk work counters the next launch uses (DevCtl::group_counter)
     hyb_params p;
     int64_t n;
     int device;

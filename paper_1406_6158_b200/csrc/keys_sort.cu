@@ -11,7 +11,7 @@ __device__ void root_cube(DevCtl *ctl)
 {
     double L = 0.0;
     for (int a = 0; a < 3; a++) {
-        float lo = dec_float(ld_volatile_u32(&ctl->bbox_enc[a])), hi = dec_float(ld_volatile_u32(&ctl->bbox_enc[3 + a]));
+        float lo = dec_float(~ld_volatile_u32(&ctl->bbox_enc[a])), hi = dec_float(ld_volatile_u32(&ctl->bbox_enc[3 + a]));
         ctl->bbox[a] = lo; ctl->bbox[3 + a] = hi;
         double e = __dsub_rn((double)hi, (double)lo);
         if (e > L) L = e;
@@ -47,7 +47,8 @@ __global__ void __launch_bounds__(256) bbox_kernel(const float4 *__restrict__ po
     }
     if (__any_sync(0xFFFFFFFFu, bad) && (threadIdx.x & 31) == 0) atomicOr(&ctl->status, ST_NONFINITE);
     __syncthreads();
-    if (threadIdx.x < 3) atomicMin(&ctl->bbox_enc[threadIdx.x], s_enc[threadIdx.x]);
+    // the minima are kept complemented, so that both halves grow by atomicMax from the zero of the build's memset
+    if (threadIdx.x < 3) atomicMax(&ctl->bbox_enc[threadIdx.x], ~s_enc[threadIdx.x]);
     else if (threadIdx.x < 6) atomicMax(&ctl->bbox_enc[threadIdx.x], s_enc[threadIdx.x]);
     // the last CTA to get here sees every CTA's contribution and derives the root cube
     __threadfence();

@@ -570,10 +570,9 @@ cudaError_t launch_build_tree(Ctx *c)
     cudaStream_t st = c->stream;
     DevCtl *ctl = c->ctl;
     // reset per-build device state
-    cudaMemsetAsync(reinterpret_cast<char *>(ctl) + offsetof(DevCtl, bbox_enc), 0,
-                    offsetof(DevCtl, bbox) - offsetof(DevCtl, bbox_enc), st);
-    cudaMemsetAsync(reinterpret_cast<char *>(ctl) + offsetof(DevCtl, bbox_enc), 0xFF, 3 * sizeof(u32), st);
-    cudaMemsetAsync(c->ws + L.zero_begin, 0, L.zero_end - L.zero_begin, st);     // look-back statuses, group flags
+    // one memset: the build block of the control words, the look-back statuses and the group flags
+    char *zb = reinterpret_cast<char *>(ctl) + offsetof(DevCtl, bbox_enc);
+    cudaMemsetAsync(zb, 0, (size_t)((c->ws + L.zero_end) - zb), st);
 
     cudaError_t e = launch_keys_sort_permute(c);
     if (e != cudaSuccess) return e;

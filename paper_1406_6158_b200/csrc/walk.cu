@@ -30,6 +30,7 @@ struct WalkArgs {
     const float4 *glo, *ghi;
     u32 *ncell, *npart, *nhard;
     const u32 *heavy;             // hard walk: sink ranges of split groups (see split_kernel)
+    u32 par;                      // which slot of DevCtl::group_counter / nheavy this launch uses
     const u32 *ganc;              // hard walk: start node of every group (octree.cu, ganc_kernel)
     const unsigned char *is_split; // hard walk: group is handled as ranges
     float4 *a_soft, *a_hard;
@@ -412,7 +413,10 @@ __global__ void __launch_bounds__(WK_WARPS * 32, SmemLayout<MODE>::ctas_per_sm) 
 
     const u32 lt_mask = (1u << lane) - 1u;
     const u32 ng = a.ctl->ng;
-    if (blockIdx.x == 0 && threadIdx.x == 0) a.ctl->walk_ng = ng;      // read by the next split_kernel
+    if (blockIdx.x == 0 && threadIdx.x == 0) {
+        a.ctl->walk_ng = ng;                                            // read by the next split_kernel
+        a.ctl->group_counter[a.par ^ 1u] = 0u; a.ctl->nheavy[a.par ^ 1u] = 0u;      // the next launch's slots
+    }
     const float rout2 = __fmul_rn(a.rout, a.rout);
     const float eps2 = a.eps2, kc0 = a.kc0, kc1 = a.kc1;
     unsigned long long isoft = 0, ihard = 0;
@@ -423,15 +427,15 @@ __global__ void __launch_bounds__(WK_WARPS * 32, SmemLayout<MODE>::ctas_per_sm) 
     // Every range walks with the box of the WHOLE group, so its lists are the group's lists (T12-T13);
     // only the sinks differ.
     constexpr bool SPLIT = MODE == WALK_HARD;
-    const u32 nheavy = SPLIT ? a.ctl->nheavy : 0u;
+    const u32 nheavy = SPLIT ? a.ctl->nheavy[a.par] : 0u;
     const u32 nitems = ng + nheavy;
     u32 item = 0;
-    if (lane == 0) item = atomicAdd(&a.ctl->group_counter, 1u);
+    if (lane == 0) item = atomicAdd(&a.ctl->group_counter[a.par], 1u);
     item = __shfl_sync(FULL, item, 0);
 
     while (item < nitems) {
         u32 item_next = 0;
-        if (lane == 0) item_next = atomicAdd(&a.ctl->group_counter, 1u);      // consumed at the end of this item
+        if (lane == 0) item_next = atomicAdd(&a.ctl->group_counter[a.par], 1u);      // consumed at the end of this item
         u32 g, rsub = 0, nsub = 1;
         if (SPLIT && item < nheavy) {
             const u32 it = __ldg(a.heavy + item);
@@ -741,7 +745,8 @@ __global__ void __launch_bounds__(WK_WARPS * 32, SmemLayout<MODE>::ctas_per_sm) 
 // in the ordinary sequence.
 __global__ void __launch_bounds__(256) split_kernel(DevCtl *ctl, const u32 *__restrict__ gcount,
                                                     const u32 *__restrict__ nhard, u32 *__restrict__ heavy,
-                                                    unsigned char *__restrict__ is_split, unsigned long long t2, unsigned long long t4)
+                                                    unsigned char *__restrict__ is_split, unsigned long long t2, unsigned long long t4,
+                                                    u32 par)
 {
     const u32 ng = ctl->ng, prev = ctl->walk_ng;
     // the estimate is only meaningful when the previous walk had about the same groups
@@ -753,7 +758,7 @@ __global__ void __launch_bounds__(256) split_kernel(DevCtl *ctl, const u32 *__re
         if (est >= t4 && n >= 32u) nsub = 4;
         else if (est >= t2 && n >= 16u) nsub = 2;
         if (nsub > 1) {
-            const u32 at = atomicAdd(&ctl->nheavy, nsub);
+            const u32 at = atomicAdd(&ctl->nheavy[par], nsub);
             for (u32 i = 0; i < nsub; i++) heavy[at + i] = g | (i << 28) | ((nsub - 1u) << 30);
         }
         is_split[g] = nsub > 1;
@@ -810,11 +815,11 @@ cudaError_t launch_walk(Ctx *c, int mode)
     a.heavy = wsptr<u32>(c, L.splitq);
     a.ganc = c->tree_refit ? nullptr : wsptr<u32>(c, L.ganc);      // refitted boxes: the Morton cells are stale
     a.is_split = wsptr<unsigned char>(c, L.gflag);      // the build's flag array is free between builds
-    cudaMemsetAsync(&c->ctl->group_counter, 0, 2 * sizeof(u32), c->stream);      // counter, nheavy
+    a.par = c->walk_par; c->walk_par ^= 1u;      // both slots start at zero (hyb_init); each walk clears the other one
     if (mode == WALK_HARD)
         split_kernel<<<(int)imin64((c->n + 255) / 256, (int64_t)c->num_sms * 4), 256, 0, c->stream>>>(
             c->ctl, a.gcount, a.nhard, wsptr<u32>(c, L.splitq), wsptr<unsigned char>(c, L.gflag),
-            WK_SPLIT2, WK_SPLIT4);
+            WK_SPLIT2, WK_SPLIT4, a.par);
     const bool poly7 = c->p.kfunc == HYB_K_POLY7, tree = c->p.hard_tree != 0;
     if (mode == WALK_NORMAL) return launch_walk_mode<WALK_NORMAL, HYB_K_PAPER, false>(c, a);
     if (mode == WALK_HYBRID) {
