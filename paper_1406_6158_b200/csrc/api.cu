@@ -103,8 +103,18 @@ static int status_to_error(Ctx *c, u32 st)
     return HYB_OK;
 }
 
+// a box reduced by a drift that no build consumed (a step that failed in between): drop it, the positions
+// are the caller's and may have changed
+static void discard_pending_bbox(Ctx *c)
+{
+    if (!c->bbox_ready) return;
+    cudaMemsetAsync(&c->ctl->bbox_enc[0], 0, 7 * sizeof(u32), c->stream);      // bbox_enc[6], bbox_done
+    c->bbox_ready = false;
+}
+
 static int do_build(Ctx *c, bool hard_only = false)
 {
+    const bool had_bbox = c->bbox_ready;
     // HYB_GROUP_AUTO: runs of sibling cells, of up to group_max sinks for the soft walk and up to
     // group_max / 2 when only a hard walk follows
     c->grouping_now = c->p.grouping == HYB_GROUP_AUTO ? HYB_GROUP_SIBLINGS : c->p.grouping;
@@ -119,7 +129,7 @@ static int do_build(Ctx *c, bool hard_only = false)
     c->acc_valid = false;
     // bbox (+ root cube), keys, digit bases, 8 sort passes, permute | preorder (+ level offsets), level sort,
     // link, upsweep, group mark / scan / info (+ b_max, r_b in absolute-MAC mode)
-    c->launches += 12 + 7 + (c->p.mac == HYB_MAC_ABS && !hard_only ? 2 : 0) + (c->p.split ? 1 : 0);     // + ganc
+    c->launches += 12 + 7 + (c->p.mac == HYB_MAC_ABS && !hard_only ? 2 : 0) + (c->p.split ? 1 : 0) - (had_bbox ? 1 : 0);     // + ganc
     return HYB_OK;
 }
 
@@ -244,6 +254,7 @@ int hyb_build_tree(hyb_ctx *ctx)
     Ctx *c = reinterpret_cast<Ctx *>(ctx);
     if (!c) return fail(nullptr, HYB_ERR_INVALID_ARG, "ctx is NULL");
     cudaSetDevice(c->device);
+    discard_pending_bbox(c);
     return do_build(c);
 }
 
@@ -299,6 +310,7 @@ int hyb_step(hyb_ctx *ctx, int32_t n_soft_steps)
     const int nsub = c->p.n_sub;
     const float dts = c->p.dt_soft, dth = dts / (float)nsub;
     int rc;
+    discard_pending_bbox(c);
     if (!c->acc_valid || (c->p.hard_refit && (!c->tree_valid || c->tree_refit))) {
         if ((rc = do_build(c)) != HYB_OK) return rc;
         if ((rc = do_soft(c)) != HYB_OK) return rc;
@@ -316,11 +328,12 @@ int hyb_step(hyb_ctx *ctx, int32_t n_soft_steps)
             // Inside a cycle the closing half kick of one substep and the opening half kick of the next
             // use the same acceleration, so they are one full kick fused with the drift (k > 0).
             const float open_c = k == 0 ? 0.5f * dth : dth;
-            if (split) e = launch_kick_drift(c, k == 0 ? 0.5f * dts : 0.0f, open_c, dth);
-            else e = launch_kick_drift(c, open_c, 0.0f, dth);
+            const bool soft_step = !split || k == nsub - 1;
+            const bool rebuild = soft_step || !c->p.hard_refit;      // a full build follows: the drift reduces its bounding box
+            if (split) e = launch_kick_drift(c, k == 0 ? 0.5f * dts : 0.0f, open_c, dth, rebuild);
+            else e = launch_kick_drift(c, open_c, 0.0f, dth, rebuild);
             if (e != cudaSuccess) return cuda_fail(c, e, "kick_drift");
             cudaEvent_t e1 = c->timing ? ev() : nullptr;
-            const bool soft_step = !split || k == nsub - 1;
             if (!soft_step && c->p.hard_refit) rc = do_refit(c, k == 0 && c->p.grouping == HYB_GROUP_AUTO);
             else rc = do_build(c, !soft_step);
             if (rc != HYB_OK) return rc;

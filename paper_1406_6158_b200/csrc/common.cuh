@@ -44,7 +44,7 @@ constexpr int WK_PART_CAP = 192;         // K-weighted (near) particle buffer en
 enum WalkMode { WALK_HYBRID = 0, WALK_HARD = 1, WALK_NORMAL = 2 };
 
 // Device control block.  It sits in the workspace right in front of the look-back statuses, and its last
-// block of fields is what a build starts from zero: ONE memset per build clears from bbox_enc to the end of
+// block of fields is what a build starts from zero: ONE memset per build clears from build_zero_begin to the end of
 // the status arrays (Layout::zero_end).
 struct DevCtl {
     u32 status;
@@ -62,8 +62,11 @@ struct DevCtl {
     u32 nheavy[2];              // sink ranges of split groups (hard walk)
     u32 walk_ng;                // number of groups of the last walk (is its nhard[] comparable?)
     u64 inter_soft, inter_hard, inter_hard_fused;   // pair counts: soft lists, hard lists (all walks), hard lists of fused walks
-    // ---- zero at the start of every build (keep last) ----
+    // ---- bounding box reduction: filled by bbox_kernel or by the drift, cleared again by keys_kernel ----
     u32 bbox_enc[6];            // order-preserving encodings: ~min xyz, max xyz (atomicMax from 0 for both)
+    u32 bbox_done;              // CTAs that have contributed (the last one derives the root cube)
+    // ---- zero at the start of every build (keep last) ----
+    u32 build_zero_begin;       // (marks the start of the memset range)
     u32 digit_hist[RS_PASSES * 256];
     u32 node_hist[256];
     u32 tile_counter[16];       // dynamic tile ids, one slot per lookback kernel instance
@@ -136,6 +139,7 @@ inline int64_t imin64(int64_t a, int64_t b) { return a < b ? a : b; }
 Layout plan_workspace(int64_t n);
 
 struct Ctx {
+    bool bbox_ready = false;    // the last drift has already reduced the bounding box of the current positions
     u32 walk_par = 0;           // slot of the walk work counters the next launch uses (DevCtl::group_counter)
     hyb_params p;
     int64_t n;
@@ -170,7 +174,7 @@ cudaError_t launch_build_tree(Ctx *c);
 cudaError_t launch_regroup(Ctx *c);        // sink groups again (group_max_now / grouping_now) on the existing topology
 cudaError_t launch_refit_tree(Ctx *c);     // tight boxes of nodes and groups for the current positions, same topology
 cudaError_t launch_walk(Ctx *c, int mode);
-cudaError_t launch_kick_drift(Ctx *c, float c_soft, float c_hard, float dt_drift);
+cudaError_t launch_kick_drift(Ctx *c, float c_soft, float c_hard, float dt_drift, bool with_bbox = false);
 cudaError_t launch_zero_acc(Ctx *c, hyb_float4 *a);
 cudaError_t launch_let_count(Ctx *c, int ndom, const float *d_boxes, unsigned long long *d_out);
 size_t energy_scratch_doubles(const Ctx *c, u32 *ni, u32 *nj, u32 *nk);
@@ -193,6 +197,52 @@ __device__ __forceinline__ u32 ld_volatile_u32(const u32 *p)
 __device__ __forceinline__ u64 ld_volatile_u64(const u64 *p)
 {
     return *reinterpret_cast<const volatile u64 *>(p);
+}
+
+// a1 (T1-T3): bounding box of the particles and the root cube.  Every thread brings the minima / maxima and
+// the validity of the particles it has seen; the block combines them, adds them to the control block, and the
+// last block to arrive derives the root cube.  Used by bbox_kernel and by the drift (integrate.cu), which
+// sees every new position anyway.  All threads of the block must call it (256 threads).
+__device__ __forceinline__ void root_cube(DevCtl *ctl)
+{
+    double L = 0.0;
+    for (int a = 0; a < 3; a++) {
+        float lo = dec_float(~ld_volatile_u32(&ctl->bbox_enc[a])), hi = dec_float(ld_volatile_u32(&ctl->bbox_enc[3 + a]));
+        ctl->bbox[a] = lo; ctl->bbox[3 + a] = hi;
+        double e = __dsub_rn((double)hi, (double)lo);
+        if (e > L) L = e;
+        ctl->origin[a] = (double)lo;
+    }
+    if (!(L > 0.0) || !isfinite(L)) L = 1.0;
+    ctl->L = L;
+    ctl->inv = __ddiv_rn(2097152.0, L);
+    ctl->Lf = __double2float_rn(L);
+}
+
+__device__ __forceinline__ void bbox_block_reduce(const float lo[3], const float hi[3], bool bad, DevCtl *ctl)
+{
+    __shared__ u32 s_enc[6];
+    if (threadIdx.x < 3) s_enc[threadIdx.x] = 0xFFFFFFFFu;
+    else if (threadIdx.x < 6) s_enc[threadIdx.x] = 0u;
+    __syncthreads();
+#pragma unroll
+    for (int a = 0; a < 3; a++) {
+        u32 mn = __reduce_min_sync(0xFFFFFFFFu, enc_float(lo[a]));
+        u32 mx = __reduce_max_sync(0xFFFFFFFFu, enc_float(hi[a]));
+        if ((threadIdx.x & 31) == 0) { atomicMin(&s_enc[a], mn); atomicMax(&s_enc[3 + a], mx); }
+    }
+    if (__any_sync(0xFFFFFFFFu, bad) && (threadIdx.x & 31) == 0) atomicOr(&ctl->status, ST_NONFINITE);
+    __syncthreads();
+    // the minima are kept complemented, so that both halves grow by atomicMax from zero
+    if (threadIdx.x < 3) atomicMax(&ctl->bbox_enc[threadIdx.x], ~s_enc[threadIdx.x]);
+    else if (threadIdx.x < 6) atomicMax(&ctl->bbox_enc[threadIdx.x], s_enc[threadIdx.x]);
+    // the last CTA to get here sees every CTA's contribution and derives the root cube
+    __threadfence();
+    __syncthreads();
+    if (threadIdx.x == 0 && atomicAdd(&ctl->bbox_done, 1u) == gridDim.x - 1) {
+        __threadfence();
+        root_cube(ctl);
+    }
 }
 
 // Decoupled look-back over one value per tile (status word: bits 63..62 flag, low 62 bits value).

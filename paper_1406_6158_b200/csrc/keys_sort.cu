@@ -6,24 +6,6 @@
 namespace hyb {
 
 // ------------------------------------------------------------------ a1: bounding box (T1, T2)
-// T3: root cube.  One thread (of the last CTA of bbox_kernel to finish).
-__device__ void root_cube(DevCtl *ctl)
-{
-    double L = 0.0;
-    for (int a = 0; a < 3; a++) {
-        float lo = dec_float(~ld_volatile_u32(&ctl->bbox_enc[a])), hi = dec_float(ld_volatile_u32(&ctl->bbox_enc[3 + a]));
-        ctl->bbox[a] = lo; ctl->bbox[3 + a] = hi;
-        double e = __dsub_rn((double)hi, (double)lo);
-        if (e > L) L = e;
-        ctl->origin[a] = (double)lo;
-    }
-    if (!(L > 0.0) || !isfinite(L)) L = 1.0;
-    ctl->L = L;
-    ctl->inv = __ddiv_rn(2097152.0, L);
-    ctl->Lf = __double2float_rn(L);
-}
-
-
 __global__ void __launch_bounds__(256) bbox_kernel(const float4 *__restrict__ pos, u32 n, DevCtl *ctl)
 {
     float lo[3] = {INFINITY, INFINITY, INFINITY}, hi[3] = {-INFINITY, -INFINITY, -INFINITY};
@@ -35,28 +17,7 @@ __global__ void __launch_bounds__(256) bbox_kernel(const float4 *__restrict__ po
         lo[1] = fminf(lo[1], p.y); hi[1] = fmaxf(hi[1], p.y);
         lo[2] = fminf(lo[2], p.z); hi[2] = fmaxf(hi[2], p.z);
     }
-    __shared__ u32 s_enc[6];
-    if (threadIdx.x < 3) s_enc[threadIdx.x] = 0xFFFFFFFFu;
-    else if (threadIdx.x < 6) s_enc[threadIdx.x] = 0u;
-    __syncthreads();
-#pragma unroll
-    for (int a = 0; a < 3; a++) {
-        u32 mn = __reduce_min_sync(0xFFFFFFFFu, enc_float(lo[a]));
-        u32 mx = __reduce_max_sync(0xFFFFFFFFu, enc_float(hi[a]));
-        if ((threadIdx.x & 31) == 0) { atomicMin(&s_enc[a], mn); atomicMax(&s_enc[3 + a], mx); }
-    }
-    if (__any_sync(0xFFFFFFFFu, bad) && (threadIdx.x & 31) == 0) atomicOr(&ctl->status, ST_NONFINITE);
-    __syncthreads();
-    // the minima are kept complemented, so that both halves grow by atomicMax from the zero of the build's memset
-    if (threadIdx.x < 3) atomicMax(&ctl->bbox_enc[threadIdx.x], ~s_enc[threadIdx.x]);
-    else if (threadIdx.x < 6) atomicMax(&ctl->bbox_enc[threadIdx.x], s_enc[threadIdx.x]);
-    // the last CTA to get here sees every CTA's contribution and derives the root cube
-    __threadfence();
-    __syncthreads();
-    if (threadIdx.x == 0 && atomicAdd(&ctl->tile_counter[11], 1u) == gridDim.x - 1) {
-        __threadfence();
-        root_cube(ctl);
-    }
+    bbox_block_reduce(lo, hi, bad, ctl);
 }
 
 // ------------------------------------------------------------------ a2: keys (T4, T5)
@@ -84,6 +45,8 @@ __global__ void __launch_bounds__(256) keys_kernel(const float4 *__restrict__ po
 {
     __shared__ u32 hist[RS_PASSES * 256];
     for (int i = threadIdx.x; i < RS_PASSES * 256; i += blockDim.x) hist[i] = 0;
+    // the box reduction has been consumed (root cube derived): clear it for the next bbox_kernel / drift
+    if (blockIdx.x == 0 && threadIdx.x < 7) (&ctl->bbox_enc[0])[threadIdx.x] = 0u;      // bbox_enc[6], bbox_done
     __syncthreads();
     const double ox = ctl->origin[0], oy = ctl->origin[1], oz = ctl->origin[2], inv = ctl->inv;
     for (u32 i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
@@ -138,7 +101,9 @@ cudaError_t launch_keys_sort_permute(Ctx *c)
     DevCtl *ctl = c->ctl;
     const int grid = (int)imin64((c->n + 255) / 256, (int64_t)c->num_sms * 8);
 
-    bbox_kernel<<<grid, 256, 0, st>>>(reinterpret_cast<const float4 *>(c->pos), n, ctl);
+    // the drift of hyb_step has already reduced the box of the positions it wrote (integrate.cu)
+    if (!c->bbox_ready) bbox_kernel<<<grid, 256, 0, st>>>(reinterpret_cast<const float4 *>(c->pos), n, ctl);
+    c->bbox_ready = false;
     u64 *key_orig = wsptr<u64>(c, L.key_orig), *key_a = wsptr<u64>(c, L.key_a), *key_b = wsptr<u64>(c, L.key_b);
     u32 *val_a = wsptr<u32>(c, L.val_a), *val_b = wsptr<u32>(c, L.val_b);
     // few CTAs: every CTA ends with up to 2048 global atomics for its share of the digit histograms

@@ -571,7 +571,7 @@ cudaError_t launch_build_tree(Ctx *c)
     DevCtl *ctl = c->ctl;
     // reset per-build device state
     // one memset: the build block of the control words, the look-back statuses and the group flags
-    char *zb = reinterpret_cast<char *>(ctl) + offsetof(DevCtl, bbox_enc);
+    char *zb = reinterpret_cast<char *>(ctl) + offsetof(DevCtl, build_zero_begin);
     cudaMemsetAsync(zb, 0, (size_t)((c->ws + L.zero_end) - zb), st);
 
     cudaError_t e = launch_keys_sort_permute(c);
