@@ -166,7 +166,7 @@ static int do_hard(Ctx *c)
 {
     cudaError_t e = c->p.split ? launch_walk(c, WALK_HARD) : launch_zero_acc(c, c->a_hard);
     if (e != cudaSuccess) return cuda_fail(c, e, "hard walk");
-    c->launches += c->p.split ? 2 : 1;          // split_kernel + walk, or the zero fill
+    c->launches += 1;                           // the walk (launch_walk counts a split_kernel), or the zero fill
     return HYB_OK;
 }
 

@@ -139,6 +139,8 @@ inline int64_t imin64(int64_t a, int64_t b) { return a < b ? a : b; }
 Layout plan_workspace(int64_t n);
 
 struct Ctx {
+    bool split_ready = false;   // ganc_kernel has already queued the heavy groups for the walk that uses slot split_par
+    u32 split_par = 0;
     bool bbox_ready = false;    // the last drift has already reduced the bounding box of the current positions
     u32 walk_par = 0;           // slot of the walk work counters the next launch uses (DevCtl::group_counter)
     hyb_params p;
@@ -243,6 +245,25 @@ __device__ __forceinline__ void bbox_block_reduce(const float lo[3], const float
         __threadfence();
         root_cube(ctl);
     }
+}
+
+// Hard walk scheduling: a group whose hard list was long at the previous walk (n x nhard of the group with the
+// same index -- an estimate that only steers the order of work, never the result) is cut into 2 or 4 sink
+// ranges, which are queued in front of everything else; the walk skips it in the ordinary sequence.
+// Called once per group by ganc_kernel (during the build, off the critical path) or by split_kernel.
+constexpr unsigned long long WK_SPLIT2 = 24576ull, WK_SPLIT4 = 65536ull;
+__device__ __forceinline__ void split_group(DevCtl *ctl, u32 g, u32 n, u32 h_prev, bool comparable, u32 *__restrict__ heavy,
+                                            unsigned char *__restrict__ is_split, u32 par)
+{
+    const unsigned long long est = (unsigned long long)n * (unsigned long long)(comparable ? h_prev : 0u);
+    u32 nsub = 1;
+    if (est >= WK_SPLIT4 && n >= 32u) nsub = 4;
+    else if (est >= WK_SPLIT2 && n >= 16u) nsub = 2;
+    if (nsub > 1) {
+        const u32 at = atomicAdd(&ctl->nheavy[par], nsub);
+        for (u32 i = 0; i < nsub; i++) heavy[at + i] = g | (i << 28) | ((nsub - 1u) << 30);
+    }
+    is_split[g] = nsub > 1;
 }
 
 // Decoupled look-back over one value per tile (status word: bits 63..62 flag, low 62 bits value).

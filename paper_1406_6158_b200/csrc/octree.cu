@@ -537,11 +537,17 @@ __device__ __forceinline__ u32 quantise_d(double x, double o, double inv)
 __global__ void __launch_bounds__(256) ganc_kernel(const DevCtl *__restrict__ ctl, const u32 *__restrict__ gnode,
                                                    const float4 *__restrict__ glo, const float4 *__restrict__ ghi,
                                                    const unsigned char *__restrict__ level, const u32 *__restrict__ parent,
-                                                   float r_out, u32 *__restrict__ ganc)
+                                                   float r_out, u32 *__restrict__ ganc, DevCtl *ctl_rw,
+                                                   const u32 *__restrict__ gcount, const u32 *__restrict__ nhard_prev,
+                                                   u32 *__restrict__ heavy, unsigned char *__restrict__ is_split, u32 par)
 {
     const u32 ng = ctl->ng;
     const u32 g = blockIdx.x * blockDim.x + threadIdx.x;
     if (g >= ng) return;
+    {   // work order of the next hard walk (the group flags of the build are free again by now)
+        const u32 prev = ctl->walk_ng;
+        split_group(ctl_rw, g, gcount[g], nhard_prev[g], (prev > ng ? prev - ng : ng - prev) <= ng / 16u, heavy, is_split, par);
+    }
     const float4 lo = glo[g], hi = ghi[g];
     const double inv = ctl->inv;
     int lstar = MAXLEVEL;
@@ -614,10 +620,16 @@ cudaError_t launch_build_tree(Ctx *c)
                                                  wsptr<u32>(c, L.gnode));
     ginfo_kernel<<<(int)imin64((c->n + 255) / 256, (int64_t)c->num_sms * 8), 256, 0, ax>>>(
         ctl, n, pos_t, gfirst, wsptr<u32>(c, L.gcount), wsptr<float4>(c, L.glo), wsptr<float4>(c, L.ghi));
-    if (c->p.split)
+    c->split_ready = false;
+    if (c->p.split) {
+        // + the work order of the next hard walk (split_group), for the counter slot that walk will use
         ganc_kernel<<<(int)((L.group_cap + 255) / 256), 256, 0, ax>>>(ctl, wsptr<u32>(c, L.gnode), wsptr<float4>(c, L.glo),
                                                                      wsptr<float4>(c, L.ghi), level, parent, c->p.r_out,
-                                                                     wsptr<u32>(c, L.ganc));
+                                                                     wsptr<u32>(c, L.ganc), ctl, wsptr<u32>(c, L.gcount),
+                                                                     wsptr<u32>(c, L.nhard), wsptr<u32>(c, L.splitq), gflag,
+                                                                     c->walk_par);
+        c->split_ready = true; c->split_par = c->walk_par;
+    }
     cudaEventRecord(c->ev_groups, ax);
 
     NodeArrays na;
@@ -651,6 +663,7 @@ cudaError_t launch_regroup(Ctx *c)
     const u32 n = (u32)c->n;
     cudaStream_t st = c->stream;
     DevCtl *ctl = c->ctl;
+    c->split_ready = false;                      // the flag array is re-used below
     cudaMemsetAsync(c->ws + L.gflag, 0, (size_t)n, st);
     cudaMemsetAsync(c->ws + L.sc_status + sizeof(u64) * (size_t)L.po_tiles, 0, sizeof(u64) * (size_t)L.sc_tiles, st);
     cudaMemsetAsync(&ctl->tile_counter[9], 0, sizeof(u32), st);

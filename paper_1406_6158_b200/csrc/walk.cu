@@ -43,7 +43,6 @@ constexpr int WK_SMAX = 4;          // most sinks per lane
 constexpr int WK_PAD_SLACK = 64;    // spare buffer entries for padding to a multiple of P U (<= 16 * 4)
 constexpr u32 FULL = 0xFFFFFFFFu;
 // hard walk: estimated pair count (members x hard-list length) above which a group is cut in 2 / 4 ranges
-constexpr unsigned long long WK_SPLIT2 = 24576ull, WK_SPLIT4 = 65536ull;
 constexpr u32 DESC_MASK = 0x1FFFFFFFu;      // node index bits of a stack descriptor
 
 template <int MODE>
@@ -739,30 +738,17 @@ __global__ void __launch_bounds__(WK_WARPS * 32, SmemLayout<MODE>::ctas_per_sm) 
     }
 }
 
-// Hard walk scheduling: a group whose hard list was long at the previous walk (n x nhard of the group
-// with the same index -- an estimate that only steers the order of work, never the result) is cut
-// into 2 or 4 sink ranges, which are queued in front of everything else; the walk skips it
-// in the ordinary sequence.
+// Hard walk scheduling (split_group, common.cuh) for a walk whose tree build has not done it: a second
+// hyb_hard_force on the same tree, or a refitted tree.
 __global__ void __launch_bounds__(256) split_kernel(DevCtl *ctl, const u32 *__restrict__ gcount,
                                                     const u32 *__restrict__ nhard, u32 *__restrict__ heavy,
-                                                    unsigned char *__restrict__ is_split, unsigned long long t2, unsigned long long t4,
-                                                    u32 par)
+                                                    unsigned char *__restrict__ is_split, u32 par)
 {
     const u32 ng = ctl->ng, prev = ctl->walk_ng;
     // the estimate is only meaningful when the previous walk had about the same groups
     const bool comparable = (prev > ng ? prev - ng : ng - prev) <= ng / 16u;
-    for (u32 g = blockIdx.x * blockDim.x + threadIdx.x; g < ng; g += gridDim.x * blockDim.x) {
-        const u32 n = gcount[g], h = comparable ? nhard[g] : 0u;
-        const unsigned long long est = (unsigned long long)n * (unsigned long long)h;
-        u32 nsub = 1;
-        if (est >= t4 && n >= 32u) nsub = 4;
-        else if (est >= t2 && n >= 16u) nsub = 2;
-        if (nsub > 1) {
-            const u32 at = atomicAdd(&ctl->nheavy[par], nsub);
-            for (u32 i = 0; i < nsub; i++) heavy[at + i] = g | (i << 28) | ((nsub - 1u) << 30);
-        }
-        is_split[g] = nsub > 1;
-    }
+    for (u32 g = blockIdx.x * blockDim.x + threadIdx.x; g < ng; g += gridDim.x * blockDim.x)
+        split_group(ctl, g, gcount[g], nhard[g], comparable, heavy, is_split, par);
 }
 
 __global__ void zero_acc_kernel(float4 *a, u32 n)
@@ -816,10 +802,12 @@ cudaError_t launch_walk(Ctx *c, int mode)
     a.ganc = c->tree_refit ? nullptr : wsptr<u32>(c, L.ganc);      // refitted boxes: the Morton cells are stale
     a.is_split = wsptr<unsigned char>(c, L.gflag);      // the build's flag array is free between builds
     a.par = c->walk_par; c->walk_par ^= 1u;      // both slots start at zero (hyb_init); each walk clears the other one
-    if (mode == WALK_HARD)
+    if (mode == WALK_HARD && !(c->split_ready && c->split_par == a.par)) {
         split_kernel<<<(int)imin64((c->n + 255) / 256, (int64_t)c->num_sms * 4), 256, 0, c->stream>>>(
-            c->ctl, a.gcount, a.nhard, wsptr<u32>(c, L.splitq), wsptr<unsigned char>(c, L.gflag),
-            WK_SPLIT2, WK_SPLIT4, a.par);
+            c->ctl, a.gcount, a.nhard, wsptr<u32>(c, L.splitq), wsptr<unsigned char>(c, L.gflag), a.par);
+        c->launches += 1;
+    }
+    c->split_ready = false;
     const bool poly7 = c->p.kfunc == HYB_K_POLY7, tree = c->p.hard_tree != 0;
     if (mode == WALK_NORMAL) return launch_walk_mode<WALK_NORMAL, HYB_K_PAPER, false>(c, a);
     if (mode == WALK_HYBRID) {
