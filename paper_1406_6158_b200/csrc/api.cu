@@ -129,7 +129,7 @@ static int do_build(Ctx *c, bool hard_only = false)
     c->acc_valid = false;
     // bbox (+ root cube), keys, digit bases, 8 sort passes, permute | preorder (+ level offsets), level sort,
     // link, upsweep, group mark / scan / info (+ b_max, r_b in absolute-MAC mode)
-    c->launches += 12 + 7 + (c->p.mac == HYB_MAC_ABS && !hard_only ? 2 : 0) + (c->p.split ? 1 : 0) - (had_bbox ? 1 : 0);     // + ganc
+    c->launches += 12 + 7 + (c->p.mac == HYB_MAC_ABS && !hard_only ? 2 : 0) - (had_bbox ? 1 : 0);
     return HYB_OK;
 }
 

@@ -139,7 +139,7 @@ inline int64_t imin64(int64_t a, int64_t b) { return a < b ? a : b; }
 Layout plan_workspace(int64_t n);
 
 struct Ctx {
-    bool split_ready = false;   // ganc_kernel has already queued the heavy groups for the walk that uses slot split_par
+    bool split_ready = false;   // ginfo_kernel has already queued the heavy groups for the walk that uses slot split_par
     u32 split_par = 0;
     bool bbox_ready = false;    // the last drift has already reduced the bounding box of the current positions
     u32 walk_par = 0;           // slot of the walk work counters the next launch uses (DevCtl::group_counter)
@@ -250,7 +250,7 @@ __device__ __forceinline__ void bbox_block_reduce(const float lo[3], const float
 // Hard walk scheduling: a group whose hard list was long at the previous walk (n x nhard of the group with the
 // same index -- an estimate that only steers the order of work, never the result) is cut into 2 or 4 sink
 // ranges, which are queued in front of everything else; the walk skips it in the ordinary sequence.
-// Called once per group by ganc_kernel (during the build, off the critical path) or by split_kernel.
+// Called once per group by ginfo_kernel (during the build, off the critical path) or by split_kernel.
 constexpr unsigned long long WK_SPLIT2 = 24576ull, WK_SPLIT4 = 65536ull;
 __device__ __forceinline__ void split_group(DevCtl *ctl, u32 g, u32 n, u32 h_prev, bool comparable, u32 *__restrict__ heavy,
                                             unsigned char *__restrict__ is_split, u32 par)

@@ -269,6 +269,7 @@ __global__ void __launch_bounds__(128) upsweep_kernel(NodeArrays na, const float
     const float Lf = ctl->Lf;
     u32 b = blockIdx.x * blockDim.x + threadIdx.x;
     if (b >= nn || na.child[b] != NOCHILD) return;
+    u32 par = na.parent[b];            // requested now, needed after the leaf sums
     // ---- leaf: sequential sums over its particles, ascending (T9)
     {
         const u32 f = na.first[b], c = na.count[b];
@@ -306,12 +307,11 @@ __global__ void __launch_bounds__(128) upsweep_kernel(NodeArrays na, const float
         }
     }
     // ---- climb: the last child to arrive computes the parent, children in ascending order
-    u32 cur = b;
-    for (;;) {
-        const u32 par = na.parent[cur];
-        if (par == NOCHILD) break;
+    // (the topology of the parent and the index of ITS parent come back in one round trip)
+    while (par != NOCHILD) {
         const u32 nc = na.nchild[par], c0 = na.child[par];      // topology: requested before the fence
         const int plev = na.level[par];
+        const u32 gpar = na.parent[par];
         // arrival counter with release (this node's record is written) / acquire (the siblings' records
         // are read next) ordering at device scope
         u32 old;
@@ -347,7 +347,7 @@ __global__ void __launch_bounds__(128) upsweep_kernel(NodeArrays na, const float
                 na.B2[par] = B2;
             }
         }
-        cur = par;
+        par = gpar;
     }
 }
 
@@ -487,11 +487,55 @@ __global__ void __launch_bounds__(SC_THREADS) gscan_kernel(const unsigned char *
     }
 }
 
+// Start node of the hard walk of every group (walk.cu): the lowest ancestor of the group's node whose
+// Morton cell contains the group box grown by r_out (plus a margin far above the fp32 rounding of the
+// T12 distance).  A leaf whose tight box comes within r_out of the group box in the fp32 arithmetic of
+// T12 overlaps the grown box, so its cell meets that ancestor's cell; Morton cells are nested or disjoint,
+// hence the leaf lies below the ancestor (or is it) and a walk that starts there finds the same hard list
+// as a walk from the root.
+__device__ __forceinline__ u32 quantise_d(double x, double o, double inv)
+{
+    const double f = floor((x - o) * inv);
+    return f >= 2097151.0 ? 2097151u : (f > 0.0 ? (u32)f : 0u);
+}
+
+struct AncArgs {       // what ginfo_kernel<true> needs beyond the boxes (one thread per group does this part)
+    const u32 *gnode; const unsigned char *level; const u32 *parent;
+    float r_out;
+    u32 *ganc;
+    DevCtl *ctl_rw; const u32 *nhard_prev; u32 *heavy; unsigned char *is_split; u32 par;      // split_group (common.cuh)
+};
+
+__device__ __forceinline__ void group_anc(const DevCtl *__restrict__ ctl, const AncArgs &x, u32 g, u32 ng, u32 count,
+                                          const float3 lo, const float3 hi)
+{
+    {   // work order of the next hard walk (the group flags of the build are free again by now)
+        const u32 prev = ctl->walk_ng;
+        split_group(x.ctl_rw, g, count, x.nhard_prev[g], (prev > ng ? prev - ng : ng - prev) <= ng / 16u, x.heavy, x.is_split, x.par);
+    }
+    const double inv = ctl->inv;
+    int lstar = MAXLEVEL;
+    const float l3[3] = {lo.x, lo.y, lo.z}, h3[3] = {hi.x, hi.y, hi.z};
+#pragma unroll
+    for (int a = 0; a < 3; a++) {
+        const double o = ctl->origin[a];
+        const double R = (double)x.r_out * (1.0 + 1.0 / 1024.0) +
+                         (fabs((double)l3[a]) + fabs((double)h3[a]) + (double)x.r_out) * (1.0 / 1048576.0);
+        const u32 qa = quantise_d((double)l3[a] - R, o, inv), qb = quantise_d((double)h3[a] + R, o, inv);
+        const u32 d = qa ^ qb;
+        lstar = min(lstar, d ? __clz((int)d) - 11 : MAXLEVEL);       // common leading bits of the 21
+    }
+    u32 node = x.gnode[g];
+    while ((int)x.level[node] > lstar) node = x.parent[node];
+    x.ganc[g] = node;
+}
+
 // eight lanes per group: each takes every eighth member, then the octet combines by shuffles
+template <bool ANC>
 __global__ void __launch_bounds__(256) ginfo_kernel(const DevCtl *__restrict__ ctl, u32 n,
                                                     const float4 *__restrict__ pos, const u32 *__restrict__ gfirst,
                                                     u32 *__restrict__ gcount, float4 *__restrict__ glo,
-                                                    float4 *__restrict__ ghi)
+                                                    float4 *__restrict__ ghi, const AncArgs anc)
 {
     const u32 ng = ctl->ng;
     const u32 sub = threadIdx.x & 7u;
@@ -518,52 +562,9 @@ __global__ void __launch_bounds__(256) ginfo_kernel(const DevCtl *__restrict__ c
             gcount[g] = e - f;
             glo[g] = make_float4(lo.x, lo.y, lo.z, 0.0f);
             ghi[g] = make_float4(hi.x, hi.y, hi.z, 0.0f);
+            if (ANC) group_anc(ctl, anc, g, ng, e - f, lo, hi);
         }
     }
-}
-
-// Start node of the hard walk of every group (walk.cu): the lowest ancestor of the group's node whose
-// Morton cell contains the group box grown by r_out (plus a margin far above the fp32 rounding of the
-// T12 distance).  A leaf whose tight box comes within r_out of the group box in the fp32 arithmetic of
-// T12 overlaps the grown box, so its cell meets that ancestor's cell; Morton cells are nested or disjoint,
-// hence the leaf lies below the ancestor (or is it) and a walk that starts there finds the same hard list
-// as a walk from the root.
-__device__ __forceinline__ u32 quantise_d(double x, double o, double inv)
-{
-    const double f = floor((x - o) * inv);
-    return f >= 2097151.0 ? 2097151u : (f > 0.0 ? (u32)f : 0u);
-}
-
-__global__ void __launch_bounds__(256) ganc_kernel(const DevCtl *__restrict__ ctl, const u32 *__restrict__ gnode,
-                                                   const float4 *__restrict__ glo, const float4 *__restrict__ ghi,
-                                                   const unsigned char *__restrict__ level, const u32 *__restrict__ parent,
-                                                   float r_out, u32 *__restrict__ ganc, DevCtl *ctl_rw,
-                                                   const u32 *__restrict__ gcount, const u32 *__restrict__ nhard_prev,
-                                                   u32 *__restrict__ heavy, unsigned char *__restrict__ is_split, u32 par)
-{
-    const u32 ng = ctl->ng;
-    const u32 g = blockIdx.x * blockDim.x + threadIdx.x;
-    if (g >= ng) return;
-    {   // work order of the next hard walk (the group flags of the build are free again by now)
-        const u32 prev = ctl->walk_ng;
-        split_group(ctl_rw, g, gcount[g], nhard_prev[g], (prev > ng ? prev - ng : ng - prev) <= ng / 16u, heavy, is_split, par);
-    }
-    const float4 lo = glo[g], hi = ghi[g];
-    const double inv = ctl->inv;
-    int lstar = MAXLEVEL;
-    const float l3[3] = {lo.x, lo.y, lo.z}, h3[3] = {hi.x, hi.y, hi.z};
-#pragma unroll
-    for (int a = 0; a < 3; a++) {
-        const double o = ctl->origin[a];
-        const double R = (double)r_out * (1.0 + 1.0 / 1024.0) +
-                         (fabs((double)l3[a]) + fabs((double)h3[a]) + (double)r_out) * (1.0 / 1048576.0);
-        const u32 qa = quantise_d((double)l3[a] - R, o, inv), qb = quantise_d((double)h3[a] + R, o, inv);
-        const u32 x = qa ^ qb;
-        lstar = min(lstar, x ? __clz((int)x) - 11 : MAXLEVEL);       // common leading bits of the 21
-    }
-    u32 node = gnode[g];
-    while ((int)level[node] > lstar) node = parent[node];
-    ganc[g] = node;
 }
 
 // ------------------------------------------------------------------ host side
@@ -618,17 +619,21 @@ cudaError_t launch_build_tree(Ctx *c)
     u32 *gfirst = wsptr<u32>(c, L.gfirst);
     gscan_kernel<<<sc_grid, SC_THREADS, 0, ax>>>(gflag, n, ctl, sc_status + L.po_tiles, gfirst, wsptr<u32>(c, L.gnode_at),
                                                  wsptr<u32>(c, L.gnode));
-    ginfo_kernel<<<(int)imin64((c->n + 255) / 256, (int64_t)c->num_sms * 8), 256, 0, ax>>>(
-        ctl, n, pos_t, gfirst, wsptr<u32>(c, L.gcount), wsptr<float4>(c, L.glo), wsptr<float4>(c, L.ghi));
+    // group boxes; with the force split also the start node of each group's hard walk and the work order of
+    // the next hard walk (split_group), for the counter slot that walk will use
+    const int gi_grid = (int)imin64((c->n + 255) / 256, (int64_t)c->num_sms * 8);
+    AncArgs anc = {};
     c->split_ready = false;
     if (c->p.split) {
-        // + the work order of the next hard walk (split_group), for the counter slot that walk will use
-        ganc_kernel<<<(int)((L.group_cap + 255) / 256), 256, 0, ax>>>(ctl, wsptr<u32>(c, L.gnode), wsptr<float4>(c, L.glo),
-                                                                     wsptr<float4>(c, L.ghi), level, parent, c->p.r_out,
-                                                                     wsptr<u32>(c, L.ganc), ctl, wsptr<u32>(c, L.gcount),
-                                                                     wsptr<u32>(c, L.nhard), wsptr<u32>(c, L.splitq), gflag,
-                                                                     c->walk_par);
+        anc.gnode = wsptr<u32>(c, L.gnode); anc.level = level; anc.parent = parent; anc.r_out = c->p.r_out;
+        anc.ganc = wsptr<u32>(c, L.ganc); anc.ctl_rw = ctl; anc.nhard_prev = wsptr<u32>(c, L.nhard);
+        anc.heavy = wsptr<u32>(c, L.splitq); anc.is_split = gflag; anc.par = c->walk_par;
+        ginfo_kernel<true><<<gi_grid, 256, 0, ax>>>(ctl, n, pos_t, gfirst, wsptr<u32>(c, L.gcount), wsptr<float4>(c, L.glo),
+                                                    wsptr<float4>(c, L.ghi), anc);
         c->split_ready = true; c->split_par = c->walk_par;
+    } else {
+        ginfo_kernel<false><<<gi_grid, 256, 0, ax>>>(ctl, n, pos_t, gfirst, wsptr<u32>(c, L.gcount), wsptr<float4>(c, L.glo),
+                                                     wsptr<float4>(c, L.ghi), anc);
     }
     cudaEventRecord(c->ev_groups, ax);
 
@@ -674,9 +679,9 @@ cudaError_t launch_regroup(Ctx *c)
     const int sc_grid = (int)imin64(L.sc_tiles, (int64_t)c->num_sms * 8);
     gscan_kernel<<<sc_grid, SC_THREADS, 0, st>>>(gflag, n, ctl, wsptr<u64>(c, L.sc_status) + L.po_tiles, wsptr<u32>(c, L.gfirst),
                                                  wsptr<u32>(c, L.gnode_at), wsptr<u32>(c, L.gnode));
-    ginfo_kernel<<<(int)imin64((c->n + 255) / 256, (int64_t)c->num_sms * 8), 256, 0, st>>>(
+    ginfo_kernel<false><<<(int)imin64((c->n + 255) / 256, (int64_t)c->num_sms * 8), 256, 0, st>>>(
         ctl, n, reinterpret_cast<const float4 *>(c->pos), wsptr<u32>(c, L.gfirst), wsptr<u32>(c, L.gcount),
-        wsptr<float4>(c, L.glo), wsptr<float4>(c, L.ghi));
+        wsptr<float4>(c, L.glo), wsptr<float4>(c, L.ghi), AncArgs{});
     return cudaGetLastError();
 }
 
@@ -694,9 +699,9 @@ cudaError_t launch_refit_tree(Ctx *c)
     na.B2 = wsptr<double>(c, L.B2); na.leaf_of = wsptr<u32>(c, L.leaf_of);
     upsweep_kernel<false><<<(int)((L.node_cap + 127) / 128), 128, 0, st>>>(na, reinterpret_cast<const float4 *>(c->pos), c->ctl,
                                                                            c->p.mac, c->p.theta);
-    ginfo_kernel<<<(int)imin64((c->n + 255) / 256, (int64_t)c->num_sms * 8), 256, 0, st>>>(
+    ginfo_kernel<false><<<(int)imin64((c->n + 255) / 256, (int64_t)c->num_sms * 8), 256, 0, st>>>(
         c->ctl, (u32)c->n, reinterpret_cast<const float4 *>(c->pos), wsptr<u32>(c, L.gfirst), wsptr<u32>(c, L.gcount),
-        wsptr<float4>(c, L.glo), wsptr<float4>(c, L.ghi));
+        wsptr<float4>(c, L.glo), wsptr<float4>(c, L.ghi), AncArgs{});
     return cudaGetLastError();
 }
 

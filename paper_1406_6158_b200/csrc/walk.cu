@@ -31,7 +31,7 @@ struct WalkArgs {
     u32 *ncell, *npart, *nhard;
     const u32 *heavy;             // hard walk: sink ranges of split groups (see split_kernel)
     u32 par;                      // which slot of DevCtl::group_counter / nheavy this launch uses
-    const u32 *ganc;              // hard walk: start node of every group (octree.cu, ganc_kernel)
+    const u32 *ganc;              // hard walk: start node of every group (octree.cu, group_anc)
     const unsigned char *is_split; // hard walk: group is handled as ranges
     float4 *a_soft, *a_hard;
     DevCtl *ctl;
