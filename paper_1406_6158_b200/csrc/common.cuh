@@ -22,9 +22,10 @@ constexpr u32 ST_NODE_OVERFLOW = 2u;
 constexpr u32 ST_STACK_OVERFLOW = 4u;
 constexpr u32 ST_WAIT_EXPIRED = 8u;
 
-// radix sort tiling (onesweep): 256 threads x 16 keys
+// radix sort tiling (onesweep): 256 threads x 14 keys = 3584 keys per tile (2^20 keys = 293 tiles, two per SM on
+// 148 SMs; with 4096-key tiles 40 SMs had one tile and 108 had two)
 constexpr int RS_THREADS = 256;
-constexpr int RS_KPT = 16;
+constexpr int RS_KPT = 14;
 constexpr int RS_TILE = RS_THREADS * RS_KPT;
 constexpr int RS_PASSES = 8;      // 8 x 8 bits >= 63 bits
 constexpr int LB_WIN = 16;        // radix look-back: tiles per block = status words requested together
