@@ -249,7 +249,8 @@ __device__ __forceinline__ void bbox_block_reduce(const float lo[3], const float
 }
 
 // Hard walk scheduling: a group whose hard list was long at the previous walk (n x nhard of the group with the
-// same index -- an estimate that only steers the order of work, never the result) is cut into 2 or 4 sink
+// same index -- an estimate that steers the order of work: the lists are the group's either way, only the
+// last bits of a sum can differ, because a range of fewer sinks combines its partial sums differently) is cut into 2 or 4 sink
 // ranges, which are queued in front of everything else; the walk skips it in the ordinary sequence.
 // Called once per group by ginfo_kernel (during the build, off the critical path) or by split_kernel.
 constexpr unsigned long long WK_SPLIT2 = 24576ull, WK_SPLIT4 = 65536ull;

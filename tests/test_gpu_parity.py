@@ -1,6 +1,7 @@
 """-m gpu: the CUDA path (through the C-ABI) against the oracle, stage by stage."""
 import numpy as np
 import pytest
+import torch
 
 from oracle import oracle as O
 from workloads import CONFIGS, make_ic
@@ -205,3 +206,38 @@ def test_bitwise_reproducible():
         h.close()
     for a, b in zip(*outs):
         assert np.array_equal(a, b)
+
+
+def test_hard_walk_work_order_paths_agree():
+    """The work order of a hard walk (heavy groups cut into sink ranges, chosen from the list lengths of the
+    previous walk) is prepared by the tree build for the first walk after it and by split_kernel for any
+    further walk on the same tree; the two counter slots alternate between launches.  The lists never
+    change; the sums are bit-identical whenever the same groups are cut, and differ only in rounding
+    when the cut set differs (a range of fewer sinks combines its partial sums in another order)."""
+    cfg = CONFIGS[2].with_(n=150001)                        # Hernquist cusp: some groups are heavy enough to be cut
+    pos, vel = make_ic(cfg.kind, cfg.n, 9)
+    h = make_hyb(cfg, pos, vel)
+
+    def close(a, b):
+        return float((a - b).norm() / b.norm()) < 1e-6
+
+    h.build_tree(); h.hard_force(); h.sync()                 # no previous walk: nothing is cut
+    first = h.a_hard.clone()
+    nh = h.export("nhard").copy()
+    h.hard_force(); h.sync()                                 # split_kernel, estimates from the first walk
+    second = h.a_hard.clone()
+    assert np.array_equal(nh, h.export("nhard")) and close(second, first)
+    for _ in range(3):                                       # same estimates, both counter slots
+        h.hard_force(); h.sync()
+        assert torch.equal(second, h.a_hard)
+        assert np.array_equal(nh, h.export("nhard"))
+    h.soft_force(); h.sync()                                 # fused walk: the same lists, another summation order
+    assert close(h.a_hard, first)
+    h.hard_force(); h.sync()
+    assert torch.equal(second, h.a_hard)
+    h.step(1); h.build_tree(); h.hard_force(); h.sync()      # after a step: the build prepares the order
+    again = h.a_hard.clone()
+    nh2 = h.export("nhard").copy()
+    h.hard_force(); h.sync()
+    assert np.array_equal(nh2, h.export("nhard")) and close(h.a_hard, again)
+    h.close()
