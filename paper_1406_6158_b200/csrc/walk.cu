@@ -48,7 +48,8 @@ constexpr u32 DESC_MASK = 0x1FFFFFFFu;      // node index bits of a stack descri
 template <int MODE>
 struct SmemLayout {                 // per warp
     static constexpr int cell_cap = MODE == WALK_HARD ? 0 : WK_CELL_CAP;
-    static constexpr int part_cap = MODE == WALK_NORMAL ? 0 : WK_PART_CAP;
+    // the hard walk has no monopole buffer, so its K-weighted buffer can be larger (fewer flushes) at 3 CTAs per SM
+    static constexpr int part_cap = MODE == WALK_NORMAL ? 0 : (MODE == WALK_HARD ? 256 : WK_PART_CAP);
     static constexpr int stack_cap = 512;
     static constexpr int lq_cap = 96;
     static constexpr int cell_alloc = cell_cap ? cell_cap + WK_PAD_SLACK : 0;
