@@ -75,3 +75,15 @@ def test_plummer_virial_and_energy_drift():
     err = abs((t1 + w1 - t0 - w0) / (t0 + w0))
     print(f"N = {n}: E0 = {t0 + w0:.6f}, {ncyc} soft cycles, |dE/E0| = {err:.2e}")
     assert err < 2e-3
+
+
+def test_energy_null_pointer_is_an_error():
+    from paper_1406_6158_b200 import lib
+    cfg = CONFIGS[0].with_(n=64)
+    pos, vel = make_ic("plummer", 64, 1)
+    h = make_hyb(cfg, pos, vel)
+    assert lib().hyb_energy(h._h, None) != 0
+    assert b"h_energy" in lib().hyb_last_error(h._h)
+    t, w = h.energy()                                           # the context is still usable
+    assert t > 0.0 and w < 0.0
+    h.close()
