@@ -165,7 +165,11 @@ int hyb_soft_force(hyb_ctx *ctx);
 
 /* Step a9 alone (a hard-step): neighbour search cut off at r_out
  * and the K-weighted direct sum; writes d_a_hard only.  split = 0: writes zeros.
- * Requires a tree.  Asynchronous. */
+ * Requires a tree.  Asynchronous.
+ * Reproducibility: the same sequence of calls on the same input gives the same bits.  The heaviest sink
+ * groups are cut into sink ranges for load balance, chosen from the list lengths of the previous walk; the
+ * neighbour lists never depend on that, but a cut group adds its partial sums in another order, so a walk
+ * repeated on one tree can differ from the first in the last bits. */
 int hyb_hard_force(hyb_ctx *ctx);
 
 /* n_soft_steps cycles of the two-rate leapfrog (Eq. 3-4), in the
