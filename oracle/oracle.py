@@ -36,7 +36,8 @@ _lib = None
 def lib():
     global _lib
     if _lib is None:
-        L = C.CDLL(build())
+        import os
+        L = C.CDLL(build(sanitize=os.environ.get("HYB_ORACLE_SANITIZE") == "1"))
         L.orc_K.restype = C.c_double
         L.orc_K.argtypes = [C.c_double, C.c_double, C.c_double, C.c_int]
         L.orc_rb.restype = C.c_double
