@@ -473,6 +473,26 @@ static float dist2_box_box(const orc_tree *t, int64_t g, int64_t k)
     return s + zz;
 }
 
+/* T13 with hard_cut = 1 (R30): is particle j (sorted order) within r_out of the box of group g?
+ * the hard force acts only within R_2 ("cut-off").  Every sink of the group lies in
+ * the group box, so a particle at least r_out away from the box has K = 0 for all of them.  fp32, one
+ * rounding per operation, strict "<" like rule (b). */
+static int in_cut(const orc_tree *t, int64_t g, uint32_t j)
+{
+    float e[3];
+    for (int a = 0; a < 3; a++) {
+        float x = t->pos_s[4 * (size_t)j + a];
+        float u = t->glo[3 * g + a] - x;
+        float w = x - t->ghi[3 * g + a];
+        e[a] = fmax0(u, w);
+    }
+    float xx = e[0] * e[0], yy = e[1] * e[1], zz = e[2] * e[2];
+    float s = xx + yy;
+    float d2 = s + zz;
+    float rout = t->p.r_out;
+    return d2 < rout * rout;
+}
+
 /* T13.  Visits the tree for group g; calls back for accepted cells and opened leaves. */
 typedef struct {
     uint32_t *cells; uint8_t *cellhard; int64_t ncells, cap_cells;
@@ -491,7 +511,7 @@ static void push_cell(walk_out *w, uint32_t k, int hard)
     w->ncells++;
     if (hard) w->nhard += 1;
 }
-static void push_leaf(walk_out *w, uint32_t k, int hard, uint32_t count)
+static void push_leaf(walk_out *w, uint32_t k, int hard, uint32_t count, uint32_t count_hard)
 {
     if (w->leaves) {
         if (w->nleaves == w->cap_leaves) { w->cap_leaves = w->cap_leaves ? 2 * w->cap_leaves : 1024;
@@ -501,7 +521,7 @@ static void push_leaf(walk_out *w, uint32_t k, int hard, uint32_t count)
     }
     w->nleaves++;
     w->npart += count;
-    if (hard) w->nhard += count;
+    if (hard) w->nhard += count_hard;
 }
 
 static void walk_group(const orc_tree *t, int mode, int64_t g, walk_out *w, int keep)
@@ -537,7 +557,12 @@ static void walk_group(const orc_tree *t, int mode, int64_t g, walk_out *w, int 
         if (!open) { push_cell(w, k, tree && near); continue; }
         if (t->child[k] == NOCHILD) {
             int hard = (mode == ORC_MODE_NORMAL) ? 0 : near;
-            push_leaf(w, k, hard, t->count[k]);
+            uint32_t nh = t->count[k];
+            if (hard && t->p.hard_cut) {                               /* R30: particle-level cut */
+                nh = 0;
+                for (uint32_t j = t->first[k]; j < t->first[k] + t->count[k]; j++) nh += (uint32_t)in_cut(t, g, j);
+            }
+            push_leaf(w, k, hard, t->count[k], nh);
             continue;
         }
         if (sp + 8 > scap) { scap *= 2; stack = (uint32_t *)realloc(stack, 4 * (size_t)scap); }
@@ -582,7 +607,11 @@ int orc_walk_lists(const orc_tree *t, int mode, int64_t g,
         int64_t q = 0;
         for (int64_t l = 0; l < w.nleaves; l++) {
             uint32_t k = w.leaves[l];
-            for (uint32_t j = t->first[k]; j < t->first[k] + t->count[k]; j++) { parts[q] = j; hard[q] = w.leafhard[l]; q++; }
+            for (uint32_t j = t->first[k]; j < t->first[k] + t->count[k]; j++) {
+                parts[q] = j;
+                hard[q] = (uint8_t)(w.leafhard[l] && (!t->p.hard_cut || in_cut(t, g, j)));
+                q++;
+            }
         }
     }
     free(w.cells); free(w.cellhard); free(w.leaves); free(w.leafhard);
@@ -717,7 +746,7 @@ void orc_forces(const orc_tree *t, int mode, int64_t ngsel, const int64_t *gsel,
                             double ws = (1.0 - K) * ms;
                             as[0] += ws * dx[0]; as[1] += ws * dx[1]; as[2] += ws * dx[2];
                         }
-                        if (hard) {
+                        if (hard && (!t->p.hard_cut || in_cut(t, g, j))) {
                             double wh = K * ms;
                             ah[0] += wh * dx[0]; ah[1] += wh * dx[1]; ah[2] += wh * dx[2];
                         }

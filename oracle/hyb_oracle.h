@@ -14,7 +14,10 @@
  *   keys / sort      lattice values, stable-sort equivalence          pinned
  *   octree / groups  invariants + independent geometric bisection     pinned
  *   moments / r_b    direct sums, worked value of Eq. 5               pinned
- *   walk lists       completeness, brute-force neighbour superset     pinned
+ *   walk lists       completeness, brute-force neighbour superset,
+ *                    rule (a) and Eq. 14-15 re-derived as sets, mutated
+ *                    oracles fail (test_oracle_mac.py); hard_cut = 1:
+ *                    list == brute-force set over all particles      pinned
  *   forces           two-body closed form, theta=0 == brute force,
  *                    momentum of the hard sum, Plummer/Hernquist/ball pinned
  *   step             circular binary, reversibility, 2nd order        pinned
@@ -43,6 +46,9 @@ typedef struct {
     int32_t split;         /* 1 hybrid, 0 normal tree */
     int32_t grouping;      /* T11: 0 sink group = one tree node, 1 = run of consecutive small siblings (R17) */
     int32_t hard_tree;     /* R20: 0 hard force = direct K-weighted sum, 1 = the paper's MAC-approximated hard walk */
+    int32_t hard_cut;      /* R30 (T13): 0 = the hard list holds every particle of a leaf whose box comes within r_out
+                              of the group box; 1 = only those particles that are themselves within r_out of the group
+                              box ("neighbours within r_out": cut-off beyond R_2) */
 } orc_params;
 
 enum { ORC_MODE_HYBRID = 0, ORC_MODE_HARD = 1, ORC_MODE_NORMAL = 2 };
