@@ -104,6 +104,8 @@ def main():
                     help="1: hard-only substeps refit the boxes instead of rebuilding the tree (not the paper's procedure)")
     ap.add_argument("--hard-tree", type=int, default=None, choices=[0, 1],
                     help="1: the paper's MAC-approximated hard walk instead of the direct hard sum (DESIGN.md R20)")
+    ap.add_argument("--hard-cut", type=int, default=None, choices=[0, 1],
+                    help="hard list: 0 every particle of the leaves within r_out of the group box, 1 only the particles within r_out of it (DESIGN.md R30)")
     ap.add_argument("--grouping", type=int, default=None, choices=[0, 1, 2],
                     help="sink groups: 0 single tree nodes, 1 runs of sibling cells, 2 auto (the configs' default)")
     args = ap.parse_args()
@@ -123,6 +125,8 @@ def main():
         cfg = cfg.with_(hard_tree=args.hard_tree)
     if args.hard_refit is not None:
         cfg = cfg.with_(hard_refit=args.hard_refit)
+    if args.hard_cut is not None:
+        cfg = cfg.with_(hard_cut=args.hard_cut)
     config = {"workload": f"{cfg.name}: {cfg.kind} N={cfg.n}, eps={cfg.eps}, theta={cfg.theta}, leaf<={cfg.leaf_max}, "
                           f"group<={cfg.group_max}, r_in={cfg.r_in}, r_out={cfg.r_out}, dt_soft=1/{round(1 / cfg.dt_soft)}, "
                           f"n_sub={cfg.n_sub}, grouping={cfg.grouping}, hard_tree={cfg.hard_tree}, hard_refit={cfg.hard_refit}, seed {cfg.seed}",

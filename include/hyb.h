@@ -65,6 +65,12 @@ typedef struct hyb_params {
                           rebuilt at soft steps only; the hard-only substeps keep the store order and the
                           topology and refit the tight boxes (see hyb_refit_tree): the hard force is the same
                           direct sum, only the order of the fp32 additions differs                          */
+    int32_t hard_cut;  /* the hard list of a sink group (K = 0 beyond R_2; R30).
+                          0 = every particle of every leaf whose tight box comes within r_out of the group box;
+                          1 = only the particles that are themselves within r_out of the group box (what the
+                          fused walk drops from the hard list it evaluates as plain Eq. 2 pairs).  The forces are
+                          the same (the dropped pairs carry K = 0); HYB_X_NHARD and the hard interaction count
+                          report the list that was evaluated                                               */
 } hyb_params;
 
 enum {

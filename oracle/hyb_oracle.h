@@ -97,7 +97,9 @@ int64_t orc_tree_ng(const orc_tree *t);
 /* copies the selected array; returns bytes written or -1 */
 int64_t orc_tree_get(const orc_tree *t, int what, void *dst, int64_t bytes);
 
-/* T12-T13: list lengths per group. */
+/* T12-T13: list lengths per group.  npart counts the particles of every opened leaf; nhard the hard list
+ * (hard_cut = 0: the particles of the leaves within r_out of the group box; hard_cut = 1: those of them that are
+ * themselves within r_out of the group box). */
 void orc_walk_counts(const orc_tree *t, int mode, uint32_t *ncell, uint32_t *npart, uint32_t *nhard);
 /* T12-T13 for the ngsel groups listed in gsel: output entry k belongs to group gsel[k]. */
 void orc_walk_counts_sel(const orc_tree *t, int mode, int64_t ngsel, const int64_t *gsel,

@@ -39,7 +39,8 @@ class HybParams(C.Structure):
     _fields_ = [("G", C.c_float), ("eps", C.c_float), ("theta", C.c_float), ("a_err", C.c_float),
                 ("r_in", C.c_float), ("r_out", C.c_float), ("dt_soft", C.c_float),
                 ("n_sub", C.c_int32), ("leaf_max", C.c_int32), ("group_max", C.c_int32),
-                ("mac", C.c_int32), ("kfunc", C.c_int32), ("split", C.c_int32), ("grouping", C.c_int32), ("hard_tree", C.c_int32), ("hard_refit", C.c_int32)]
+                ("mac", C.c_int32), ("kfunc", C.c_int32), ("split", C.c_int32), ("grouping", C.c_int32), ("hard_tree", C.c_int32), ("hard_refit", C.c_int32),
+                ("hard_cut", C.c_int32)]
 
     @classmethod
     def from_config(cls, cfg, **over):

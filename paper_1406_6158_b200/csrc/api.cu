@@ -3,6 +3,7 @@
 #include <stdio.h>
 #include <stddef.h>
 #include <string.h>
+#include <stdlib.h>
 
 #include <mutex>
 #include <new>
@@ -75,6 +76,7 @@ static bool params_ok(const hyb_params *p, int64_t n, char *msg)
     if (p->split != 0 && p->split != 1) return bad("split must be 0 or 1");
     if (p->hard_tree != 0 && p->hard_tree != 1) return bad("hard_tree must be 0 or 1");
     if (p->hard_refit != 0 && p->hard_refit != 1) return bad("hard_refit must be 0 or 1");
+    if (p->hard_cut != 0 && p->hard_cut != 1) return bad("hard_cut must be 0 or 1");
     if (p->hard_refit == 1 && (p->split != 1 || p->hard_tree != 0)) return bad("hard_refit needs split = 1 and hard_tree = 0");
     if (p->grouping != HYB_GROUP_NODE && p->grouping != HYB_GROUP_SIBLINGS && p->grouping != HYB_GROUP_AUTO) return bad("unknown grouping");
     if (p->split == 1 && !(p->r_in >= 0.0f && p->r_out > p->r_in && isfinite(p->r_out))) return bad("need 0 <= r_in < r_out");
@@ -231,6 +233,11 @@ int hyb_init(hyb_ctx **out, const hyb_params *params, int64_t n, hyb_float4 *d_p
     c->timing = true;
     e = cudaMemsetAsync(c->ctl, 0, sizeof(DevCtl), c->stream);
     if (e == cudaSuccess) e = cudaMemsetAsync(c->ws + L.nhard, 0, 4 * (size_t)L.group_cap, c->stream);
+    {
+        u32 t[4] = {8192u, 24576u, 65536u, (u32)imin64(4 * L.group_cap, 0xFFFFFFFFll)};
+        if (const char *sp = getenv("HYB_SPLIT")) sscanf(sp, "%u,%u,%u", &t[0], &t[1], &t[2]);
+        if (e == cudaSuccess) e = cudaMemcpyAsync(&c->ctl->split_t[0], t, sizeof t, cudaMemcpyHostToDevice, c->stream);
+    }
     if (e != cudaSuccess) { delete c; return cuda_fail(nullptr, e, "cudaMemsetAsync"); }
     *out = reinterpret_cast<hyb_ctx *>(c);
     return HYB_OK;

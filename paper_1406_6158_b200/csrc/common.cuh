@@ -62,6 +62,8 @@ struct DevCtl {
     u32 group_counter[2];
     u32 nheavy[2];              // sink ranges of split groups (hard walk)
     u32 walk_ng;                // number of groups of the last walk (is its nhard[] comparable?)
+    u32 split_t[3];             // hard walk scheduling thresholds (pairs): queue first / cut in 2 / cut in 4 (set by hyb_init)
+    u32 split_cap;              // entries the queue of sink ranges can hold
     u64 inter_soft, inter_hard, inter_hard_fused;   // pair counts: soft lists, hard lists (all walks), hard lists of fused walks
     // ---- bounding box reduction: filled by bbox_kernel or by the drift, cleared again by keys_kernel ----
     u32 bbox_enc[6];            // order-preserving encodings: ~min xyz, max xyz (atomicMax from 0 for both)
@@ -108,7 +110,7 @@ struct __align__(16) NodeRec {
     float4 B;        // tight box minimum, squared opening radius (T8, T10)
     float4 C;        // tight box maximum, 0
     uint2 meta;      // cell: (first child, nchild);  leaf: (first particle, count | 0x80000000)
-    uint2 pad;
+    uint2 pad;       // (first particle, count) of the node, cell or leaf
 };
 
 struct Layout {   // byte offsets into the workspace; computed by plan_workspace
@@ -250,22 +252,28 @@ __device__ __forceinline__ void bbox_block_reduce(const float lo[3], const float
 
 // Hard walk scheduling: a group whose hard list was long at the previous walk (n x nhard of the group with the
 // same index -- an estimate that steers the order of work: the lists are the group's either way, only the
-// last bits of a sum can differ, because a range of fewer sinks combines its partial sums differently) is cut into 2 or 4 sink
-// ranges, which are queued in front of everything else; the walk skips it in the ordinary sequence.
+// last bits of a sum can differ, because a range of fewer sinks combines its partial sums differently) is queued
+// in front of everything else, the heaviest ones cut into 2 or 4 sink ranges; the walk skips it in the ordinary
+// sequence.
 // Called once per group by ginfo_kernel (during the build, off the critical path) or by split_kernel.
-constexpr unsigned long long WK_SPLIT2 = 24576ull, WK_SPLIT4 = 65536ull;
 __device__ __forceinline__ void split_group(DevCtl *ctl, u32 g, u32 n, u32 h_prev, bool comparable, u32 *__restrict__ heavy,
                                             unsigned char *__restrict__ is_split, u32 par)
 {
     const unsigned long long est = (unsigned long long)n * (unsigned long long)(comparable ? h_prev : 0u);
-    u32 nsub = 1;
-    if (est >= WK_SPLIT4 && n >= 32u) nsub = 4;
-    else if (est >= WK_SPLIT2 && n >= 16u) nsub = 2;
-    if (nsub > 1) {
+    u32 nsub = 0;                                   // 0: stays in the ordinary sequence
+    if (est >= ctl->split_t[2] && n >= 32u) nsub = 4;
+    else if (est >= ctl->split_t[1] && n >= 16u) nsub = 2;
+    else if (est >= ctl->split_t[0]) nsub = 1;      // whole, but queued in front
+    if (nsub) {
         const u32 at = atomicAdd(&ctl->nheavy[par], nsub);
-        for (u32 i = 0; i < nsub; i++) heavy[at + i] = g | (i << 28) | ((nsub - 1u) << 30);
+        if (at + nsub <= ctl->split_cap) {
+            for (u32 i = 0; i < nsub; i++) heavy[at + i] = g | (i << 28) | ((nsub - 1u) << 30);
+        } else {
+            atomicSub(&ctl->nheavy[par], nsub);     // the queue is full (it cannot be: 4 entries per group): leave the group where it is
+            nsub = 0;
+        }
     }
-    is_split[g] = nsub > 1;
+    is_split[g] = nsub > 0;
 }
 
 // Decoupled look-back over one value per tile (status word: bits 63..62 flag, low 62 bits value).

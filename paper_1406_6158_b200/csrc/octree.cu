@@ -213,6 +213,7 @@ __global__ void __launch_bounds__(256) link_kernel(
         first[b] = f; count[b] = c; child[b] = ch; nchild[b] = (unsigned char)nc; parent[b] = par;
         arrived[b] = 0; bmax2[b] = 0ull;
         rec[b].meta = internal ? make_uint2(ch, nc) : make_uint2(f, c | 0x80000000u);
+        rec[b].pad = make_uint2(f, c);
     }
 }
 
@@ -506,13 +507,8 @@ struct AncArgs {       // what ginfo_kernel<true> needs beyond the boxes (one th
     DevCtl *ctl_rw; const u32 *nhard_prev; u32 *heavy; unsigned char *is_split; u32 par;      // split_group (common.cuh)
 };
 
-__device__ __forceinline__ void group_anc(const DevCtl *__restrict__ ctl, const AncArgs &x, u32 g, u32 ng, u32 count,
-                                          const float3 lo, const float3 hi)
+__device__ __forceinline__ u32 node_anc(const DevCtl *__restrict__ ctl, const AncArgs &x, u32 node, const float3 lo, const float3 hi)
 {
-    {   // work order of the next hard walk (the group flags of the build are free again by now)
-        const u32 prev = ctl->walk_ng;
-        split_group(x.ctl_rw, g, count, x.nhard_prev[g], (prev > ng ? prev - ng : ng - prev) <= ng / 16u, x.heavy, x.is_split, x.par);
-    }
     const double inv = ctl->inv;
     int lstar = MAXLEVEL;
     const float l3[3] = {lo.x, lo.y, lo.z}, h3[3] = {hi.x, hi.y, hi.z};
@@ -525,9 +521,18 @@ __device__ __forceinline__ void group_anc(const DevCtl *__restrict__ ctl, const 
         const u32 d = qa ^ qb;
         lstar = min(lstar, d ? __clz((int)d) - 11 : MAXLEVEL);       // common leading bits of the 21
     }
-    u32 node = x.gnode[g];
     while ((int)x.level[node] > lstar) node = x.parent[node];
-    x.ganc[g] = node;
+    return node;
+}
+
+__device__ __forceinline__ void group_anc(const DevCtl *__restrict__ ctl, const AncArgs &x, u32 g, u32 ng, u32 count,
+                                          const float3 lo, const float3 hi)
+{
+    {   // work order of the next hard walk (the group flags of the build are free again by now)
+        const u32 prev = ctl->walk_ng;
+        split_group(x.ctl_rw, g, count, x.nhard_prev[g], (prev > ng ? prev - ng : ng - prev) <= ng / 16u, x.heavy, x.is_split, x.par);
+    }
+    x.ganc[g] = node_anc(ctl, x, x.gnode[g], lo, hi);
 }
 
 // eight lanes per group: each takes every eighth member, then the octet combines by shuffles

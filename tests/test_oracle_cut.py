@@ -35,6 +35,7 @@ def test_hard_list_is_the_brute_force_set(grouping, mac):
     nc0, np0, nh0 = t0.walk_counts(O.MODE_HYBRID)
     # the cut changes nothing but the hard list: same cells, same particle list, hard walk == fused walk
     assert np.array_equal(nc, nc0) and np.array_equal(npart, np0) and np.array_equal(nh, nh_h)
+    assert np.array_equal(np_h, nh0) and np.all(nc_h == 0)           # a hard walk opens the leaves within r_out, nothing else
     assert np.all(nh <= nh0) and nh.sum() < 0.8 * nh0.sum() and np.all(nh >= gc)
     x64 = ps[:, :3].astype(np.float64)
     for g in range(0, t.ng, 3):
