@@ -140,8 +140,10 @@ size_t hyb_workspace_bytes(int64_t n, const hyb_params *params);
  *                  positions (fill with 0..n-1 to track the permutation).
  *  d_workspace     DEVICE scratch of at least hyb_workspace_bytes(n, params), 256-byte aligned.
  *  device, cuda_stream   CUDA device ordinal and cudaStream_t (as void*) all work is issued on.
- * All device buffers stay owned by the caller and must outlive the context.  The library
- * allocates no device memory of its own.  hyb_init itself only zeroes its control block. */
+ * All device buffers stay owned by the caller and must outlive the context.  A context allocates no
+ * device memory: every call, hyb_energy and hyb_let_count included, works inside d_workspace (the only
+ * device allocation of the library is the buffer hyb_run_host keeps, see there).  The context owns host
+ * memory, one auxiliary CUDA stream and CUDA events.  hyb_init itself only zeroes its control block. */
 int hyb_init(hyb_ctx **out, const hyb_params *params, int64_t n,
              hyb_float4 *d_pos_m, hyb_float4 *d_vel, hyb_float4 *d_a_soft, hyb_float4 *d_a_hard,
              uint32_t *d_id, void *d_workspace, size_t workspace_bytes, int device, void *cuda_stream);
@@ -154,6 +156,15 @@ int hyb_set_params(hyb_ctx *ctx, const hyb_params *params);
  * linear octree, centre-of-mass / opening-radius upsweep
  * and sink groups for the current positions.  Asynchronous. */
 int hyb_build_tree(hyb_ctx *ctx);
+
+/* The tree of a hard-step (a hard-step computes only the hard force; the tree is
+ * rebuilt for it): steps a1-a5 and a7 as in hyb_build_tree and the tight boxes of a6, but no moments and no
+ * opening radius, which only the soft walk reads (with hard_tree = 1 they are computed, the hard walk applies
+ * the MAC).  With grouping = HYB_GROUP_AUTO the sink groups are runs of at most group_max / 2 sinks
+ * (R17).  This is the build hyb_step uses in front of every hard-only force
+ * evaluation.  Afterwards hyb_hard_force works; hyb_soft_force and hyb_let_count return HYB_ERR_NO_TREE.
+ * Needs split = 1.  Asynchronous. */
+int hyb_build_tree_hard(hyb_ctx *ctx);
 
 /* After the positions have moved a little since the last hyb_build_tree (same store order): recompute the
  * tight boxes of all nodes and sink groups for the current positions, keeping the topology.  The result
@@ -187,7 +198,10 @@ int hyb_hard_force(hyb_ctx *ctx);
  * end to read the device status word (capacity overflow, non-finite input). */
 int hyb_step(hyb_ctx *ctx, int32_t n_soft_steps);
 
-/* Synchronise the stream and return the device status as an error code. */
+/* Synchronise the stream and return the device status as an error code.  An error (non-finite input, capacity
+ * overflow) is reported once: the status word is cleared, the tree and the accelerations of the context are
+ * marked invalid, and the context can be used again after the caller has repaired the input (the next
+ * hyb_build_tree / hyb_step starts from the particle arrays as they are). */
 int hyb_sync(hyb_ctx *ctx);
 
 /* Debug / test / bench read-back into HOST memory; synchronises the stream.

@@ -66,7 +66,7 @@ def lib():
         L.hyb_init.restype = C.c_int
         L.hyb_init.argtypes = [C.POINTER(vp), C.POINTER(HybParams), C.c_int64, vp, vp, vp, vp, vp, vp, C.c_size_t,
                                C.c_int, vp]
-        for name in ("hyb_build_tree", "hyb_refit_tree", "hyb_soft_force", "hyb_hard_force", "hyb_sync"):
+        for name in ("hyb_build_tree", "hyb_build_tree_hard", "hyb_refit_tree", "hyb_soft_force", "hyb_hard_force", "hyb_sync"):
             getattr(L, name).restype = C.c_int
             getattr(L, name).argtypes = [vp]
         L.hyb_set_params.restype = C.c_int
@@ -159,6 +159,9 @@ class Hyb:
 
     def build_tree(self):
         self._check(lib().hyb_build_tree(self._h))
+
+    def build_tree_hard(self):
+        self._check(lib().hyb_build_tree_hard(self._h))
 
     def refit_tree(self):
         self._check(lib().hyb_refit_tree(self._h))

@@ -55,6 +55,9 @@ Layout plan_workspace(int64_t n)
     L.ncell = take(4 * GC); L.npart = take(4 * GC); L.nhard = take(4 * GC);
     L.splitq = take(4 * 4 * GC);
     L.gnode = take(4 * GC); L.ganc = take(4 * GC);
+    // scratch of hyb_energy and hyb_let_count (partial sums; domain boxes and counts)
+    L.scratch_bytes = 8 * (N / 16 + 32768);
+    L.scratch = take(L.scratch_bytes);
     L.total = off;
     return L;
 }
@@ -218,17 +221,17 @@ int hyb_init(hyb_ctx **out, const hyb_params *params, int64_t n, hyb_float4 *d_p
     c->pos = d_pos_m; c->vel = d_vel; c->a_soft = d_a_soft; c->a_hard = d_a_hard; c->id = d_id;
     c->ws = (char *)d_workspace; c->L = L; c->ctl = (DevCtl *)(c->ws + L.ctl);
     e = cudaDeviceGetAttribute(&c->num_sms, cudaDevAttrMultiProcessorCount, device);
-    if (e != cudaSuccess) { delete c; return cuda_fail(nullptr, e, "cudaDeviceGetAttribute"); }
+    if (e != cudaSuccess) { const int rc = cuda_fail(nullptr, e, "cudaDeviceGetAttribute"); hyb_free(reinterpret_cast<hyb_ctx *>(c)); return rc; }
     for (int i = 0; i < 5; i++) {
         e = cudaEventCreate(&c->ev[i]);
-        if (e != cudaSuccess) { delete c; return cuda_fail(nullptr, e, "cudaEventCreate"); }
+        if (e != cudaSuccess) { const int rc = cuda_fail(nullptr, e, "cudaEventCreate"); hyb_free(reinterpret_cast<hyb_ctx *>(c)); return rc; }
     }
     e = cudaStreamCreateWithFlags(&c->aux, cudaStreamNonBlocking);
-    if (e != cudaSuccess) { delete c; return cuda_fail(nullptr, e, "cudaStreamCreate"); }
+    if (e != cudaSuccess) { const int rc = cuda_fail(nullptr, e, "cudaStreamCreate"); hyb_free(reinterpret_cast<hyb_ctx *>(c)); return rc; }
     cudaEvent_t *evs[4] = {&c->ev_sorted, &c->ev_perm, &c->ev_linked, &c->ev_groups};
     for (int i = 0; i < 4; i++) {
         e = cudaEventCreateWithFlags(evs[i], cudaEventDisableTiming);
-        if (e != cudaSuccess) { delete c; return cuda_fail(nullptr, e, "cudaEventCreate"); }
+        if (e != cudaSuccess) { const int rc = cuda_fail(nullptr, e, "cudaEventCreate"); hyb_free(reinterpret_cast<hyb_ctx *>(c)); return rc; }
     }
     c->timing = true;
     e = cudaMemsetAsync(c->ctl, 0, sizeof(DevCtl), c->stream);
@@ -238,7 +241,7 @@ int hyb_init(hyb_ctx **out, const hyb_params *params, int64_t n, hyb_float4 *d_p
         if (const char *sp = getenv("HYB_SPLIT")) sscanf(sp, "%u,%u,%u", &t[0], &t[1], &t[2]);
         if (e == cudaSuccess) e = cudaMemcpyAsync(&c->ctl->split_t[0], t, sizeof t, cudaMemcpyHostToDevice, c->stream);
     }
-    if (e != cudaSuccess) { delete c; return cuda_fail(nullptr, e, "cudaMemsetAsync"); }
+    if (e != cudaSuccess) { const int rc = cuda_fail(nullptr, e, "cudaMemsetAsync"); hyb_free(reinterpret_cast<hyb_ctx *>(c)); return rc; }
     *out = reinterpret_cast<hyb_ctx *>(c);
     return HYB_OK;
 }
@@ -265,6 +268,16 @@ int hyb_build_tree(hyb_ctx *ctx)
     return do_build(c);
 }
 
+int hyb_build_tree_hard(hyb_ctx *ctx)
+{
+    Ctx *c = reinterpret_cast<Ctx *>(ctx);
+    if (!c) return fail(nullptr, HYB_ERR_INVALID_ARG, "ctx is NULL");
+    if (c->p.split != 1) return fail(c, HYB_ERR_INVALID_ARG, "a hard-step tree needs split = 1");
+    cudaSetDevice(c->device);
+    discard_pending_bbox(c);
+    return do_build(c, true);
+}
+
 int hyb_refit_tree(hyb_ctx *ctx)
 {
     Ctx *c = reinterpret_cast<Ctx *>(ctx);
@@ -279,7 +292,8 @@ int hyb_soft_force(hyb_ctx *ctx)
 {
     Ctx *c = reinterpret_cast<Ctx *>(ctx);
     if (!c) return fail(nullptr, HYB_ERR_INVALID_ARG, "ctx is NULL");
-    if (!c->tree_valid || c->tree_refit) return fail(c, HYB_ERR_NO_TREE, "no tree for the current positions");
+    if (!c->tree_valid || c->tree_refit || c->boxes_only)
+        return fail(c, HYB_ERR_NO_TREE, "no tree with moments for the current positions");
     cudaSetDevice(c->device);
     int rc = do_soft(c);
     if (rc == HYB_OK) c->acc_valid = true;
@@ -304,6 +318,11 @@ int hyb_sync(hyb_ctx *ctx)
     cudaError_t e = cudaMemcpyAsync(&st, &c->ctl->status, sizeof st, cudaMemcpyDeviceToHost, c->stream);
     if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
     if (e != cudaSuccess) return cuda_fail(c, e, "hyb_sync");
+    if (st) {       // reported once: the word is cleared, what was computed from the bad state is dropped
+        cudaMemsetAsync(&c->ctl->status, 0, sizeof(u32), c->stream);
+        c->tree_valid = false; c->acc_valid = false; c->bbox_ready = false;
+        cudaMemsetAsync(&c->ctl->bbox_enc[0], 0, 7 * sizeof(u32), c->stream);
+    }
     return status_to_error(c, st);
 }
 
@@ -325,8 +344,20 @@ int hyb_step(hyb_ctx *ctx, int32_t n_soft_steps)
     }
     struct Seg { int kind; cudaEvent_t a, b; };     // kind: 0 build, 1 soft, 2 hard, 3 integrate
     std::vector<Seg> segs;
-    std::vector<cudaEvent_t> pool;
-    auto ev = [&]() { cudaEvent_t e; cudaEventCreate(&e); pool.push_back(e); cudaEventRecord(e, c->stream); return e; };
+    // stage timers: events come from a pool the context keeps (it grows to the longest call and is destroyed by hyb_free)
+    if (c->timing) {
+        const size_t need = 5 * (size_t)nsub * (size_t)n_soft_steps;
+        if (need > c->evpool_n) {
+            cudaEvent_t *np = (cudaEvent_t *)realloc(c->evpool, need * sizeof(cudaEvent_t));
+            if (!np) return fail(c, HYB_ERR_INTERNAL, "out of host memory");
+            c->evpool = np;
+            for (; c->evpool_n < need; c->evpool_n++)
+                if (cudaEventCreate(&c->evpool[c->evpool_n]) != cudaSuccess) return cuda_fail(c, cudaGetLastError(), "cudaEventCreate");
+        }
+    }
+    size_t ev_used = 0;
+    auto ev = [&]() { cudaEvent_t e = c->evpool[ev_used++]; cudaEventRecord(e, c->stream); return e; };
+    auto bail = [&](int code) { c->tree_valid = false; c->acc_valid = false; return code; };
     for (int32_t cyc = 0; cyc < n_soft_steps; cyc++) {
         for (int k = 0; k < nsub; k++) {
             cudaEvent_t e0 = c->timing ? ev() : nullptr;
@@ -339,20 +370,20 @@ int hyb_step(hyb_ctx *ctx, int32_t n_soft_steps)
             const bool rebuild = soft_step || !c->p.hard_refit;      // a full build follows: the drift reduces its bounding box
             if (split) e = launch_kick_drift(c, k == 0 ? 0.5f * dts : 0.0f, open_c, dth, rebuild);
             else e = launch_kick_drift(c, open_c, 0.0f, dth, rebuild);
-            if (e != cudaSuccess) return cuda_fail(c, e, "kick_drift");
+            if (e != cudaSuccess) return bail(cuda_fail(c, e, "kick_drift"));
             cudaEvent_t e1 = c->timing ? ev() : nullptr;
             if (!soft_step && c->p.hard_refit) rc = do_refit(c, k == 0 && c->p.grouping == HYB_GROUP_AUTO);
             else rc = do_build(c, !soft_step);
-            if (rc != HYB_OK) return rc;
+            if (rc != HYB_OK) return bail(rc);
             cudaEvent_t e2 = c->timing ? ev() : nullptr;
             if (soft_step) rc = do_soft(c); else rc = do_hard(c);
-            if (rc != HYB_OK) return rc;
+            if (rc != HYB_OK) return bail(rc);
             cudaEvent_t e3 = c->timing ? ev() : nullptr;
             const bool last = k == nsub - 1;           // the closing half kick of the other substeps is fused above
             if (last) {
                 if (split) e = launch_kick_drift(c, 0.5f * dts, 0.5f * dth, 0.0f);
                 else e = launch_kick_drift(c, 0.5f * dth, 0.0f, 0.0f);
-                if (e != cudaSuccess) return cuda_fail(c, e, "kick");
+                if (e != cudaSuccess) return bail(cuda_fail(c, e, "kick"));
             }
             c->launches += last ? 2 : 1;
             if (c->timing) {
@@ -364,8 +395,8 @@ int hyb_step(hyb_ctx *ctx, int32_t n_soft_steps)
         c->acc_valid = true;
     }
     rc = hyb_sync(ctx);
-    for (auto &s : segs) { float ms = 0; cudaEventElapsedTime(&ms, s.a, s.b); c->t_acc[s.kind] += ms; }
-    for (auto e : pool) cudaEventDestroy(e);
+    if (rc == HYB_OK)
+        for (auto &s : segs) { float ms = 0; cudaEventElapsedTime(&ms, s.a, s.b); c->t_acc[s.kind] += ms; }
     c->t_acc[7] += (float)n_soft_steps;
     return rc;
 }
@@ -525,24 +556,27 @@ int hyb_let_count(hyb_ctx *ctx, int32_t ndom, const float *h_boxes, uint64_t *h_
     Ctx *c = reinterpret_cast<Ctx *>(ctx);
     if (!c) return fail(nullptr, HYB_ERR_INVALID_ARG, "ctx is NULL");
     if (ndom < 1 || !h_boxes || !h_counts) return fail(c, HYB_ERR_INVALID_ARG, "need ndom >= 1 and two host pointers");
-    if (!c->tree_valid || c->tree_refit) return fail(c, HYB_ERR_NO_TREE, "no tree for the current positions");
+    if (!c->tree_valid || c->tree_refit || c->boxes_only)
+        return fail(c, HYB_ERR_NO_TREE, "no tree with moments for the current positions");
     if (c->p.mac != HYB_MAC_ABS) return fail(c, HYB_ERR_INVALID_ARG, "hyb_let_count needs HYB_MAC_ABS (r_b and b_max per node)");
     for (int32_t i = 0; i < ndom; i++)
         for (int a = 0; a < 3; a++)
             if (!(h_boxes[6 * i + a] < h_boxes[6 * i + 3 + a])) return fail(c, HYB_ERR_INVALID_ARG, "a domain box is empty or NaN");
     cudaSetDevice(c->device);
-    char *d = nullptr;
-    const size_t bb = sizeof(float) * 6 * (size_t)ndom, ob = sizeof(uint64_t) * 3 * (size_t)ndom;
-    cudaError_t e = cudaMalloc(&d, ((bb + 255) & ~(size_t)255) + ob);
-    if (e != cudaSuccess) return cuda_fail(c, e, "cudaMalloc");
-    unsigned long long *d_out = reinterpret_cast<unsigned long long *>(d + ((bb + 255) & ~(size_t)255));
+    // boxes and counts go through the scratch area of the workspace, as many domains at a time as fit
+    char *d = c->ws + c->L.scratch;
+    const int32_t chunk = (int32_t)imin64((int64_t)(c->L.scratch_bytes / 64), (int64_t)ndom);
     int rc = HYB_OK;
-    e = cudaMemcpyAsync(d, h_boxes, bb, cudaMemcpyHostToDevice, c->stream);
-    if (e == cudaSuccess) e = launch_let_count(c, ndom, reinterpret_cast<const float *>(d), d_out);
-    if (e == cudaSuccess) e = cudaMemcpyAsync(h_counts, d_out, ob, cudaMemcpyDeviceToHost, c->stream);
-    if (e != cudaSuccess) rc = cuda_fail(c, e, "hyb_let_count");
-    else { c->launches += 1; rc = hyb_sync(ctx); }
-    cudaFree(d);
+    for (int32_t d0 = 0; d0 < ndom && rc == HYB_OK; d0 += chunk) {
+        const int32_t nd = ndom - d0 < chunk ? ndom - d0 : chunk;
+        const size_t bb = sizeof(float) * 6 * (size_t)nd, ob = sizeof(uint64_t) * 3 * (size_t)nd;
+        unsigned long long *d_out = reinterpret_cast<unsigned long long *>(d + 32 * (size_t)chunk);
+        cudaError_t e = cudaMemcpyAsync(d, h_boxes + 6 * (size_t)d0, bb, cudaMemcpyHostToDevice, c->stream);
+        if (e == cudaSuccess) e = launch_let_count(c, nd, reinterpret_cast<const float *>(d), d_out);
+        if (e == cudaSuccess) e = cudaMemcpyAsync(h_counts + 3 * (size_t)d0, d_out, ob, cudaMemcpyDeviceToHost, c->stream);
+        if (e != cudaSuccess) rc = cuda_fail(c, e, "hyb_let_count");
+        else { c->launches += 1; rc = hyb_sync(ctx); }
+    }
     return rc;
 }
 
@@ -554,15 +588,13 @@ int hyb_energy(hyb_ctx *ctx, double *h_energy)
     cudaSetDevice(c->device);
     u32 ni, nj, nk;
     const size_t nd = energy_scratch_doubles(c, &ni, &nj, &nk);
-    double *d = nullptr;
-    cudaError_t e = cudaMalloc(&d, nd * sizeof(double));
-    if (e != cudaSuccess) return cuda_fail(c, e, "cudaMalloc");
+    if (nd * sizeof(double) > c->L.scratch_bytes) return fail(c, HYB_ERR_INTERNAL, "energy scratch does not fit the workspace");
+    double *d = reinterpret_cast<double *>(c->ws + c->L.scratch);
     int rc = HYB_OK;
-    e = launch_energy(c, d, ni, nj, nk);
+    cudaError_t e = launch_energy(c, d, ni, nj, nk);
     if (e == cudaSuccess) e = cudaMemcpyAsync(h_energy, d, 2 * sizeof(double), cudaMemcpyDeviceToHost, c->stream);
     if (e != cudaSuccess) rc = cuda_fail(c, e, "hyb_energy");
     else { c->launches += 3; rc = hyb_sync(ctx); }
-    cudaFree(d);
     return rc;
 }
 
@@ -577,6 +609,8 @@ void hyb_free(hyb_ctx *ctx)
     Ctx *c = reinterpret_cast<Ctx *>(ctx);
     if (!c) return;
     for (int i = 0; i < 5; i++) if (c->ev[i]) cudaEventDestroy(c->ev[i]);
+    for (size_t i = 0; i < c->evpool_n; i++) cudaEventDestroy(c->evpool[i]);
+    free(c->evpool);
     if (c->aux) { cudaStreamSynchronize(c->aux); cudaStreamDestroy(c->aux); }
     cudaEvent_t evs[4] = {c->ev_sorted, c->ev_perm, c->ev_linked, c->ev_groups};
     for (int i = 0; i < 4; i++) if (evs[i]) cudaEventDestroy(evs[i]);

@@ -130,6 +130,7 @@ struct Layout {   // byte offsets into the workspace; computed by plan_workspace
     size_t gfirst, gcount, glo, ghi, ncell, npart, nhard;   // [group_cap]
     size_t gnode, ganc;         // u32[group_cap]: tree node a group hangs from; start node of its hard walk
     size_t splitq;              // u32[4 group_cap]: sink ranges of split groups, processed first (walk.cu)
+    size_t scratch, scratch_bytes; // hyb_energy / hyb_let_count
     size_t zero_begin, zero_end; // look-back statuses and group flags: cleared by one memset per build
     size_t total;
     int64_t n, node_cap, group_cap;
@@ -163,6 +164,8 @@ struct Ctx {
     int grouping_now;              // HYB_GROUP_NODE / SIBLINGS of the build being enqueued
     bool boxes_only;               // the build being enqueued is read by a hard walk only: no moments
     cudaEvent_t ev[5];
+    cudaEvent_t *evpool;           // stage timers of hyb_step, kept between calls
+    size_t evpool_n;
     float t_acc[8];
     bool timing;
     unsigned long long launches;   // kernels launched since hyb_init
@@ -170,6 +173,17 @@ struct Ctx {
     // typed views of the workspace
     DevCtl *ctl;
 };
+
+// Per-device one-time set-up (function attributes, constant tables): bit d of *mask says device d is done.
+// Two threads may both do the set-up; that is harmless.
+static inline bool device_ready(const unsigned long long *mask, int device)
+{
+    return (__atomic_load_n(mask, __ATOMIC_ACQUIRE) >> (device & 63)) & 1ull;
+}
+static inline void device_set_ready(unsigned long long *mask, int device)
+{
+    __atomic_fetch_or(mask, 1ull << (device & 63), __ATOMIC_RELEASE);
+}
 
 template <typename T>
 static inline T *wsptr(const Ctx *c, size_t off) { return reinterpret_cast<T *>(c->ws + off); }

@@ -585,6 +585,9 @@ cudaError_t launch_build_tree(Ctx *c)
     // one memset: the build block of the control words, the look-back statuses and the group flags
     char *zb = reinterpret_cast<char *>(ctl) + offsetof(DevCtl, build_zero_begin);
     cudaMemsetAsync(zb, 0, (size_t)((c->ws + L.zero_end) - zb), st);
+    // the queue of sink ranges this build fills for the next hard walk (ginfo_kernel): a build that no walk
+    // consumed (two builds in a row) must not leave its entries behind
+    if (c->p.split) cudaMemsetAsync(&ctl->nheavy[c->walk_par], 0, sizeof(u32), st);
 
     cudaError_t e = launch_keys_sort_permute(c);
     if (e != cudaSuccess) return e;
@@ -602,7 +605,7 @@ cudaError_t launch_build_tree(Ctx *c)
     const int ngrid = (int)imin64(L.node_tiles, (int64_t)c->num_sms * 3);
     e = launch_radix_pass<unsigned char>(pre_level, nullptr, level, pre_of_bfs, bfs_of_pre, 0, &ctl->nn, 0,
                                          ctl->node_base, wsptr<u32>(c, L.node_status), (u32)L.node_tiles, &ctl->tile_counter[10],
-                                         &ctl->status, ngrid, st);
+                                         &ctl->status, ngrid, st, c->device);
     if (e != cudaSuccess) return e;
 
     u32 *first = wsptr<u32>(c, L.first), *count = wsptr<u32>(c, L.count), *child = wsptr<u32>(c, L.child);

@@ -199,14 +199,14 @@ __global__ void __launch_bounds__(RS_THREADS) radix_pass_kernel(
 template <typename KeyT>
 static cudaError_t launch_radix_pass(const KeyT *kin, const u32 *vin, KeyT *kout, u32 *vout, u32 *inv_out, u32 n_host,
                                      const u32 *n_dev, int shift, const u32 *digit_base, u32 *status, u32 tiles_alloc,
-                                     u32 *tile_counter, u32 *dev_status, int grid, cudaStream_t st)
+                                     u32 *tile_counter, u32 *dev_status, int grid, cudaStream_t st, int device)
 {
-    static bool attr_set = false;
-    if (!attr_set) {
+    static unsigned long long ready = 0ull;
+    if (!device_ready(&ready, device)) {
         cudaError_t e = cudaFuncSetAttribute(radix_pass_kernel<KeyT>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                              (int)sizeof(RadixSmem));
         if (e != cudaSuccess) return e;
-        attr_set = true;
+        device_set_ready(&ready, device);
     }
     return launch_pdl(radix_pass_kernel<KeyT>, dim3((unsigned)grid), dim3(RS_THREADS), sizeof(RadixSmem), st, kin, vin, kout, vout,
                       inv_out, n_host, n_dev, shift, digit_base, status, tiles_alloc, tile_counter, dev_status);

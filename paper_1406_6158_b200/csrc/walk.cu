@@ -478,15 +478,15 @@ static cudaError_t launch_walk_mode(Ctx *c, const WalkArgs &a)
 {
     using SL = SmemLayout<MODE>;
     const size_t smem = SL::bytes * WK_WARPS;
-    static bool attr_set = false;
-    if (!attr_set) {
+    static unsigned long long ready = 0ull;
+    if (!device_ready(&ready, c->device)) {
         ushort4 t[65];
         sink_layout(t);
         cudaError_t e = cudaMemcpyToSymbol(c_layout, t, sizeof t);
         if (e != cudaSuccess) return e;
         e = cudaFuncSetAttribute(walk_kernel<MODE, KF, TREE, CUT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
-        attr_set = true;
+        device_set_ready(&ready, c->device);
     }
     walk_kernel<MODE, KF, TREE, CUT><<<c->num_sms * SL::ctas_per_sm, WK_WARPS * 32, smem, c->stream>>>(a);
     return cudaGetLastError();

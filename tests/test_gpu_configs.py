@@ -35,10 +35,10 @@ def test_cfg1_full(mac):
     h.close()
 
 
-@pytest.mark.parametrize("mac", [0, 1])
-def test_cfg2_full(mac):
-    """the configuration bench.py times (N = 2^20 Hernquist), every particle."""
-    cfg = CONFIGS[2]
+@pytest.mark.parametrize("mac,hard_cut", [(0, 1), (1, 1), (0, 0)])
+def test_cfg2_full(mac, hard_cut):
+    """the configuration bench.py times (N = 2^20 Hernquist), every particle; both readings of the hard list (R30)."""
+    cfg = CONFIGS[2].with_(hard_cut=hard_cut)
     pos, vel = make_ic(cfg.kind, cfg.n, cfg.seed)
     h = make_hyb(cfg, pos, vel, mac=mac)
     h.build_tree(); h.sync()

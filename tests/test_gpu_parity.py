@@ -22,12 +22,13 @@ def _run_case(cfg, pos, vel, **over):
     return res
 
 
+@pytest.mark.parametrize("hard_cut", [1, 0])
 @pytest.mark.parametrize("grouping", [1, 0])
 @pytest.mark.parametrize("mac", [0, 1])
-def test_cfg0_all_stages(mac, grouping):
+def test_cfg0_all_stages(mac, grouping, hard_cut):
     cfg = CONFIGS[0]
     pos, vel = make_ic(cfg.kind, cfg.n, cfg.seed)
-    print(_run_case(cfg, pos, vel, mac=mac, grouping=grouping))
+    print(_run_case(cfg, pos, vel, mac=mac, grouping=grouping, hard_cut=hard_cut))
 
 
 def test_cfg0_normal_tree():
@@ -41,8 +42,8 @@ def test_cfg0_normal_tree():
                                                (1, "cold_sphere", 8, 32), (2, "cold_sphere", 8, 32),
                                                (37, "plummer", 8, 32)])
 def test_ragged_sizes(n, kind, leaf, group):
-    for grouping in (1, 0):
-        cfg = CONFIGS[1].with_(n=n, kind=kind, leaf_max=leaf, group_max=group, grouping=grouping)
+    for grouping, hard_cut in ((1, 1), (0, 1), (1, 0)):
+        cfg = CONFIGS[1].with_(n=n, kind=kind, leaf_max=leaf, group_max=group, grouping=grouping, hard_cut=hard_cut)
         pos, vel = make_ic(kind, n, 17)
         print(_run_case(cfg, pos, vel))
 
@@ -58,6 +59,7 @@ def test_coincident_points_and_depth_limit():
     vel = np.zeros_like(pos)
     print(_run_case(cfg, pos, vel))
     print(_run_case(cfg, pos, vel, grouping=0))
+    print(_run_case(cfg, pos, vel, hard_cut=0))
 
 
 def test_theta_zero_opens_everything():
@@ -152,13 +154,14 @@ def test_error_paths_on_device():
     assert rc == -1 and not hnd.value
 
 
+@pytest.mark.parametrize("hard_cut", [1, 0])
 @pytest.mark.parametrize("kfunc", [0, 1])
-def test_paper_literal_hard_walk(kfunc):
+def test_paper_literal_hard_walk(kfunc, hard_cut):
     """hard_tree = 1: MAC-approximated hard force, K-weighted cells"""
     for cfg, seed in ((CONFIGS[0].with_(r_out=0.25, r_in=0.02, theta=0.6), 0), (CONFIGS[1].with_(n=40013, r_out=0.15), 9),
                       (CONFIGS[0].with_(n=777, theta=0.0), 3)):
         pos, vel = make_ic(cfg.kind, cfg.n, seed)
-        print(_run_case(cfg, pos, vel, hard_tree=1, kfunc=kfunc))
+        print(_run_case(cfg, pos, vel, hard_tree=1, kfunc=kfunc, hard_cut=hard_cut))
     cfg = CONFIGS[0].with_(hard_tree=1, r_out=0.2)
     pos, vel = make_ic(cfg.kind, cfg.n, 5)
     h = make_hyb(cfg, pos, vel)

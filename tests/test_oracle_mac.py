@@ -69,8 +69,9 @@ def _arrays(t):
                                   "ghi", "gfirst", "gcount")}
 
 
-def expected_lists(a, g, mode, r_out):
-    """the T12/T13 lists of group g as sets, from whole-array predicates"""
+def expected_lists(a, g, mode, r_out, in_cut=None):
+    """the T12/T13 lists of group g as sets, from whole-array predicates; in_cut (hard_cut = 1, R30): the
+    particles that are themselves within r_out of the group box, as a boolean array over all particles"""
     glo, ghi = a["glo"][g].astype(F), a["ghi"][g].astype(F)
     d2a = _point_box_d2(a["com_m"][:, :3].astype(F), glo, ghi)
     d2b = _box_box_d2(a["nlo"].astype(F), a["nhi"].astype(F), glo, ghi)
@@ -92,16 +93,20 @@ def expected_lists(a, g, mode, r_out):
         rng = range(int(a["first"][k]), int(a["first"][k] + a["count"][k]))
         parts.update(rng)
         if mode != O.MODE_NORMAL and near[k]:
-            hard.update(rng)
+            hard.update(j for j in rng if in_cut is None or in_cut[j])
     return cells, parts, hard
 
 
-def check_tree_lists(walk_lists, a, ng, r_out, step):
+def check_tree_lists(walk_lists, a, ng, r_out, step, ps=None):
+    """ps: sorted positions when the oracle under test was built with hard_cut = 1"""
     bad = 0
     for mode in (O.MODE_HYBRID, O.MODE_NORMAL, O.MODE_HARD):
         for g in range(0, ng, step):
             cells, parts, hard = walk_lists(mode, g)
-            ec, ep, eh = expected_lists(a, g, mode, r_out)
+            in_cut = None
+            if ps is not None:
+                in_cut = _point_box_d2(ps[:, :3].astype(F), a["glo"][g].astype(F), a["ghi"][g].astype(F)) < F(r_out) * F(r_out)
+            ec, ep, eh = expected_lists(a, g, mode, r_out, in_cut)
             got_hard = set(parts[hard].tolist())
             if mode == O.MODE_HARD:
                 cells = cells[:0]           # the hard walk reports no cell list
@@ -112,13 +117,13 @@ def check_tree_lists(walk_lists, a, ng, r_out, step):
     return bad
 
 
-@pytest.mark.parametrize("mac", [0, 1])
-def test_walk_lists_are_the_sets_the_rule_defines(mac):
-    cfg = CONFIGS[0].with_(mac=mac)
+@pytest.mark.parametrize("mac,hard_cut", [(0, 0), (1, 0), (0, 1)])
+def test_walk_lists_are_the_sets_the_rule_defines(mac, hard_cut):
+    cfg = CONFIGS[0].with_(mac=mac, hard_cut=hard_cut)
     pos, _ = make_ic(cfg.kind, cfg.n, cfg.seed)
     t = O.Tree(pos, O.params_from(cfg))
     a = _arrays(t)
-    assert check_tree_lists(t.walk_lists, a, t.ng, cfg.r_out, 5) == 0
+    assert check_tree_lists(t.walk_lists, a, t.ng, cfg.r_out, 5, t.get("pos_sorted") if hard_cut else None) == 0
     # the accepted cells really are far (rule (a)) and every ancestor of a list entry really was opened:
     # restated per entry, as PAPER.md:66 puts it
     glo, ghi = a["glo"], a["ghi"]
@@ -251,7 +256,7 @@ def test_mutants_are_caught(name, tmp_path):
     M.orc_walk_lists.restype = C.c_int
     M.orc_walk_lists.argtypes = [C.c_void_p, C.c_int, C.c_int64, C.c_void_p, C.c_int64, C.c_void_p, C.c_void_p, C.c_void_p,
                                  C.c_int64, C.c_void_p]
-    cfg = CONFIGS[0]
+    cfg = CONFIGS[0].with_(hard_cut=0)
     pos, _ = make_ic(cfg.kind, cfg.n, cfg.seed)
     P = O.params_from(cfg)
     t = O.Tree(pos, P)                       # tree arrays do not depend on the walk tests

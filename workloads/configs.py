@@ -31,7 +31,7 @@ class Config:
 
     hard_refit: int = 0          # 0 = tree rebuilt before every force evaluation (paper), 1 = hard-only substeps refit the boxes
 
-    hard_cut: int = 0            # T13 hard list: 0 = every particle of a leaf within r_out of the group box,
+    hard_cut: int = 1            # T13 hard list: 0 = every particle of a leaf within r_out of the group box,
                                  # 1 = only the particles that are themselves within r_out of the group box (R30)
 
     def with_(self, **kw) -> "Config":
