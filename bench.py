@@ -76,7 +76,7 @@ def oracle_sample(cfg, pos, seconds):
     t0 = time.perf_counter()
     while True:
         _, _, inter = tree.forces(O.MODE_HYBRID, gsel)
-        n_inter += inter[0] + inter[1]
+        n_inter += inter[0]                # pair evaluations: a near pair is on both lists but evaluated once
         reps += 1
         dt = time.perf_counter() - t0
         if dt >= 0.8 * seconds or reps >= 64:
@@ -85,6 +85,33 @@ def oracle_sample(cfg, pos, seconds):
             "sample": f"{reps} x fp64 soft+hard force evaluation on {len(gsel)} of {tree.ng} sink groups "
                       f"({n_inter:.3e} interactions in {dt:.2f} s; full tree build {t_build:.2f} s not included)"}, \
         (tree, gsel, n_inter, dt)
+
+
+def oracle_cycle_split(cfg, pos, vel):
+    """one soft cycle of the oracle (as it stands), stage by stage on the full workload: a full tree build and the fused
+    soft+hard force evaluation once, a hard-step tree build and a hard-only evaluation once (scaled by n_sub - 1), and the
+    kick/drift arithmetic; seconds on the host cores (SURVEY.md 8(d) 'oracle timing')."""
+    import numpy as np
+    from oracle import oracle as O
+    t = {}
+    t0 = time.perf_counter(); tree = O.Tree(pos, O.params_from(cfg)); t["build_soft_step_s"] = time.perf_counter() - t0
+    t0 = time.perf_counter(); tree.forces(O.MODE_HYBRID); t["soft_step_forces_s"] = time.perf_counter() - t0
+    del tree
+    gm = max(cfg.group_max // 2, cfg.leaf_max) if cfg.grouping == 2 else cfg.group_max
+    t0 = time.perf_counter(); tree = O.Tree(pos, O.params_from(cfg, group_max=gm)); t["build_hard_step_s"] = time.perf_counter() - t0
+    t0 = time.perf_counter(); tree.forces(O.MODE_HARD); t["hard_step_forces_s"] = time.perf_counter() - t0
+    del tree
+    x = pos[:, :3].astype(np.float64); v = vel[:, :3].astype(np.float64); a = np.zeros_like(x)
+    t0 = time.perf_counter()
+    for _ in range(cfg.n_sub):
+        v += 0.5 * a; x += 0.1 * v; v += 0.5 * a
+    t["integrate_s"] = time.perf_counter() - t0
+    k = cfg.n_sub - 1 if cfg.split else 0
+    t["cycle_s"] = (t["build_soft_step_s"] + t["soft_step_forces_s"] + k * (t["build_hard_step_s"] + t["hard_step_forces_s"])
+                    + t["integrate_s"])
+    t["what"] = (f"1 soft-step (build + fused forces) + {k} hard-steps (build + hard forces), each stage timed once on all "
+                 f"{cfg.n} particles; PAPER.md:87, 200")
+    return t
 
 
 def main():
@@ -106,6 +133,8 @@ def main():
                     help="1: the paper's MAC-approximated hard walk instead of the direct hard sum (DESIGN.md R20)")
     ap.add_argument("--hard-cut", type=int, default=None, choices=[0, 1],
                     help="hard list: 0 every particle of the leaves within r_out of the group box, 1 only the particles within r_out of it (DESIGN.md R30)")
+    ap.add_argument("--mac", type=int, default=None, choices=[0, 1],
+                    help="opening criterion: 0 theta (the configurations), 1 the paper's absolute MAC with a_err = 2^-8 (Eq. 5-6)")
     ap.add_argument("--grouping", type=int, default=None, choices=[0, 1, 2],
                     help="sink groups: 0 single tree nodes, 1 runs of sibling cells, 2 auto (the configs' default)")
     args = ap.parse_args()
@@ -127,9 +156,12 @@ def main():
         cfg = cfg.with_(hard_refit=args.hard_refit)
     if args.hard_cut is not None:
         cfg = cfg.with_(hard_cut=args.hard_cut)
+    if args.mac is not None:
+        cfg = cfg.with_(mac=args.mac)
     config = {"workload": f"{cfg.name}: {cfg.kind} N={cfg.n}, eps={cfg.eps}, theta={cfg.theta}, leaf<={cfg.leaf_max}, "
                           f"group<={cfg.group_max}, r_in={cfg.r_in}, r_out={cfg.r_out}, dt_soft=1/{round(1 / cfg.dt_soft)}, "
-                          f"n_sub={cfg.n_sub}, grouping={cfg.grouping}, hard_tree={cfg.hard_tree}, hard_refit={cfg.hard_refit}, seed {cfg.seed}",
+                          f"n_sub={cfg.n_sub}, mac={cfg.mac}, grouping={cfg.grouping}, hard_tree={cfg.hard_tree}, hard_refit={cfg.hard_refit}, "
+                          f"hard_cut={cfg.hard_cut}, seed {cfg.seed}",
               "step": "one soft cycle: n_sub tree builds + 1 fused soft/hard walk + (n_sub-1) hard walks + kick/drift",
               "l2": "256 MiB L2 flush between timed steps", "replicas": world}
 
@@ -147,7 +179,7 @@ def main():
             _, _, inter = tree.forces(O.MODE_HYBRID, gsel)
             dt = time.perf_counter() - t0
             if i >= args.warmup:
-                times.append(dt); inters.append(inter[0] + inter[1])
+                times.append(dt); inters.append(inter[0])
         value = sum(inters) / sum(times)
         cb["value"] = value
         print(json.dumps({"impl": "reference", "metric": "interactions/s", "value": value, "unit": "interactions/s",
@@ -203,7 +235,9 @@ def main():
     stage = h.export("timings").astype(np.float64)
     launches = int(h.export("counts")[6]) - launches0
     from paper_1406_6158_b200.replicas import aggregate
-    total_ms, _, value = aggregate(total_ms, float(inter[0] + inter[1]), device="cuda")     # max over ranks, sum of work
+    # pair EVALUATIONS: a near pair of a fused soft+hard walk is on the soft list and on the hard list (inter[0] and
+    # inter[1] both count it, inter[2] says how many) but is evaluated once
+    total_ms, _, value = aggregate(total_ms, float(inter[0] + inter[1] - inter[2]), device="cuda")     # max over ranks, sum of work
 
     # ---- roofline of the dominant kernel (the fused soft+hard group walk), rank 0's numbers
     K = args.steps
@@ -230,9 +264,14 @@ def main():
                 "frac_at_sampled_clock": (achieved / (N_SM * FP32_LANES * 2 * sm_mhz * 1e6 / 1e12)) if sm_mhz else None,
                 "interactions_per_s": (mono + fused_hard) / K / (soft_ms * 1e-3),
                 "flop_per_pair": {"monopole": FLOP_MONO, "k_fused": FLOP_KFUSED, "k_hard": FLOP_KHARD},
+                # the hard-only walks: pairs on the hard lists as evaluated (hard_cut = 1: particles within r_out of the group
+                # box) and as the leaf-level reading of T13 would list them (every particle of a leaf within r_out)
                 "hard_walk": {"interactions_per_s": (inter[1] - fused_hard) / max(stage[2] * 1e-3, 1e-12),
                               "tflops": FLOP_KHARD * (inter[1] - fused_hard) / max(stage[2] * 1e-3, 1e-12) / 1e12,
-                              "frac": FLOP_KHARD * (inter[1] - fused_hard) / max(stage[2] * 1e-3, 1e-12) / 1e12 / peak}}
+                              "frac": FLOP_KHARD * (inter[1] - fused_hard) / max(stage[2] * 1e-3, 1e-12) / 1e12 / peak,
+                              "frac_leaf_list_count": FLOP_KHARD * inter[3] / max(stage[2] * 1e-3, 1e-12) / 1e12 / peak,
+                              "pairs_per_walk": {"evaluated": (inter[1] - fused_hard) / K / max(cfg.n_sub - 1, 1),
+                                                 "leaf_list": inter[3] / K / max(cfg.n_sub - 1, 1)}}}
     stages = {"build_ms": stage[0] / K, "soft_ms": soft_ms, "hard_ms": stage[2] / K, "integrate_ms": stage[3] / K}
     # ---- HBM-bound stages: algorithmic bytes over the measured time, against the measured copy peak
     peaks_path = os.path.join(ROOT, "MEASURED_PEAKS.json")
@@ -259,20 +298,23 @@ def main():
         hp = torch.from_numpy(pos).pin_memory(); hv = torch.from_numpy(vel).pin_memory()
         hid = torch.arange(cfg.n, dtype=torch.int32).pin_memory()
         has = torch.empty(cfg.n, 4).pin_memory(); hah = torch.empty(cfg.n, 4).pin_memory()      # results
-        p0, v0 = hp.clone(), hv.clone()
         e_int, e_t = 0.0, 0.0
+        # the state lives in (pinned) host memory between the calls; every timed call is one soft cycle:
+        # upload pos / vel / id and the accelerations of the previous call, hyb_step(1), download all five
+        hyb_run_host(P, hp.numpy(), hv.numpy(), hid.numpy(), 0, local_rank, has.numpy(), hah.numpy())     # initial forces
         for i in range(2 + 3):
-            hp.copy_(p0); hv.copy_(v0)
             t0 = time.perf_counter()
-            _, _, it = hyb_run_host(P, hp.numpy(), hv.numpy(), hid.numpy(), 1, local_rank, has.numpy(), hah.numpy())
+            _, _, it = hyb_run_host(P, hp.numpy(), hv.numpy(), hid.numpy(), 1, local_rank, has.numpy(), hah.numpy(),
+                                    acc_valid=True)
             dt = time.perf_counter() - t0
             if i >= 2:
-                e_int += float(it.sum()); e_t += dt
+                e_int += float(it[0]) + float(it[1]) - float(it[2]); e_t += dt
         n = cfg.n
-        e2e = {"value": e_int / e_t, "unit": "interactions/s", "h2d_bytes_per_step": 36 * n,
-               "d2h_bytes_per_step": 68 * n, "ms_per_call": 1e3 * e_t / 3,
-               "what": "hyb_run_host: upload pos/vel/id, initial tree+forces, one soft cycle, download "
-                       "pos/vel/id/a_soft/a_hard; all host buffers pinned; the device buffer is kept between calls (2 untimed calls first)"}
+        e2e = {"value": e_int / e_t, "unit": "interactions/s", "h2d_bytes_per_step": 68 * n,
+               "d2h_bytes_per_step": 68 * n, "ms_per_step": 1e3 * e_t / 3,
+               "what": "hyb_run_host(acc_valid = 1), one soft cycle per call with the state in pinned host memory: upload "
+                       "pos/vel/id/a_soft/a_hard, hyb_step(1), download the same five arrays; wall clock around the call "
+                       "(2 untimed calls first; the device buffer is kept between calls)"}
 
     # ---- the same cycle with a plain (unsplit, theta-only) tree at dt_h: n_sub
     #      builds + n_sub full walks per cycle; reported beside the hybrid to show its compute ratio
@@ -331,13 +373,17 @@ def main():
     cpu_baseline = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         cpu_baseline, _ = oracle_sample(cfg, pos, args.cpu_seconds)
+        if cfg.n <= (1 << 20):
+            cpu_baseline["cycle_split"] = oracle_cycle_split(cfg, pos, vel)
 
     if rank == 0:
         print(json.dumps({
             "metric": "interactions/s", "value": value, "unit": "interactions/s", "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": total_ms / K, "higher_is_better": True, "scaling": "weak",
-            "vs_baseline": None, "dtype": "f32", "data": "synthetic", "config": config, "stages": stages,
-            "interactions_per_step": {"soft": inter[0] / K, "hard": inter[1] / K},
+            "stages": stages, "vs_baseline": None, "dtype": "f32", "data": "synthetic", "config": config,
+            "interactions_per_step": {"evaluated": (inter[0] + inter[1] - inter[2]) / K, "soft_lists": inter[0] / K,
+                                      "hard_lists": inter[1] / K, "on_both_lists_of_a_fused_walk": inter[2] / K},
+            "value_counts": "pair evaluations (a near pair of the fused walk is on both lists and counted once)",
             "roofline": roofline, "hbm_stages": hbm_stages, "normal_tree": normal, "hard_refit_variant": refit, "cpu_baseline": cpu_baseline, "e2e": e2e,
             "gpu_launches": launches,
             "clocks": {"sm_mhz": sm_mhz, "sm_max_mhz": sm_max, "reasons": sorted(clk["reasons"]),

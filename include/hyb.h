@@ -111,8 +111,10 @@ enum {
     HYB_X_NCELL = 18,      /* uint32[ng] cell-list length of the last walk                      */
     HYB_X_NPART = 19,      /* uint32[ng] particle-list length of the last walk                  */
     HYB_X_NHARD = 20,      /* uint32[ng] hard-list length of the last walk                      */
-    HYB_X_INTERACTIONS = 21,/* uint64[3] since the last read: sum over groups of members x (ncell+npart),
-                              members x nhard (all walks), members x nhard of the fused soft+hard walks */
+    HYB_X_INTERACTIONS = 21,/* uint64[4] since the last read: sum over groups of members x (ncell+npart),
+                              members x nhard (all walks), members x nhard of the fused soft+hard walks (those pairs
+                              are on both lists but evaluated once), members x npart of the hard-only walks (their
+                              hard lists at leaf granularity, whatever hard_cut is) */
     HYB_X_TIMINGS = 22,    /* float[8] ms accumulated in hyb_step since the last read:
                               build, soft walk, hard walk, integrate, 0, 0, 0, cycles           */
     HYB_X_BBOX = 23,       /* float[6] lo xyz, hi xyz of the last build                         */
@@ -208,14 +210,18 @@ int hyb_sync(hyb_ctx *ctx);
  * *written (optional) receives the byte count; too small a buffer -> HYB_ERR_INVALID_ARG. */
 int hyb_export(hyb_ctx *ctx, int32_t what, void *host_dst, size_t bytes, size_t *written);
 
-/* End-to-end convenience for HOST buffers: allocates device memory, copies the particles in,
- * runs hyb_step(n_soft_steps) (n_soft_steps = 0: one build + soft-step evaluation only), copies
- * positions, velocities, ids and both accelerations back.  The device buffer and its stream are kept for
- * the next call on the same device (freed by hyb_run_host_release, or replaced when a larger n comes);
- * concurrent calls are serialised.  Every pointer is a HOST pointer to n elements; h_interactions (optional) receives uint64[2] as HYB_X_INTERACTIONS. */
+/* End-to-end call for HOST buffers: copies the particles to the device, runs hyb_step(n_soft_steps)
+ * (n_soft_steps = 0: one build + soft-step evaluation only), copies positions, velocities, ids and both
+ * accelerations back.  acc_valid = 0: the accelerations of the incoming positions are evaluated first (one more
+ * tree build and soft-step walk); acc_valid = 1: h_a_soft / h_a_hard are INPUTS too -- the accelerations this
+ * call returned for exactly these positions the last time -- so a run whose state lives on the host advances
+ * one call per cycle with nothing computed twice.  The device buffer (particles + workspace, the library's
+ * only device allocation) and its stream are kept for the next call on the same device (freed by
+ * hyb_run_host_release, or replaced when a larger n comes); concurrent calls are serialised.  Every pointer is
+ * a HOST pointer to n elements; h_interactions (optional) receives uint64[4] as HYB_X_INTERACTIONS. */
 int hyb_run_host(const hyb_params *params, int64_t n, hyb_float4 *h_pos_m, hyb_float4 *h_vel,
                  hyb_float4 *h_a_soft, hyb_float4 *h_a_hard, uint32_t *h_id, int32_t n_soft_steps,
-                 int device, uint64_t *h_interactions);
+                 int32_t acc_valid, int device, uint64_t *h_interactions);
 
 /* Frees what hyb_run_host keeps between calls (nothing else holds device memory in this library). */
 void hyb_run_host_release(void);

@@ -22,7 +22,7 @@ EXPORTS = {
     "ropen2": (11, np.float32, 1, "nn"), "nlo": (12, np.float32, 4, "nn"), "nhi": (13, np.float32, 4, "nn"),
     "gfirst": (14, np.uint32, 1, "ng"), "gcount": (15, np.uint32, 1, "ng"), "glo": (16, np.float32, 4, "ng"),
     "ghi": (17, np.float32, 4, "ng"), "ncell": (18, np.uint32, 1, "ng"), "npart": (19, np.uint32, 1, "ng"),
-    "nhard": (20, np.uint32, 1, "ng"), "interactions": (21, np.uint64, 3, "fixed"),
+    "nhard": (20, np.uint32, 1, "ng"), "interactions": (21, np.uint64, 4, "fixed"),
     "timings": (22, np.float32, 8, "fixed"), "bbox": (23, np.float32, 6, "fixed"), "keys": (24, np.uint64, 1, "n"),
     "M64": (25, np.float64, 1, "nn"), "C64": (26, np.float64, 3, "nn"), "B2": (27, np.float64, 1, "nn"),
     "bmax": (28, np.float64, 1, "nn"),
@@ -76,7 +76,7 @@ def lib():
         L.hyb_export.restype = C.c_int
         L.hyb_export.argtypes = [vp, C.c_int32, vp, C.c_size_t, C.POINTER(C.c_size_t)]
         L.hyb_run_host.restype = C.c_int
-        L.hyb_run_host.argtypes = [C.POINTER(HybParams), C.c_int64, vp, vp, vp, vp, vp, C.c_int32, C.c_int, vp]
+        L.hyb_run_host.argtypes = [C.POINTER(HybParams), C.c_int64, vp, vp, vp, vp, vp, C.c_int32, C.c_int32, C.c_int, vp]
         L.hyb_energy.restype = C.c_int
         L.hyb_energy.argtypes = [vp, vp]
         L.hyb_let_count.restype = C.c_int
@@ -96,9 +96,11 @@ def hyb_workspace_bytes(n: int, params: HybParams) -> int:
 
 
 def hyb_run_host(params: HybParams, pos_m: np.ndarray, vel: np.ndarray, ids: np.ndarray, n_soft_steps: int,
-                 device: int = 0, a_soft: np.ndarray | None = None, a_hard: np.ndarray | None = None):
+                 device: int = 0, a_soft: np.ndarray | None = None, a_hard: np.ndarray | None = None,
+                 acc_valid: bool = False):
     """End-to-end call on HOST (NumPy / pinned torch) buffers; updates pos_m, vel, ids in place and
-    returns (a_soft, a_hard, interactions).  a_soft / a_hard: optional float32 [n,4] result buffers (pass
+    returns (a_soft, a_hard, interactions).  acc_valid: a_soft / a_hard hold the accelerations of pos_m (from the
+    previous call) and are uploaded instead of being evaluated again.  a_soft / a_hard: optional float32 [n,4] result buffers (pass
     pinned ones to keep the download off the pageable-memory path); allocated here when omitted."""
     n = pos_m.shape[0]
     if a_soft is None:
@@ -107,10 +109,10 @@ def hyb_run_host(params: HybParams, pos_m: np.ndarray, vel: np.ndarray, ids: np.
         a_hard = np.empty((n, 4), np.float32)
     for a in (a_soft, a_hard):
         assert a.dtype == np.float32 and a.shape == (n, 4) and a.flags.c_contiguous
-    inter = np.zeros(2, np.uint64)
+    inter = np.zeros(4, np.uint64)
     p = lambda a: C.c_void_p(a.ctypes.data)  # noqa: E731
-    rc = lib().hyb_run_host(C.byref(params), n, p(pos_m), p(vel), p(a_soft), p(a_hard), p(ids), n_soft_steps, device,
-                            p(inter))
+    rc = lib().hyb_run_host(C.byref(params), n, p(pos_m), p(vel), p(a_soft), p(a_hard), p(ids), n_soft_steps,
+                            int(acc_valid), device, p(inter))
     if rc != 0:
         raise HybError(rc, lib().hyb_last_error(None).decode())
     return a_soft, a_hard, inter

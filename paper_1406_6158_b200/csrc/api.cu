@@ -428,10 +428,10 @@ int hyb_export(hyb_ctx *ctx, int32_t what, void *host_dst, size_t bytes, size_t 
         if (bytes < sizeof h.bbox) return fail(c, HYB_ERR_INVALID_ARG, "buffer too small");
         memcpy(host_dst, h.bbox, sizeof h.bbox); if (written) *written = sizeof h.bbox; return HYB_OK;
     case HYB_X_INTERACTIONS: {
-        u64 v[3] = {h.inter_soft, h.inter_hard, h.inter_hard_fused};
+        u64 v[4] = {h.inter_soft, h.inter_hard, h.inter_hard_fused, h.inter_hard_leaf};
         if (bytes < sizeof v) return fail(c, HYB_ERR_INVALID_ARG, "buffer too small");
         memcpy(host_dst, v, sizeof v); if (written) *written = sizeof v;
-        cudaMemset(&c->ctl->inter_soft, 0, 3 * sizeof(u64));
+        cudaMemset(&c->ctl->inter_soft, 0, 4 * sizeof(u64));
         return HYB_OK; }
     case HYB_X_TIMINGS:
         if (bytes < sizeof c->t_acc) return fail(c, HYB_ERR_INVALID_ARG, "buffer too small");
@@ -494,7 +494,8 @@ int hyb_export(hyb_ctx *ctx, int32_t what, void *host_dst, size_t bytes, size_t 
 }
 
 int hyb_run_host(const hyb_params *params, int64_t n, hyb_float4 *h_pos_m, hyb_float4 *h_vel, hyb_float4 *h_a_soft,
-                 hyb_float4 *h_a_hard, uint32_t *h_id, int32_t n_soft_steps, int device, uint64_t *h_interactions)
+                 hyb_float4 *h_a_hard, uint32_t *h_id, int32_t n_soft_steps, int32_t acc_valid, int device,
+                 uint64_t *h_interactions)
 {
     char msg[256];
     if (!params_ok(params, n, msg)) return fail(nullptr, HYB_ERR_INVALID_ARG, msg);
@@ -522,10 +523,15 @@ int hyb_run_host(const hyb_params *params, int64_t n, hyb_float4 *h_pos_m, hyb_f
         cudaMemcpyAsync(d + o_pos, h_pos_m, 16 * N, cudaMemcpyHostToDevice, st);
         cudaMemcpyAsync(d + o_vel, h_vel, 16 * N, cudaMemcpyHostToDevice, st);
         cudaMemcpyAsync(d + o_id, h_id, 4 * N, cudaMemcpyHostToDevice, st);
+        if (acc_valid) {       // the caller continues a run: the accelerations of these positions come with them
+            cudaMemcpyAsync(d + o_as, h_a_soft, 16 * N, cudaMemcpyHostToDevice, st);
+            cudaMemcpyAsync(d + o_ah, h_a_hard, 16 * N, cudaMemcpyHostToDevice, st);
+        }
         rc = hyb_init(&ctx, params, n, (hyb_float4 *)(d + o_pos), (hyb_float4 *)(d + o_vel), (hyb_float4 *)(d + o_as),
                       (hyb_float4 *)(d + o_ah), (uint32_t *)(d + o_id), d + o_ws, ws_bytes, device, st);
         if (rc != HYB_OK) break;
         reinterpret_cast<Ctx *>(ctx)->timing = false;
+        reinterpret_cast<Ctx *>(ctx)->acc_valid = acc_valid != 0 && params->hard_refit == 0;
         rc = hyb_step(ctx, n_soft_steps);
         if (rc != HYB_OK) break;
         cudaMemcpyAsync(h_pos_m, d + o_pos, 16 * N, cudaMemcpyDeviceToHost, st);
@@ -535,9 +541,9 @@ int hyb_run_host(const hyb_params *params, int64_t n, hyb_float4 *h_pos_m, hyb_f
         cudaMemcpyAsync(h_id, d + o_id, 4 * N, cudaMemcpyDeviceToHost, st);
         if ((e = cudaStreamSynchronize(st)) != cudaSuccess) { rc = cuda_fail(nullptr, e, "copy back"); break; }
         if (h_interactions) {
-            uint64_t v[3];
+            uint64_t v[4];
             rc = hyb_export(ctx, HYB_X_INTERACTIONS, v, sizeof v, nullptr);
-            h_interactions[0] = v[0]; h_interactions[1] = v[1];
+            for (int i = 0; i < 4; i++) h_interactions[i] = v[i];
         }
     } while (0);
     if (ctx) hyb_free(ctx);

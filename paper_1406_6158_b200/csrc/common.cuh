@@ -65,6 +65,7 @@ struct DevCtl {
     u32 split_t[3];             // hard walk scheduling thresholds (pairs): queue first / cut in 2 / cut in 4 (set by hyb_init)
     u32 split_cap;              // entries the queue of sink ranges can hold
     u64 inter_soft, inter_hard, inter_hard_fused;   // pair counts: soft lists, hard lists (all walks), hard lists of fused walks
+    u64 inter_hard_leaf;        // hard-only walks: members x particles of the leaves within r_out (the hard list without the particle cut)
     // ---- bounding box reduction: filled by bbox_kernel or by the drift, cleared again by keys_kernel ----
     u32 bbox_enc[6];            // order-preserving encodings: ~min xyz, max xyz (atomicMax from 0 for both)
     u32 bbox_done;              // CTAs that have contributed (the last one derives the root cube)

@@ -88,7 +88,7 @@ __global__ void __launch_bounds__(WK_WARPS * 32, SmemLayout<MODE>::ctas_per_sm) 
     }
     const float rout2 = __fmul_rn(a.rout, a.rout);
     const float eps2 = a.eps2, kc0 = a.kc0, kc1 = a.kc1;
-    unsigned long long isoft = 0, ihard = 0;
+    unsigned long long isoft = 0, ihard = 0, ileaf = 0;
 
     // Work items come from one atomic counter.  In the hard walk the heaviest sink groups (by the
     // estimate of split_kernel) have been cut into 2 or 4 sink ranges that are handed out first, so
@@ -437,6 +437,7 @@ __global__ void __launch_bounds__(WK_WARPS * 32, SmemLayout<MODE>::ctas_per_sm) 
             if (rsub == 0) { a.ncell[g] = ncell; a.npart[g] = npart; a.nhard[g] = nhard; }
             if (MODE != WALK_HARD) isoft += (unsigned long long)n * (unsigned long long)(ncell + npart);
             if (MODE != WALK_NORMAL) ihard += (unsigned long long)n * (unsigned long long)nhard;
+            if (MODE == WALK_HARD) ileaf += (unsigned long long)n * (unsigned long long)npart;
         }
         item = __shfl_sync(FULL, item_next, 0);
     }
@@ -444,6 +445,7 @@ __global__ void __launch_bounds__(WK_WARPS * 32, SmemLayout<MODE>::ctas_per_sm) 
         if (isoft) atomicAdd(&a.ctl->inter_soft, isoft);
         if (ihard) atomicAdd(&a.ctl->inter_hard, ihard);
         if (ihard && MODE == WALK_HYBRID) atomicAdd(&a.ctl->inter_hard_fused, ihard);
+        if (ileaf) atomicAdd(&a.ctl->inter_hard_leaf, ileaf);
     }
 }
 

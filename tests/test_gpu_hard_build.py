@@ -155,3 +155,23 @@ def test_no_device_allocation_after_init():
     free1, _ = torch.cuda.mem_get_info()
     assert free1 == free0, (free0, free1)
     h.close()
+
+
+def test_run_host_continues_a_run_cycle_by_cycle():
+    """hyb_run_host with the state in host memory: two calls of one cycle each (the second with acc_valid = 1)
+    give the same bits as two cycles on a device-resident context"""
+    from paper_1406_6158_b200 import HybParams, hyb_run_host
+    cfg = CONFIGS[1].with_(n=40009)
+    pos, vel = make_ic(cfg.kind, cfg.n, 31)
+    h = make_hyb(cfg, pos, vel)
+    h.step(2); h.sync()
+    P = HybParams.from_config(cfg)
+    hp, hv = pos.copy(), vel.copy()
+    ids = np.arange(cfg.n, dtype=np.int32)
+    a_s, a_h, it0 = hyb_run_host(P, hp, hv, ids, 1, 0)
+    a_s, a_h, it1 = hyb_run_host(P, hp, hv, ids, 1, 0, a_s, a_h, acc_valid=True)
+    assert np.array_equal(hp, h.pos_m.cpu().numpy()) and np.array_equal(hv, h.vel.cpu().numpy())
+    assert np.array_equal(ids, h.ids.cpu().numpy())
+    assert np.array_equal(a_s, h.a_soft.cpu().numpy()) and np.array_equal(a_h, h.a_hard.cpu().numpy())
+    assert it1[0] > 0 and it1[2] <= it1[1] and it0[0] > it1[0]          # the first call also evaluated the initial forces
+    h.close()
