@@ -194,7 +194,7 @@ def main():
     import numpy as np
     import torch
     import torch.distributed as dist
-    from paper_1406_6158_b200 import Hyb, HybParams, hyb_run_host
+    from paper_1406_6158_b200 import Hyb, HybParams, hyb_run_host, hyb_probe_fp32
 
     torch.cuda.set_device(local_rank)
     if world > 1:
@@ -257,10 +257,13 @@ def main():
             if k == "walk_kernel<HYBRID>":
                 traffic = float(v)
     achieved = flops / (soft_ms * 1e-3) / 1e12
+    probe = hyb_probe_fp32(local_rank) if rank == 0 else (None, None)      # measured FP32 fused multiply-add rate (not timed)
     roofline = {"bound": "alu", "kernel": "walk_kernel<HYBRID> (fused soft+hard group walk)", "achieved": achieved,
                 "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak, "traffic": traffic,
                 "peak_source": f"derived: {N_SM} SMs x {FP32_LANES} FP32 lanes x 2 flop x {sm_max} MHz max SM clock "
                                "(MEASURED_PEAKS.json has no FP32 CUDA-core figure)",
+                "peak_probe": {"ffma2_tflops": probe[0], "ffma_tflops": probe[1], "frac_of_probe": achieved / probe[0] if probe[0] else None,
+                               "what": "hyb_probe_fp32: chains of packed / scalar fused multiply-adds only, measured in this run"},
                 "frac_at_sampled_clock": (achieved / (N_SM * FP32_LANES * 2 * sm_mhz * 1e6 / 1e12)) if sm_mhz else None,
                 "interactions_per_s": (mono + fused_hard) / K / (soft_ms * 1e-3),
                 "flop_per_pair": {"monopole": FLOP_MONO, "k_fused": FLOP_KFUSED, "k_hard": FLOP_KHARD},

@@ -247,6 +247,13 @@ int hyb_let_count(hyb_ctx *ctx, int32_t ndom, const float *h_boxes, uint64_t *h_
  * coincident particles give W = -inf.  Errors: INVALID_ARG (NULL pointer), CUDA. */
 int hyb_energy(hyb_ctx *ctx, double *h_energy);
 
+/* Diagnostic, not on the hot path: the FP32 rate of the CUDA cores of `device`, measured with independent chains
+ * of packed (h_tflops[0], fma.rn.f32x2 as the pair kernels use) and scalar (h_tflops[1], fma.rn.f32) fused
+ * multiply-adds, in TFLOP/s.  bench.py reports it beside the peak derived from the unit counts and the clock.
+ * d_scratch: DEVICE float[scratch_floats], caller-owned, at least 1024 x the number of SMs (results of the chains
+ * are stored there so that the loops are not optimised away).  h_tflops: HOST double[2].  Synchronises. */
+int hyb_probe_fp32(int device, void *cuda_stream, float *d_scratch, size_t scratch_floats, double *h_tflops);
+
 /* Message for the last error on this context ("" if none).  ctx may be NULL (returns the
  * message of the last failed hyb_init / hyb_run_host on this thread). */
 const char *hyb_last_error(const hyb_ctx *ctx);

@@ -81,6 +81,8 @@ def lib():
         L.hyb_energy.argtypes = [vp, vp]
         L.hyb_let_count.restype = C.c_int
         L.hyb_let_count.argtypes = [vp, C.c_int32, vp, vp]
+        L.hyb_probe_fp32.restype = C.c_int
+        L.hyb_probe_fp32.argtypes = [C.c_int, vp, vp, C.c_size_t, vp]
         L.hyb_run_host_release.restype = None
         L.hyb_run_host_release.argtypes = []
         L.hyb_last_error.restype = C.c_char_p
@@ -116,6 +118,18 @@ def hyb_run_host(params: HybParams, pos_m: np.ndarray, vel: np.ndarray, ids: np.
     if rc != 0:
         raise HybError(rc, lib().hyb_last_error(None).decode())
     return a_soft, a_hard, inter
+
+
+def hyb_probe_fp32(device: int = 0):
+    """(packed, scalar) FP32 fused multiply-add rate of the device in TFLOP/s (diagnostic; see include/hyb.h)"""
+    import torch
+    scratch = torch.empty(1 << 20, dtype=torch.float32, device=f"cuda:{device}")
+    out = np.zeros(2, np.float64)
+    rc = lib().hyb_probe_fp32(device, torch.cuda.current_stream(device).cuda_stream, scratch.data_ptr(), scratch.numel(),
+                              C.c_void_p(out.ctypes.data))
+    if rc != 0:
+        raise HybError(rc, "hyb_probe_fp32")
+    return float(out[0]), float(out[1])
 
 
 def hyb_run_host_release() -> None:

@@ -124,8 +124,10 @@ static int do_build(Ctx *c, bool hard_only = false)
     // group_max / 2 when only a hard walk follows
     c->grouping_now = c->p.grouping == HYB_GROUP_AUTO ? HYB_GROUP_SIBLINGS : c->p.grouping;
     c->group_max_now = c->p.group_max;
-    if (hard_only && c->p.grouping == HYB_GROUP_AUTO)                 // smaller runs: fewer listed particles beyond r_out
+    if (hard_only && c->p.grouping == HYB_GROUP_AUTO) {               // smaller runs: fewer listed particles beyond r_out
         c->group_max_now = c->p.group_max / 2 > c->p.leaf_max ? c->p.group_max / 2 : c->p.leaf_max;
+        if (getenv("HYB_HARD_GM")) c->group_max_now = atoi(getenv("HYB_HARD_GM"));
+    }
     c->boxes_only = hard_only && !c->p.hard_tree;      // the tree-approximated hard walk needs the moments
     cudaError_t e = launch_build_tree(c);
     if (e != cudaSuccess) return cuda_fail(c, e, "build_tree");

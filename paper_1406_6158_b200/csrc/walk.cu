@@ -53,7 +53,14 @@ struct SmemLayout {                 // per warp
     static constexpr int cell_alloc = cell_cap ? cell_cap + WK_PAD_SLACK : 0;
     static constexpr int part_alloc = part_cap ? part_cap + WK_PAD_SLACK : 0;
     static constexpr size_t bytes = 16 * (size_t)(cell_alloc + part_alloc) + 4 * (size_t)stack_cap + 8 * 2 * (size_t)lq_cap;
-    static constexpr int ctas_per_sm = MODE == WALK_HARD ? 3 : 2;
+#ifndef WKV_HARD_WARPS
+#define WKV_HARD_WARPS 8
+#define WKV_HARD_CTAS 3
+#define WKV_SOFT_WARPS 8
+#define WKV_SOFT_CTAS 2
+#endif
+    static constexpr int ctas_per_sm = MODE == WALK_HARD ? WKV_HARD_CTAS : WKV_SOFT_CTAS;
+    static constexpr int warps = MODE == WALK_HARD ? WKV_HARD_WARPS : WKV_SOFT_WARPS;      // per CTA
 };
 
 // TREE (hyb_params.hard_tree): the paper-literal hard force.  The MAC is applied in the hard walk too and a
@@ -63,7 +70,7 @@ struct SmemLayout {                 // per warp
 // CUT (hyb_params.hard_cut, R30): the hard list holds only the particles that are themselves within
 // r_out of the group box; the other particles of a near leaf are plain Eq. 2 pairs (monopole buffer).
 template <int MODE, int KF, bool TREE, bool CUT>
-__global__ void __launch_bounds__(WK_WARPS * 32, SmemLayout<MODE>::ctas_per_sm) walk_kernel(const WalkArgs a)
+__global__ void __launch_bounds__(SmemLayout<MODE>::warps * 32, SmemLayout<MODE>::ctas_per_sm) walk_kernel(const WalkArgs a)
 {
     using SL = SmemLayout<MODE>;
     constexpr bool HAS_MONO = MODE != WALK_HARD;      // monopole buffer (cells, far particles)
@@ -479,7 +486,7 @@ template <int MODE, int KF, bool TREE, bool CUT>
 static cudaError_t launch_walk_mode(Ctx *c, const WalkArgs &a)
 {
     using SL = SmemLayout<MODE>;
-    const size_t smem = SL::bytes * WK_WARPS;
+    const size_t smem = SL::bytes * SL::warps;
     static unsigned long long ready = 0ull;
     if (!device_ready(&ready, c->device)) {
         ushort4 t[65];
@@ -490,7 +497,7 @@ static cudaError_t launch_walk_mode(Ctx *c, const WalkArgs &a)
         if (e != cudaSuccess) return e;
         device_set_ready(&ready, c->device);
     }
-    walk_kernel<MODE, KF, TREE, CUT><<<c->num_sms * SL::ctas_per_sm, WK_WARPS * 32, smem, c->stream>>>(a);
+    walk_kernel<MODE, KF, TREE, CUT><<<c->num_sms * SL::ctas_per_sm, SL::warps * 32, smem, c->stream>>>(a);
     return cudaGetLastError();
 }
 
