@@ -133,6 +133,9 @@ def main():
                     help="1: the paper's MAC-approximated hard walk instead of the direct hard sum (DESIGN.md R20)")
     ap.add_argument("--hard-cut", type=int, default=None, choices=[0, 1],
                     help="hard list: 0 every particle of the leaves within r_out of the group box, 1 only the particles within r_out of it (DESIGN.md R30)")
+    ap.add_argument("--sharded", action="store_true",
+                    help="N > 1: ONE problem with its sinks divided over the ranks (sharded.py, strong scaling) instead of "
+                         "independent replicas; unmeasured on hardware, not the headline")
     ap.add_argument("--mac", type=int, default=None, choices=[0, 1],
                     help="opening criterion: 0 theta (the configurations), 1 the paper's absolute MAC with a_err = 2^-8 (Eq. 5-6)")
     ap.add_argument("--grouping", type=int, default=None, choices=[0, 1, 2],
@@ -200,6 +203,39 @@ def main():
     if world > 1:
         dist.init_process_group("nccl")
     from paper_1406_6158_b200.replicas import replica_seed
+    if args.sharded:
+        # ---- sink-sharded variant: every rank holds all particles, evaluates its share of the sink
+        #      groups, one all-reduce of the accelerations after each force evaluation
+        from types import SimpleNamespace
+        from paper_1406_6158_b200.sharded import ShardedHyb
+        pos, vel = make_ic(cfg.kind, cfg.n, cfg.seed)
+        h = Hyb(HybParams.from_config(cfg), torch.from_numpy(pos).cuda(), torch.from_numpy(vel).cuda())
+        ar = (lambda t: dist.all_reduce(t)) if world > 1 else (lambda t: None)
+        sh = ShardedHyb(h, SimpleNamespace(split=cfg.split, n_sub=cfg.n_sub, dt_soft=cfg.dt_soft), rank, world, ar)
+        for _ in range(args.warmup + 1):
+            sh.step(1)
+        h.sync(); h.export("interactions")
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(args.steps):
+            sh.step(1)
+        e1.record(); h.sync(); torch.cuda.synchronize()
+        it = h.export("interactions").astype(np.float64)
+        from paper_1406_6158_b200.replicas import aggregate
+        ms, _, value = aggregate(e0.elapsed_time(e1), float(it[0] + it[1] - it[2]), device="cuda")
+        if rank == 0:
+            config["parallelism"] = f"sink-sharded x{world}: replicated particles and tree, all-reduce of a_soft / a_hard"
+            print(json.dumps({"metric": "interactions/s", "value": value, "unit": "interactions/s", "n_gpus": world,
+                              "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms / args.steps,
+                              "higher_is_better": True, "scaling": "strong", "vs_baseline": None, "dtype": "f32",
+                              "data": "synthetic", "config": config, "note": "variant, unmeasured on more than one GPU"}))
+        h.close()
+        if world > 1:
+            dist.destroy_process_group()
+        return
     pos, vel = make_ic(cfg.kind, cfg.n, replica_seed(cfg.seed, rank))      # independent replica per rank
     P = HybParams.from_config(cfg)
     dpos = torch.from_numpy(pos).cuda(); dvel = torch.from_numpy(vel).cuda()

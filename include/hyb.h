@@ -200,6 +200,22 @@ int hyb_hard_force(hyb_ctx *ctx);
  * end to read the device status word (capacity overflow, non-finite input). */
 int hyb_step(hyb_ctx *ctx, int32_t n_soft_steps);
 
+/* Sink-sharded evaluation (PAPER.md:113-122 without the LET: every replica holds all
+ * particles and builds the same tree, the sinks are divided).  After this call hyb_soft_force / hyb_hard_force
+ * evaluate only the sink groups whose first particle lies in store slots [first, last) -- groups are never cut,
+ * so the ranges of the replicas tile the groups when they tile [0, n) -- and write ZERO accelerations for all
+ * other sinks, so that the element-wise sum over the replicas (one all-reduce, or an all-gather of the owned
+ * ranges) is the full result, bit for bit.  hyb_step refuses a partial range: the caller runs the cycle with
+ * hyb_kick_drift / hyb_build_tree(_hard) / hyb_soft_force / hyb_hard_force and exchanges in between
+ * (paper_1406_6158_b200/sharded.py).  Default [0, n).  Errors: INVALID_ARG. */
+int hyb_set_sink_range(hyb_ctx *ctx, int64_t first, int64_t last);
+
+/* Step a10 alone (Eq. 3-4): v += c_soft a_soft + c_hard a_hard;  x += dt v  for every
+ * particle (dt = 0: kick only), with the accelerations as they are in d_a_soft / d_a_hard now.  The building
+ * block of hyb_step's cycle (R21) for callers that run the cycle themselves.  dt != 0 invalidates the tree.
+ * Asynchronous.  Errors: INVALID_ARG (non-finite coefficient), CUDA. */
+int hyb_kick_drift(hyb_ctx *ctx, float c_soft, float c_hard, float dt);
+
 /* Synchronise the stream and return the device status as an error code.  An error (non-finite input, capacity
  * overflow) is reported once: the status word is cleared, the tree and the accelerations of the context are
  * marked invalid, and the context can be used again after the caller has repaired the input (the next

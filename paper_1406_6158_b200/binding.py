@@ -71,6 +71,10 @@ def lib():
             getattr(L, name).argtypes = [vp]
         L.hyb_set_params.restype = C.c_int
         L.hyb_set_params.argtypes = [vp, C.POINTER(HybParams)]
+        L.hyb_set_sink_range.restype = C.c_int
+        L.hyb_set_sink_range.argtypes = [vp, C.c_int64, C.c_int64]
+        L.hyb_kick_drift.restype = C.c_int
+        L.hyb_kick_drift.argtypes = [vp, C.c_float, C.c_float, C.c_float]
         L.hyb_step.restype = C.c_int
         L.hyb_step.argtypes = [vp, C.c_int32]
         L.hyb_export.restype = C.c_int
@@ -187,6 +191,12 @@ class Hyb:
 
     def hard_force(self):
         self._check(lib().hyb_hard_force(self._h))
+
+    def set_sink_range(self, first: int, last: int):
+        self._check(lib().hyb_set_sink_range(self._h, first, last))
+
+    def kick_drift(self, c_soft: float, c_hard: float, dt: float):
+        self._check(lib().hyb_kick_drift(self._h, c_soft, c_hard, dt))
 
     def step(self, n_soft_steps: int = 1):
         self._check(lib().hyb_step(self._h, n_soft_steps))

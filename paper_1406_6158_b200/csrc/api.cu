@@ -219,6 +219,7 @@ int hyb_init(hyb_ctx **out, const hyb_params *params, int64_t n, hyb_float4 *d_p
     Ctx *c = new (std::nothrow) Ctx;
     if (!c) return fail(nullptr, HYB_ERR_INTERNAL, "out of host memory");
     memset(c, 0, sizeof *c);
+    c->sink_lo = 0u; c->sink_hi = (u32)n;
     c->p = *params; c->n = n; c->device = device; c->stream = (cudaStream_t)cuda_stream;
     c->pos = d_pos_m; c->vel = d_vel; c->a_soft = d_a_soft; c->a_hard = d_a_hard; c->id = d_id;
     c->ws = (char *)d_workspace; c->L = L; c->ctl = (DevCtl *)(c->ws + L.ctl);
@@ -311,6 +312,30 @@ int hyb_hard_force(hyb_ctx *ctx)
     return do_hard(c);
 }
 
+int hyb_set_sink_range(hyb_ctx *ctx, int64_t first, int64_t last)
+{
+    Ctx *c = reinterpret_cast<Ctx *>(ctx);
+    if (!c) return fail(nullptr, HYB_ERR_INVALID_ARG, "ctx is NULL");
+    if (first < 0 || last < first || last > c->n) return fail(c, HYB_ERR_INVALID_ARG, "need 0 <= first <= last <= n");
+    c->sink_lo = (u32)first; c->sink_hi = (u32)last;
+    c->acc_valid = false;
+    return HYB_OK;
+}
+
+int hyb_kick_drift(hyb_ctx *ctx, float c_soft, float c_hard, float dt)
+{
+    Ctx *c = reinterpret_cast<Ctx *>(ctx);
+    if (!c) return fail(nullptr, HYB_ERR_INVALID_ARG, "ctx is NULL");
+    if (!isfinite(c_soft) || !isfinite(c_hard) || !isfinite(dt)) return fail(c, HYB_ERR_INVALID_ARG, "non-finite coefficient");
+    cudaSetDevice(c->device);
+    discard_pending_bbox(c);
+    cudaError_t e = launch_kick_drift(c, c_soft, c_hard, dt, false);
+    if (e != cudaSuccess) return cuda_fail(c, e, "kick_drift");
+    c->launches += 1;
+    if (dt != 0.0f) { c->tree_valid = false; c->acc_valid = false; }
+    return HYB_OK;
+}
+
 int hyb_sync(hyb_ctx *ctx)
 {
     Ctx *c = reinterpret_cast<Ctx *>(ctx);
@@ -333,6 +358,8 @@ int hyb_step(hyb_ctx *ctx, int32_t n_soft_steps)
     Ctx *c = reinterpret_cast<Ctx *>(ctx);
     if (!c) return fail(nullptr, HYB_ERR_INVALID_ARG, "ctx is NULL");
     if (n_soft_steps < 0) return fail(c, HYB_ERR_INVALID_ARG, "n_soft_steps < 0");
+    if (c->sink_lo != 0u || (int64_t)c->sink_hi != c->n)
+        return fail(c, HYB_ERR_INVALID_ARG, "hyb_step needs the full sink range: with hyb_set_sink_range the caller exchanges the accelerations between the force calls and the kicks");
     cudaSetDevice(c->device);
     const bool split = c->p.split != 0;
     const int nsub = c->p.n_sub;

@@ -149,6 +149,7 @@ struct Ctx {
     bool bbox_ready = false;    // the last drift has already reduced the bounding box of the current positions
     u32 walk_par = 0;           // slot of the walk work counters the next launch uses (DevCtl::group_counter)
     hyb_params p;
+    u32 sink_lo, sink_hi;       // hyb_set_sink_range: the sinks this context evaluates (store slots), default all
     int64_t n;
     int device;
     cudaStream_t stream;

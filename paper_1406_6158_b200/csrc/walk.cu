@@ -36,6 +36,7 @@ struct WalkArgs {
     const unsigned char *is_split; // hard walk: group is handled as ranges
     float4 *a_soft, *a_hard;
     DevCtl *ctl;
+    u32 sink_lo, sink_hi;            // only groups whose first sink lies in [sink_lo, sink_hi) are evaluated
     float G, eps2, rout, kc0, kc1;   // Y = sat(kc0 + kc1 r)
     unsigned long long zero64;       // 0, passed as an argument so that it is opaque to the compiler
 };
@@ -123,9 +124,14 @@ __global__ void __launch_bounds__(SmemLayout<MODE>::warps * 32, SmemLayout<MODE>
                 continue;
             }
         }
+        const u32 gf0 = a.gfirst[g];
+        if (gf0 < a.sink_lo || gf0 >= a.sink_hi) {             // another replica's sinks (hyb_set_sink_range)
+            item = __shfl_sync(FULL, item_next, 0);
+            continue;
+        }
         const u32 n_all = a.gcount[g];
         const u32 n_rng = (n_all + nsub - 1u) / nsub;                  // sinks per range
-        const u32 gf = a.gfirst[g] + rsub * n_rng;
+        const u32 gf = gf0 + rsub * n_rng;
         const int n = (int)(min(n_all, (rsub + 1u) * n_rng) - rsub * n_rng);
         const float4 glo = a.glo[g], ghi = a.ghi[g];
         // sinks per lane S in {2,3,4}, lanes per copy A = ceil(n / S), copies P: from the table of
@@ -516,6 +522,11 @@ cudaError_t launch_walk(Ctx *c, int mode)
     const float w = c->p.r_out - c->p.r_in;
     a.kc0 = c->p.r_out / w; a.kc1 = -1.0f / w;
     a.zero64 = 0ull;
+    a.sink_lo = c->sink_lo; a.sink_hi = c->sink_hi;
+    if (c->sink_lo > 0u || (int64_t)c->sink_hi < c->n) {      // a sink range: everything outside it reads zero
+        if (mode != WALK_HARD) cudaMemsetAsync(c->a_soft, 0, sizeof(hyb_float4) * (size_t)c->n, c->stream);
+        cudaMemsetAsync(c->a_hard, 0, sizeof(hyb_float4) * (size_t)c->n, c->stream);
+    }
     a.heavy = wsptr<u32>(c, L.splitq);
     a.ganc = c->tree_refit ? nullptr : wsptr<u32>(c, L.ganc);      // refitted boxes: the Morton cells are stale
     a.is_split = wsptr<unsigned char>(c, L.gflag);      // the build's flag array is free between builds

@@ -1,0 +1,65 @@
+"""-m gpu: the sink-sharded evaluation on one GPU (hyb_set_sink_range, hyb_kick_drift, sharded.ShardedHyb).
+One GPU is all the pool offers, so the ranks are emulated one after the other (no kernel waits on another):
+the sum over complementary sink ranges is the full result bit for bit, and the call-by-call cycle equals
+hyb_step bit for bit."""
+import numpy as np
+import pytest
+import torch
+
+from workloads import CONFIGS, make_ic
+
+pytestmark = pytest.mark.gpu
+
+from gpu_util import make_hyb  # noqa: E402
+
+
+def test_ranges_sum_to_the_full_result():
+    cfg = CONFIGS[2].with_(n=200003)
+    pos, vel = make_ic(cfg.kind, cfg.n, 3)
+    h = make_hyb(cfg, pos, vel)
+    h.build_tree(); h.soft_force(); h.sync()
+    full_s, full_h = h.a_soft.clone(), h.a_hard.clone()
+    want = h.export("interactions")
+    h.hard_force(); h.sync()
+    full_h2 = h.a_hard.clone()
+    h.export("interactions")
+    from paper_1406_6158_b200.sharded import sink_ranges
+    for world in (2, 3):
+        b = sink_ranges(cfg.n, world)
+        sum_s, sum_h, sum_h2 = torch.zeros_like(full_s), torch.zeros_like(full_h), torch.zeros_like(full_h)
+        got = np.zeros(4, np.uint64)
+        for r in range(world):
+            h.set_sink_range(b[r], b[r + 1])
+            h.soft_force(); h.sync()
+            nz = (h.a_soft.abs().sum(dim=1) > 0).nonzero().flatten()
+            assert nz.numel() > 0
+            sum_s += h.a_soft; sum_h += h.a_hard
+            got += h.export("interactions")
+            h.hard_force(); h.sync()
+            sum_h2 += h.a_hard
+            h.export("interactions")
+        assert torch.equal(sum_s, full_s) and torch.equal(sum_h, full_h)
+        assert np.array_equal(got[:3], want[:3])                         # every pair evaluated by exactly one rank
+        # hard-only walk: heavy groups are cut into sink ranges whose partial sums combine in another order
+        assert float((sum_h2 - full_h2).norm() / full_h2.norm()) < 1e-6
+    from paper_1406_6158_b200 import HybError
+    with pytest.raises(HybError):
+        h.step(1)                                                        # a partial range needs the caller's exchange
+    h.set_sink_range(0, cfg.n)
+    h.close()
+
+
+@pytest.mark.parametrize("split", [1, 0])
+def test_call_by_call_cycle_equals_hyb_step(split):
+    from types import SimpleNamespace
+    from paper_1406_6158_b200.sharded import ShardedHyb
+    cfg = CONFIGS[1].with_(n=50021, split=split)
+    pos, vel = make_ic(cfg.kind, cfg.n, 8)
+    ref = make_hyb(cfg, pos, vel)
+    ref.step(2); ref.sync()
+    h = make_hyb(cfg, pos, vel)
+    sh = ShardedHyb(h, SimpleNamespace(split=cfg.split, n_sub=cfg.n_sub, dt_soft=cfg.dt_soft), 0, 1, lambda t: None)
+    sh.step(2); h.sync()
+    for a, b in ((h.pos_m, ref.pos_m), (h.vel, ref.vel), (h.a_soft, ref.a_soft), (h.a_hard, ref.a_hard), (h.ids, ref.ids)):
+        assert torch.equal(a, b)
+    h.close(); ref.close()
