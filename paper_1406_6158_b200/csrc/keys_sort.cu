@@ -39,7 +39,7 @@ __device__ __forceinline__ u32 quantise(float x, double o, double inv)
     return f >= 2097151.0 ? 2097151u : (f > 0.0 ? (u32)f : 0u);
 }
 
-// also accumulates the eight 8-bit digit histograms the onesweep sort needs
+// also accumulates the eight 8-bit digit histograms the onesweep sort needs; its last CTA turns them into bases
 __global__ void __launch_bounds__(256) keys_kernel(const float4 *__restrict__ pos, u32 n, DevCtl *ctl,
                                                    u64 *__restrict__ key)
 {
@@ -60,23 +60,27 @@ __global__ void __launch_bounds__(256) keys_kernel(const float4 *__restrict__ po
     __syncthreads();
     for (int i = threadIdx.x; i < RS_PASSES * 256; i += blockDim.x)
         if (hist[i]) atomicAdd(&ctl->digit_hist[i], hist[i]);
-}
-
-// exclusive scan of each 256-bin histogram -> digit_base.  One CTA of 256 threads per pass.
-__global__ void __launch_bounds__(256) digit_base_kernel(DevCtl *ctl)
-{
-    __shared__ u32 s[256];
-    const u32 *h = ctl->digit_hist + blockIdx.x * 256;
-    u32 v = h[threadIdx.x];
-    s[threadIdx.x] = v;
+    // the last CTA to get here sees the complete histograms: exclusive scan of each 256-bin histogram -> digit_base
+    __shared__ bool last;
+    __threadfence();
     __syncthreads();
-    for (int off = 1; off < 256; off <<= 1) {
-        u32 t = threadIdx.x >= off ? s[threadIdx.x - off] : 0;
+    if (threadIdx.x == 0) last = atomicAdd(&ctl->tile_counter[13], 1u) == gridDim.x - 1;
+    __syncthreads();
+    if (!last) return;
+    __threadfence();
+    for (int pass = 0; pass < RS_PASSES; pass++) {
+        const u32 v = ld_volatile_u32(&ctl->digit_hist[pass * 256 + threadIdx.x]);
+        hist[threadIdx.x] = v;
         __syncthreads();
-        s[threadIdx.x] += t;
+        for (int off = 1; off < 256; off <<= 1) {
+            const u32 t = threadIdx.x >= off ? hist[threadIdx.x - off] : 0;
+            __syncthreads();
+            hist[threadIdx.x] += t;
+            __syncthreads();
+        }
+        ctl->digit_base[pass * 256 + threadIdx.x] = hist[threadIdx.x] - v;
         __syncthreads();
     }
-    ctl->digit_base[blockIdx.x * 256 + threadIdx.x] = s[threadIdx.x] - v;
 }
 
 // ------------------------------------------------------------------ a4: re-order (T6)
@@ -109,7 +113,6 @@ cudaError_t launch_keys_sort_permute(Ctx *c)
     // few CTAs: every CTA ends with up to 2048 global atomics for its share of the digit histograms
     const int kgrid = (int)imin64((c->n + 255) / 256, (int64_t)c->num_sms * 2);
     keys_kernel<<<kgrid, 256, 0, st>>>(reinterpret_cast<const float4 *>(c->pos), n, ctl, key_orig);
-    digit_base_kernel<<<RS_PASSES, 256, 0, st>>>(ctl);
 
     u32 *status = wsptr<u32>(c, L.rs_status);
     const int sgrid = (int)imin64(L.rs_tiles, (int64_t)c->num_sms * 3);

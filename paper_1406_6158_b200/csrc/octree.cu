@@ -268,8 +268,8 @@ __global__ void __launch_bounds__(128) upsweep_kernel(NodeArrays na, const float
 {
     const u32 nn = ctl->nn;
     const float Lf = ctl->Lf;
-    u32 b = blockIdx.x * blockDim.x + threadIdx.x;
-    if (b >= nn || na.child[b] != NOCHILD) return;
+    for (u32 b = blockIdx.x * blockDim.x + threadIdx.x; b < nn; b += gridDim.x * blockDim.x) {
+    if (na.child[b] != NOCHILD) continue;
     u32 par = na.parent[b];            // requested now, needed after the leaf sums
     // ---- leaf: sequential sums over its particles, ascending (T9)
     {
@@ -350,6 +350,7 @@ __global__ void __launch_bounds__(128) upsweep_kernel(NodeArrays na, const float
         }
         par = gpar;
     }
+    }
 }
 
 // exact b_max^2 (Eq. 5; R9): every particle visits its ancestors, one level per iteration so that
@@ -410,8 +411,7 @@ __global__ void __launch_bounds__(256) gmark_kernel(const DevCtl *__restrict__ c
                                                     unsigned char *gflag, u32 *__restrict__ gnode_at)
 {
     const u32 nn = ctl->nn;
-    const u32 b = blockIdx.x * blockDim.x + threadIdx.x;
-    if (b >= nn) return;
+    for (u32 b = blockIdx.x * blockDim.x + threadIdx.x; b < nn; b += gridDim.x * blockDim.x) {
     const u32 c = count[b], f = first[b], gm = (u32)group_max;
     if (c > gm && child[b] == NOCHILD) {
         for (u32 s = f; s < f + c; s += gm) { gflag[s] = 1; gnode_at[s] = b; }     // level-21 leaf cut into chunks
@@ -430,6 +430,7 @@ __global__ void __launch_bounds__(256) gmark_kernel(const DevCtl *__restrict__ c
             if (!open || run + cq > gm) { gflag[first[q]] = 1; gnode_at[first[q]] = b; run = 0; open = true; }
             run += cq;
         }
+    }
     }
 }
 
@@ -622,7 +623,7 @@ cudaError_t launch_build_tree(Ctx *c)
     cudaEventRecord(c->ev_linked, st);
     cudaStreamWaitEvent(ax, c->ev_linked, 0);
     unsigned char *gflag = wsptr<unsigned char>(c, L.gflag);
-    gmark_kernel<<<(int)((L.node_cap + 255) / 256), 256, 0, ax>>>(ctl, first, count, child, nchild, parent,
+    gmark_kernel<<<(int)imin64((L.node_cap + 255) / 256, (int64_t)c->num_sms * 8), 256, 0, ax>>>(ctl, first, count, child, nchild, parent,
                                                                   c->group_max_now, c->grouping_now, gflag, wsptr<u32>(c, L.gnode_at));
     u32 *gfirst = wsptr<u32>(c, L.gfirst);
     gscan_kernel<<<sc_grid, SC_THREADS, 0, ax>>>(gflag, n, ctl, sc_status + L.po_tiles, gfirst, wsptr<u32>(c, L.gnode_at),
@@ -651,7 +652,8 @@ cudaError_t launch_build_tree(Ctx *c)
     na.rec = rec;
     na.MS64 = wsptr<double4>(c, L.MS64); na.C64 = wsptr<double>(c, L.C64);
     na.B2 = wsptr<double>(c, L.B2); na.leaf_of = wsptr<u32>(c, L.leaf_of);
-    const int full_node_grid = (int)((L.node_cap + 127) / 128);
+    // one thread per node; the node count is known on the device only: a bounded grid strides over the nodes
+    const int full_node_grid = (int)imin64((L.node_cap + 127) / 128, (int64_t)c->num_sms * 16);
     cudaStreamWaitEvent(st, c->ev_perm, 0);
     if (c->boxes_only) upsweep_kernel<false><<<full_node_grid, 128, 0, st>>>(na, pos_t, ctl, c->p.mac, c->p.theta);
     else upsweep_kernel<true><<<full_node_grid, 128, 0, st>>>(na, pos_t, ctl, c->p.mac, c->p.theta);
@@ -681,7 +683,7 @@ cudaError_t launch_regroup(Ctx *c)
     cudaMemsetAsync(c->ws + L.sc_status + sizeof(u64) * (size_t)L.po_tiles, 0, sizeof(u64) * (size_t)L.sc_tiles, st);
     cudaMemsetAsync(&ctl->tile_counter[9], 0, sizeof(u32), st);
     unsigned char *gflag = wsptr<unsigned char>(c, L.gflag);
-    gmark_kernel<<<(int)((L.node_cap + 255) / 256), 256, 0, st>>>(
+    gmark_kernel<<<(int)imin64((L.node_cap + 255) / 256, (int64_t)c->num_sms * 8), 256, 0, st>>>(
         ctl, wsptr<u32>(c, L.first), wsptr<u32>(c, L.count), wsptr<u32>(c, L.child), wsptr<unsigned char>(c, L.nchild),
         wsptr<u32>(c, L.parent), c->group_max_now, c->grouping_now, gflag, wsptr<u32>(c, L.gnode_at));
     const int sc_grid = (int)imin64(L.sc_tiles, (int64_t)c->num_sms * 8);
@@ -705,7 +707,7 @@ cudaError_t launch_refit_tree(Ctx *c)
     na.rec = wsptr<NodeRec>(c, L.nodes);
     na.MS64 = wsptr<double4>(c, L.MS64); na.C64 = wsptr<double>(c, L.C64);
     na.B2 = wsptr<double>(c, L.B2); na.leaf_of = wsptr<u32>(c, L.leaf_of);
-    upsweep_kernel<false><<<(int)((L.node_cap + 127) / 128), 128, 0, st>>>(na, reinterpret_cast<const float4 *>(c->pos), c->ctl,
+    upsweep_kernel<false><<<(int)imin64((L.node_cap + 127) / 128, (int64_t)c->num_sms * 16), 128, 0, st>>>(na, reinterpret_cast<const float4 *>(c->pos), c->ctl,
                                                                            c->p.mac, c->p.theta);
     ginfo_kernel<false><<<(int)imin64((c->n + 255) / 256, (int64_t)c->num_sms * 8), 256, 0, st>>>(
         c->ctl, (u32)c->n, reinterpret_cast<const float4 *>(c->pos), wsptr<u32>(c, L.gfirst), wsptr<u32>(c, L.gcount),

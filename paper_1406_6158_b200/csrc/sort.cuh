@@ -27,7 +27,7 @@ template <typename KeyT>
 __global__ void __launch_bounds__(RS_THREADS) radix_pass_kernel(
     const KeyT *__restrict__ kin, const u32 *__restrict__ vin, KeyT *__restrict__ kout, u32 *__restrict__ vout,
     u32 *__restrict__ inv_out, u32 n_host, const u32 *__restrict__ n_dev, int shift,
-    const u32 *__restrict__ digit_base, u32 *status, u32 tiles_alloc, u32 *tile_counter, u32 *dev_status)
+    const u32 *__restrict__ digit_base, u32 *status, u32 tiles_alloc, u32 *tile_counter, u32 *dev_status, int static_first)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     RadixSmem &sm = *reinterpret_cast<RadixSmem *>(smem_raw);
@@ -36,10 +36,16 @@ __global__ void __launch_bounds__(RS_THREADS) radix_pass_kernel(
     const u32 ntiles = (n + RS_TILE - 1) / RS_TILE;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const u32 lt_mask = (1u << lane) - 1u;
+    // Tile ids are normally drawn from a counter, so that a tile never waits (look-back) for a tile that has not
+    // started.  When every CTA of the grid is resident at once (static_first, set by the launcher: the grid is not
+    // larger than two CTAs per SM, which registers and shared memory allow) no tile can be left out, and the
+    // first tile of a CTA is simply its block index: the pass starts loading without the counter's round trip.
+    bool first = static_first != 0;
 
     for (;;) {
         __syncthreads();   // previous iteration's smem is dead
-        if (tid == 0) sm.tile = atomicAdd(tile_counter, 1u);
+        if (tid == 0) sm.tile = first ? blockIdx.x : (static_first ? gridDim.x : 0u) + atomicAdd(tile_counter, 1u);
+        first = false;
         for (int i = tid; i < (RS_THREADS / 32) * 256; i += RS_THREADS) (&sm.warp_cnt[0][0])[i] = 0;
         __syncthreads();
         const u32 tile = sm.tile;
@@ -208,8 +214,11 @@ static cudaError_t launch_radix_pass(const KeyT *kin, const u32 *vin, KeyT *kout
         if (e != cudaSuccess) return e;
         device_set_ready(&ready, device);
     }
+    int sms = 0;
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, device);
+    const int static_first = grid <= 2 * sms ? 1 : 0;
     return launch_pdl(radix_pass_kernel<KeyT>, dim3((unsigned)grid), dim3(RS_THREADS), sizeof(RadixSmem), st, kin, vin, kout, vout,
-                      inv_out, n_host, n_dev, shift, digit_base, status, tiles_alloc, tile_counter, dev_status);
+                      inv_out, n_host, n_dev, shift, digit_base, status, tiles_alloc, tile_counter, dev_status, static_first);
 }
 
 }  // namespace hyb
