@@ -136,7 +136,7 @@ static int do_build(Ctx *c, bool hard_only = false)
     c->acc_valid = false;
     // bbox (+ root cube), keys (+ digit bases), 8 sort passes, permute | preorder (+ level offsets), level sort,
     // link, upsweep, group mark / scan / info (+ b_max, r_b in absolute-MAC mode)
-    c->launches += 11 + 7 + (c->p.mac == HYB_MAC_ABS && !hard_only ? 2 : 0) - (had_bbox ? 1 : 0);
+    c->launches += 11 + 7 + (c->p.mac == HYB_MAC_ABS && !hard_only ? 3 : 0) - (had_bbox ? 1 : 0);
     return HYB_OK;
 }
 

@@ -255,7 +255,10 @@ __device__ __forceinline__ void finish_node(const NodeArrays &na, u32 b, int lev
     }
     na.rec[b].A = make_float4(__double2float_rn(Cx), __double2float_rn(Cy), __double2float_rn(Cz), __double2float_rn(M));
     na.rec[b].B = make_float4(lo.x, lo.y, lo.z, ropen2);
-    na.rec[b].C = make_float4(hi.x, hi.y, hi.z, 0.0f);
+    // C.w: the largest squared opening radius among the children (walk.cu: a cell farther away than this has only
+    // accepted children).  theta-mode: a child's cell side is half of this one's, so its r_open^2 is exactly a quarter;
+    // absolute MAC: filled in by ropen_abs_kernel once every node has its own radius
+    na.rec[b].C = make_float4(hi.x, hi.y, hi.z, mac == HYB_MAC_THETA ? __fmul_rn(ropen2, 0.25f) : INFINITY);
     na.MS64[b] = make_double4(M, Sx, Sy, Sz);
     na.C64[3 * (size_t)b] = Cx; na.C64[3 * (size_t)b + 1] = Cy; na.C64[3 * (size_t)b + 2] = Cz;
 }
@@ -401,6 +404,20 @@ __global__ void __launch_bounds__(256) ropen_abs_kernel(const DevCtl *__restrict
     double rb = __dadd_rn(__ddiv_rn(bm, 2.0), __dsqrt_rn(__dadd_rn(t5, t3)));
     float r = __double2float_rn(rb);
     rec[b].B.w = __fmul_rn(r, r);
+}
+
+// absolute MAC: NodeRec::C.w = largest squared opening radius among the children (see finish_node)
+__global__ void __launch_bounds__(256) cmax_kernel(const DevCtl *__restrict__ ctl, const u32 *__restrict__ child,
+                                                   const unsigned char *__restrict__ nchild, NodeRec *rec)
+{
+    const u32 nn = ctl->nn;
+    for (u32 b = blockIdx.x * blockDim.x + threadIdx.x; b < nn; b += gridDim.x * blockDim.x) {
+        const u32 c0 = child[b];
+        float m = 0.0f;
+        if (c0 != NOCHILD)
+            for (u32 q = c0; q < c0 + nchild[b]; q++) m = fmaxf(m, rec[q].B.w);
+        rec[b].C.w = m;
+    }
 }
 
 // ------------------------------------------------------------------ a7: groups (T11)
@@ -660,6 +677,7 @@ cudaError_t launch_build_tree(Ctx *c)
     if (c->p.mac == HYB_MAC_ABS && !c->boxes_only) {
         bmax_kernel<<<(n + 255) / 256, 256, 0, st>>>(pos_t, n, na.leaf_of, parent, level, na.C64, bmax2);
         ropen_abs_kernel<<<(int)((L.node_cap + 255) / 256), 256, 0, st>>>(ctl, bmax2, na.B2, c->p.a_err, rec);
+        cmax_kernel<<<(int)imin64((L.node_cap + 255) / 256, (int64_t)c->num_sms * 8), 256, 0, st>>>(ctl, child, nchild, rec);
     }
     cudaStreamWaitEvent(st, c->ev_groups, 0);       // join: groups, and (earlier on aux) the store copied back
     return cudaGetLastError();

@@ -49,11 +49,16 @@ struct SmemLayout {                 // per warp
     static constexpr int cell_cap = MODE == WALK_HARD ? 0 : WK_CELL_CAP;
     // the hard walk has no monopole buffer, so its K-weighted buffer can be larger (fewer flushes) at 3 CTAs per SM
     static constexpr int part_cap = MODE == WALK_NORMAL ? 0 : (MODE == WALK_HARD ? 256 : WK_PART_CAP);
-    static constexpr int stack_cap = 512;
+    static constexpr int stack_cap = MODE == WALK_HYBRID ? 320 : 512;
     static constexpr int lq_cap = 96;
+    static constexpr int nqueues = MODE == WALK_HYBRID ? 3 : 2;      // far leaves, near leaves, runs of accepted children
     static constexpr int cell_alloc = cell_cap ? cell_cap + WK_PAD_SLACK : 0;
     static constexpr int part_alloc = part_cap ? part_cap + WK_PAD_SLACK : 0;
-    static constexpr size_t bytes = 16 * (size_t)(cell_alloc + part_alloc) + 4 * (size_t)stack_cap + 8 * 2 * (size_t)lq_cap;
+    static constexpr size_t bytes = 16 * (size_t)(cell_alloc + part_alloc) + 4 * (size_t)stack_cap + 8 * (size_t)nqueues * (size_t)lq_cap;
+#ifndef WKV_UM
+#define WKV_UM 4
+#define WKV_UN 4
+#endif
 #ifndef WKV_HARD_WARPS
 #define WKV_HARD_WARPS 8
 #define WKV_HARD_CTAS 3
@@ -77,6 +82,11 @@ __global__ void __launch_bounds__(SmemLayout<MODE>::warps * 32, SmemLayout<MODE>
     constexpr bool HAS_MONO = MODE != WALK_HARD;      // monopole buffer (cells, far particles)
     constexpr bool HAS_NEAR = MODE != WALK_NORMAL;    // K-weighted buffer
     constexpr int C = MODE == WALK_HYBRID ? 6 : 3;    // accumulated components per sink
+    // An opened cell that is not within r_out and is at least as far from the group box as the largest opening
+    // radius of its children (NodeRec::C.w) has only accepted children: every child's centre of mass lies in the
+    // cell's tight box, so its T12 distances are not smaller than the cell's box distance.  Such a cell is not
+    // pushed; its children go to the monopole buffer as one run, without being tested (same lists, T13).
+    constexpr bool HAS_RUNS = MODE == WALK_HYBRID;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int oct = lane >> 3, sub = lane & 7;
@@ -86,6 +96,7 @@ __global__ void __launch_bounds__(SmemLayout<MODE>::warps * 32, SmemLayout<MODE>
     u32 *stack = reinterpret_cast<u32 *>(partbuf + SL::part_alloc);
     uint2 *lq0 = reinterpret_cast<uint2 *>(stack + SL::stack_cap);     // far leaves
     uint2 *lq1 = lq0 + SL::lq_cap;                                     // near leaves
+    uint2 *lq2 = lq1 + SL::lq_cap;                                     // cells whose children are all accepted (HAS_RUNS)
     float *red = reinterpret_cast<float *>(wbase);                     // reduction scratch (buffers are empty then)
 
     const u32 lt_mask = (1u << lane) - 1u;
@@ -138,7 +149,7 @@ __global__ void __launch_bounds__(SmemLayout<MODE>::warps * 32, SmemLayout<MODE>
         // sink_layout() (maximises the busy fraction n P / (32 S)); lane / A by a 15-bit reciprocal
         const ushort4 lay = c_layout[n];
         const int S = lay.x, A = lay.y, P = lay.z;
-        const int US = 4;                                             // sources per evaluation iteration (monopoles)
+        const int US = WKV_UM;                                             // sources per evaluation iteration (monopoles)
         const int copy = (lane * (int)lay.w) >> 15;                   // = lane / A  (lane < 32, A <= 32)
         const int aidx = lane - copy * A;
         const int part = copy < P ? copy : 0x40000000;               // idle lanes never enter the loops
@@ -159,7 +170,7 @@ __global__ void __launch_bounds__(SmemLayout<MODE>::warps * 32, SmemLayout<MODE>
 
         u32 ncell = 0, npart = 0, nhard = 0;
         int ncb = 0, npb = 0;             // buffer fills
-        int nlq0 = 0, nlq1 = 0;           // leaf queue fills
+        int nlq0 = 0, nlq1 = 0, nlq2 = 0; // leaf queue fills, cell-run queue fill
         int sp = 1;
         bool trav_done = false, flush_mono = false, flush_near = false, overflow = false;
         bool slow = false;                // something other than a plain traversal iteration is pending
@@ -177,18 +188,18 @@ __global__ void __launch_bounds__(SmemLayout<MODE>::warps * 32, SmemLayout<MODE>
                 if (HAS_MONO && flush_mono) {
                     const int cnt = pad_buffer(cellbuf, ncb, P * US, dummy, lane);
                     __syncwarp();
-                    if (S == 2) eval_mono<2, 4>(cellbuf, cnt, part, P, sk, eps2);
-                    else if (S == 3) eval_mono<3, 4>(cellbuf, cnt, part, P, sk, eps2);
-                    else eval_mono<4, 4>(cellbuf, cnt, part, P, sk, eps2);
+                    if (S == 2) eval_mono<2, WKV_UM>(cellbuf, cnt, part, P, sk, eps2);
+                    else if (S == 3) eval_mono<3, WKV_UM>(cellbuf, cnt, part, P, sk, eps2);
+                    else eval_mono<4, WKV_UM>(cellbuf, cnt, part, P, sk, eps2);
                     ncb = 0; flush_mono = false;
                     __syncwarp();
                 }
                 if (HAS_NEAR && flush_near) {
-                    const int cnt = pad_buffer(partbuf, npb, P * 4, dummy, lane);
+                    const int cnt = pad_buffer(partbuf, npb, P * WKV_UN, dummy, lane);
                     __syncwarp();
-                    if (S == 2) eval_near<2, 4, MODE == WALK_HYBRID, KF>(partbuf, cnt, part, P, sk, eps2, kc0, kc1);
-                    else if (S == 3) eval_near<3, 4, MODE == WALK_HYBRID, KF>(partbuf, cnt, part, P, sk, eps2, kc0, kc1);
-                    else eval_near<4, 4, MODE == WALK_HYBRID, KF>(partbuf, cnt, part, P, sk, eps2, kc0, kc1);
+                    if (S == 2) eval_near<2, WKV_UN, MODE == WALK_HYBRID, KF>(partbuf, cnt, part, P, sk, eps2, kc0, kc1);
+                    else if (S == 3) eval_near<3, WKV_UN, MODE == WALK_HYBRID, KF>(partbuf, cnt, part, P, sk, eps2, kc0, kc1);
+                    else eval_near<4, WKV_UN, MODE == WALK_HYBRID, KF>(partbuf, cnt, part, P, sk, eps2, kc0, kc1);
                     npb = 0; flush_near = false;
                     __syncwarp();
                 }
@@ -198,7 +209,7 @@ __global__ void __launch_bounds__(SmemLayout<MODE>::warps * 32, SmemLayout<MODE>
                 //      dense whatever the leaf sizes.  CUT: a particle of a near leaf goes to the K-weighted buffer only
                 //      if it is itself within r_out of the group box, else to the monopole buffer.
                 if (ex_done < ex_T) {
-                    const bool tonear = HAS_NEAR && (!HAS_MONO || ex_near);
+                    const bool tonear = HAS_NEAR && (!HAS_MONO || ex_near == 1);
                     const bool cutting = CUT && tonear;
                     if (tonear && npb + 64 > SL::part_cap) { flush_near = true; continue; }
                     if (HAS_MONO && (!tonear || cutting) && ncb + 64 > SL::cell_cap) { flush_mono = true; continue; }
@@ -244,6 +255,36 @@ __global__ void __launch_bounds__(SmemLayout<MODE>::warps * 32, SmemLayout<MODE>
                     }
                     ex_done += 64u;
                     continue;
+                }
+                // ---- runs of accepted children: eight runs per step, lane (oct, sub) copies child sub of runs oct and
+                //      oct + 4 (the centre-of-mass record only; nothing is tested)
+                if (HAS_RUNS && (nlq2 >= 32 || (trav_done && nlq2 > 0))) {
+                    __syncwarp();
+                    while (nlq2 > 0) {
+                        if (ncb + 64 > SL::cell_cap) { flush_mono = true; break; }
+                        const int m = min(8, nlq2);
+                        float4 p[2];
+                        bool hv[2];
+#pragma unroll
+                        for (int h = 0; h < 2; h++) {
+                            hv[h] = false;
+                            const int slot = oct + 4 * h;
+                            if (slot < m) {
+                                const uint2 r = lq2[nlq2 - 1 - slot];
+                                hv[h] = (u32)sub < r.y;
+                                if (hv[h]) p[h] = __ldg(&a.nodes[r.x + (u32)sub].A);
+                            }
+                        }
+                        nlq2 -= m;
+#pragma unroll
+                        for (int h = 0; h < 2; h++) {
+                            const u32 bal = __ballot_sync(FULL, hv[h]);
+                            if (hv[h]) cellbuf[ncb + __popc(bal & lt_mask)] = p[h];
+                            ncb += __popc(bal);
+                        }
+                    }
+                    __syncwarp();
+                    if (flush_mono) continue;
                 }
                 // ---- start an expansion when a leaf queue holds a full batch (or at the end)
                 {
@@ -296,10 +337,10 @@ __global__ void __launch_bounds__(SmemLayout<MODE>::warps * 32, SmemLayout<MODE>
             }
             sp -= npop;
             __syncwarp();
-            bool accept[2], accept_near[2], open_int[2], leaf_far[2], leaf_near[2];
+            bool accept[2], accept_near[2], open_int[2], leaf_far[2], leaf_near[2], cell_run[2];
 #pragma unroll
             for (int h = 0; h < 2; h++) {
-                accept[h] = accept_near[h] = open_int[h] = leaf_far[h] = leaf_near[h] = false;
+                accept[h] = accept_near[h] = open_int[h] = leaf_far[h] = leaf_near[h] = cell_run[h] = false;
                 if (have[h]) {
                     // T12: box-box distance (rule (b)), fp32, one rounding per operation
                     float fx = fmaxf(0.0f, fmaxf(__fsub_rn(nB[h].x, ghi.x), __fsub_rn(glo.x, nC[h].x)));
@@ -322,6 +363,10 @@ __global__ void __launch_bounds__(SmemLayout<MODE>::warps * 32, SmemLayout<MODE>
                     accept_near[h] = TREE && acc && near && MODE != WALK_NORMAL;
                     accept[h] = acc && !accept_near[h];
                     open_int[h] = open && !is_leaf;
+                    if (HAS_RUNS) {        // every child will be accepted: list them as one run instead of testing them
+                        cell_run[h] = open_int[h] && !near && d2b >= nC[h].w;
+                        open_int[h] = open_int[h] && !cell_run[h];
+                    }
                     leaf_near[h] = open && is_leaf && near && MODE != WALK_NORMAL;
                     leaf_far[h] = open && is_leaf && !leaf_near[h];
                 }
@@ -336,6 +381,19 @@ __global__ void __launch_bounds__(SmemLayout<MODE>::warps * 32, SmemLayout<MODE>
                 sp += npush;
             }
             if (overflow) break;
+            // cells with accepted children only -> queue of runs of node records (counted as cells now)
+            if (HAS_RUNS) {
+#pragma unroll
+                for (int h = 0; h < 2; h++) {
+                    const u32 bal = __ballot_sync(FULL, cell_run[h]);
+                    if (bal) {
+                        const u32 cnt = cell_run[h] ? mt[h].y : 0u;
+                        if (cell_run[h]) lq2[nlq2 + __popc(bal & lt_mask)] = make_uint2(mt[h].x, cnt);
+                        nlq2 += __popc(bal);
+                        ncell += __reduce_add_sync(FULL, cnt);
+                    }
+                }
+            }
             // accepted cells -> monopole buffer
             if (HAS_MONO) {
 #pragma unroll
@@ -385,7 +443,7 @@ __global__ void __launch_bounds__(SmemLayout<MODE>::warps * 32, SmemLayout<MODE>
             }
             __syncwarp();
             trav_done = sp == 0;
-            slow = trav_done || nlq0 >= 32 || nlq1 >= 32 || (HAS_MONO && ncb > SL::cell_cap - 64) ||
+            slow = trav_done || nlq0 >= 32 || nlq1 >= 32 || (HAS_RUNS && nlq2 >= 32) || (HAS_MONO && ncb > SL::cell_cap - 64) ||
                    (TREE && HAS_NEAR && npb > SL::part_cap - 64);
         }
         __syncwarp();
