@@ -68,18 +68,21 @@ __global__ void __launch_bounds__(256) keys_kernel(const float4 *__restrict__ po
     __syncthreads();
     if (!last) return;
     __threadfence();
-    for (int pass = 0; pass < RS_PASSES; pass++) {
-        const u32 v = ld_volatile_u32(&ctl->digit_hist[pass * 256 + threadIdx.x]);
-        hist[threadIdx.x] = v;
-        __syncthreads();
-        for (int off = 1; off < 256; off <<= 1) {
-            const u32 t = threadIdx.x >= off ? hist[threadIdx.x - off] : 0;
-            __syncthreads();
-            hist[threadIdx.x] += t;
-            __syncthreads();
+    {   // warp w scans the histogram of pass w: lane l takes bins 8 l .. 8 l + 7
+        static_assert(RS_PASSES == 8, "one warp of the 256-thread CTA per pass");
+        const int pass = threadIdx.x >> 5, lane = threadIdx.x & 31;
+        u32 v[8], sum = 0;
+#pragma unroll
+        for (int i = 0; i < 8; i++) { v[i] = ld_volatile_u32(&ctl->digit_hist[pass * 256 + 8 * lane + i]); sum += v[i]; }
+        u32 incl = sum;
+#pragma unroll
+        for (int off = 1; off < 32; off <<= 1) {
+            const u32 t = __shfl_up_sync(0xFFFFFFFFu, incl, off);
+            if (lane >= off) incl += t;
         }
-        ctl->digit_base[pass * 256 + threadIdx.x] = hist[threadIdx.x] - v;
-        __syncthreads();
+        u32 run = incl - sum;
+#pragma unroll
+        for (int i = 0; i < 8; i++) { ctl->digit_base[pass * 256 + 8 * lane + i] = run; run += v[i]; }
     }
 }
 
