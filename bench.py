@@ -329,7 +329,7 @@ def main():
                             "frac": gbs_build / hbm_peak, "radix_sort_share_of_bytes": build_bytes["radix_sort"] / bpp_build},
                   "integrate": {"bytes_per_particle_per_cycle": bpp_integrate, "achieved_gbs": gbs_int, "frac": gbs_int / hbm_peak},
                   "note": "N = 2^20 fits the 126 MB L2 and these stages are latency-bound (about 30 dependent kernels per "
-                          "build), so the achieved figure is far below the copy peak; see profiles/r01_profile.md"}
+                          "build), so the achieved figure is far below the copy peak; see profiles/r02_profile.md"}
 
     # ---- end to end through the C-ABI with HOST buffers (pinned), copies inside the timed region
     e2e = None

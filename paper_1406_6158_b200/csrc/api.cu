@@ -124,10 +124,8 @@ static int do_build(Ctx *c, bool hard_only = false)
     // group_max / 2 when only a hard walk follows
     c->grouping_now = c->p.grouping == HYB_GROUP_AUTO ? HYB_GROUP_SIBLINGS : c->p.grouping;
     c->group_max_now = c->p.group_max;
-    if (hard_only && c->p.grouping == HYB_GROUP_AUTO) {               // smaller runs: fewer listed particles beyond r_out
-        c->group_max_now = c->p.group_max / 2 > c->p.leaf_max ? c->p.group_max / 2 : c->p.leaf_max;
-        if (getenv("HYB_HARD_GM")) c->group_max_now = atoi(getenv("HYB_HARD_GM"));
-    }
+    if (hard_only && c->p.grouping == HYB_GROUP_AUTO)                 // smaller runs: fewer listed particles beyond r_out
+        c->group_max_now = c->p.group_max / 2 > c->p.leaf_max ? c->p.group_max / 2 : c->p.leaf_max;      // (cfg2: 16 / 24 / 40 / 48 / 64 are 4-25 % slower than 32)
     c->boxes_only = hard_only && !c->p.hard_tree;      // the tree-approximated hard walk needs the moments
     cudaError_t e = launch_build_tree(c);
     if (e != cudaSuccess) return cuda_fail(c, e, "build_tree");
@@ -240,8 +238,8 @@ int hyb_init(hyb_ctx **out, const hyb_params *params, int64_t n, hyb_float4 *d_p
     e = cudaMemsetAsync(c->ctl, 0, sizeof(DevCtl), c->stream);
     if (e == cudaSuccess) e = cudaMemsetAsync(c->ws + L.nhard, 0, 4 * (size_t)L.group_cap, c->stream);
     {
-        u32 t[4] = {8192u, 24576u, 65536u, (u32)imin64(4 * L.group_cap, 0xFFFFFFFFll)};
-        if (const char *sp = getenv("HYB_SPLIT")) sscanf(sp, "%u,%u,%u", &t[0], &t[1], &t[2]);
+        // hard walk scheduling (split_group): estimated pairs above which a group is queued in front / cut in 2 / cut in 4
+        const u32 t[4] = {8192u, 24576u, 65536u, (u32)imin64(4 * L.group_cap, 0xFFFFFFFFll)};
         if (e == cudaSuccess) e = cudaMemcpyAsync(&c->ctl->split_t[0], t, sizeof t, cudaMemcpyHostToDevice, c->stream);
     }
     if (e != cudaSuccess) { const int rc = cuda_fail(nullptr, e, "cudaMemsetAsync"); hyb_free(reinterpret_cast<hyb_ctx *>(c)); return rc; }

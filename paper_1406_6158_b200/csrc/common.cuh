@@ -39,12 +39,9 @@ constexpr int PO_TILE = SC_THREADS * PO_IPT;
 
 // walk kernel geometry
 constexpr int WK_WARPS = 8;              // warps per CTA
-#ifndef WKV_CELL
-#define WKV_CELL 320
-#define WKV_PART 192
-#endif
-constexpr int WK_CELL_CAP = WKV_CELL;         // monopole buffer entries per warp
-constexpr int WK_PART_CAP = WKV_PART;         // K-weighted (near) particle buffer entries per warp
+constexpr int WK_U = 4;                  // sources per iteration of the pair loops (pairs.cuh)
+constexpr int WK_CELL_CAP = 320;         // monopole buffer entries per warp
+constexpr int WK_PART_CAP = 192;         // K-weighted (near) particle buffer entries per warp
 
 enum WalkMode { WALK_HYBRID = 0, WALK_HARD = 1, WALK_NORMAL = 2 };
 

@@ -55,18 +55,10 @@ struct SmemLayout {                 // per warp
     static constexpr int cell_alloc = cell_cap ? cell_cap + WK_PAD_SLACK : 0;
     static constexpr int part_alloc = part_cap ? part_cap + WK_PAD_SLACK : 0;
     static constexpr size_t bytes = 16 * (size_t)(cell_alloc + part_alloc) + 4 * (size_t)stack_cap + 8 * (size_t)nqueues * (size_t)lq_cap;
-#ifndef WKV_UM
-#define WKV_UM 4
-#define WKV_UN 4
-#endif
-#ifndef WKV_HARD_WARPS
-#define WKV_HARD_WARPS 8
-#define WKV_HARD_CTAS 3
-#define WKV_SOFT_WARPS 8
-#define WKV_SOFT_CTAS 2
-#endif
-    static constexpr int ctas_per_sm = MODE == WALK_HARD ? WKV_HARD_CTAS : WKV_SOFT_CTAS;
-    static constexpr int warps = MODE == WALK_HARD ? WKV_HARD_WARPS : WKV_SOFT_WARPS;      // per CTA
+    // measured in round 2 (profiles/r02_profile.md): 2 x 8, 2 x 10, 3 x 7, 4 x 6 warps per SM make no difference to the hard
+    // walk; the fused walk needs its 128 registers (anything that caps them lower spills and loses 20 %)
+    static constexpr int ctas_per_sm = MODE == WALK_HARD ? 3 : 2;
+    static constexpr int warps = WK_WARPS;      // per CTA
 };
 
 // TREE (hyb_params.hard_tree): the paper-literal hard force.  The MAC is applied in the hard walk too and a
@@ -149,7 +141,7 @@ __global__ void __launch_bounds__(SmemLayout<MODE>::warps * 32, SmemLayout<MODE>
         // sink_layout() (maximises the busy fraction n P / (32 S)); lane / A by a 15-bit reciprocal
         const ushort4 lay = c_layout[n];
         const int S = lay.x, A = lay.y, P = lay.z;
-        const int US = WKV_UM;                                             // sources per evaluation iteration (monopoles)
+        const int US = WK_U;                                             // sources per evaluation iteration (monopoles)
         const int copy = (lane * (int)lay.w) >> 15;                   // = lane / A  (lane < 32, A <= 32)
         const int aidx = lane - copy * A;
         const int part = copy < P ? copy : 0x40000000;               // idle lanes never enter the loops
@@ -188,18 +180,18 @@ __global__ void __launch_bounds__(SmemLayout<MODE>::warps * 32, SmemLayout<MODE>
                 if (HAS_MONO && flush_mono) {
                     const int cnt = pad_buffer(cellbuf, ncb, P * US, dummy, lane);
                     __syncwarp();
-                    if (S == 2) eval_mono<2, WKV_UM>(cellbuf, cnt, part, P, sk, eps2);
-                    else if (S == 3) eval_mono<3, WKV_UM>(cellbuf, cnt, part, P, sk, eps2);
-                    else eval_mono<4, WKV_UM>(cellbuf, cnt, part, P, sk, eps2);
+                    if (S == 2) eval_mono<2, WK_U>(cellbuf, cnt, part, P, sk, eps2);
+                    else if (S == 3) eval_mono<3, WK_U>(cellbuf, cnt, part, P, sk, eps2);
+                    else eval_mono<4, WK_U>(cellbuf, cnt, part, P, sk, eps2);
                     ncb = 0; flush_mono = false;
                     __syncwarp();
                 }
                 if (HAS_NEAR && flush_near) {
-                    const int cnt = pad_buffer(partbuf, npb, P * WKV_UN, dummy, lane);
+                    const int cnt = pad_buffer(partbuf, npb, P * WK_U, dummy, lane);
                     __syncwarp();
-                    if (S == 2) eval_near<2, WKV_UN, MODE == WALK_HYBRID, KF>(partbuf, cnt, part, P, sk, eps2, kc0, kc1);
-                    else if (S == 3) eval_near<3, WKV_UN, MODE == WALK_HYBRID, KF>(partbuf, cnt, part, P, sk, eps2, kc0, kc1);
-                    else eval_near<4, WKV_UN, MODE == WALK_HYBRID, KF>(partbuf, cnt, part, P, sk, eps2, kc0, kc1);
+                    if (S == 2) eval_near<2, WK_U, MODE == WALK_HYBRID, KF>(partbuf, cnt, part, P, sk, eps2, kc0, kc1);
+                    else if (S == 3) eval_near<3, WK_U, MODE == WALK_HYBRID, KF>(partbuf, cnt, part, P, sk, eps2, kc0, kc1);
+                    else eval_near<4, WK_U, MODE == WALK_HYBRID, KF>(partbuf, cnt, part, P, sk, eps2, kc0, kc1);
                     npb = 0; flush_near = false;
                     __syncwarp();
                 }

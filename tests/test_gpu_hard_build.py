@@ -69,7 +69,6 @@ def test_cfg2_hard_build_full(hard_cut):
 def test_cfg4_hard_build_sampled():
     cfg = CONFIGS[4]
     pos, vel = make_ic(cfg.kind, cfg.n, cfg.seed)
-    t_ng = None
     h = make_hyb(cfg, pos, vel)
     h.build_tree_hard(); h.sync()
     t = O.Tree(pos, _hard_params(cfg))
