@@ -89,7 +89,8 @@ enum {
  * hyb_build_tree (Morton order). */
 enum {
     HYB_X_COUNTS = 0,      /* int64[8]: n, nn, ng, node_cap, status bits, nodes before clamping,
-                              kernels launched since hyb_init, 0                                */
+                              kernels launched since hyb_init, sink ranges the last walk was handed
+                              in front of the ordinary sequence (its work order, see hyb_soft_force) */
     HYB_X_KEYS_SORTED = 1, /* uint64[n]  63-bit Morton keys, ascending                          */
     HYB_X_PERM = 2,        /* uint32[n]  perm[j] = index, in the order the build found the
                               store in, of the particle now in slot j (stable sort)            */
@@ -179,7 +180,11 @@ int hyb_refit_tree(hyb_ctx *ctx);
 /* Step a8 (+a9 at a soft-step).  split = 1: one fused group walk that writes d_a_soft
  * (cells accepted by the MAC as monopoles, plus (1-K)-weighted neighbours, Eq. 9)
  * AND d_a_hard (K-weighted neighbours within r_out, Eq. 8).  split = 0: normal-tree walk,
- * d_a_soft = full acceleration, d_a_hard = 0.  Requires a tree.  Asynchronous. */
+ * d_a_soft = full acceleration, d_a_hard = 0.  Requires a tree.  Asynchronous.
+ * Work order: with fewer than about 160 particles per warp the GPU keeps resident (n < 3.8e5 on a B200) the
+ * longest sink groups decide how long the walk takes; they are then cut into sink ranges like those of
+ * hyb_hard_force, from the list lengths of the previous fused walk (none at the first one).  The same
+ * reproducibility statement holds. */
 int hyb_soft_force(hyb_ctx *ctx);
 
 /* Step a9 alone (a hard-step): neighbour search cut off at r_out
@@ -205,7 +210,8 @@ int hyb_step(hyb_ctx *ctx, int32_t n_soft_steps);
  * evaluate only the sink groups whose first particle lies in store slots [first, last) -- groups are never cut,
  * so the ranges of the replicas tile the groups when they tile [0, n) -- and write ZERO accelerations for all
  * other sinks, so that the element-wise sum over the replicas (one all-reduce, or an all-gather of the owned
- * ranges) is the full result, bit for bit.  hyb_step refuses a partial range: the caller runs the cycle with
+ * ranges) is the full result: every replica holds the same bits afterwards, and they are the bits of an unsharded
+ * evaluation wherever the same groups were cut into sink ranges (see hyb_hard_force; else equal to the last bits).  hyb_step refuses a partial range: the caller runs the cycle with
  * hyb_kick_drift / hyb_build_tree(_hard) / hyb_soft_force / hyb_hard_force and exchanges in between
  * (paper_1406_6158_b200/sharded.py).  Default [0, n).  Errors: INVALID_ARG. */
 int hyb_set_sink_range(hyb_ctx *ctx, int64_t first, int64_t last);
@@ -231,8 +237,9 @@ int hyb_export(hyb_ctx *ctx, int32_t what, void *host_dst, size_t bytes, size_t 
  * accelerations back.  acc_valid = 0: the accelerations of the incoming positions are evaluated first (one more
  * tree build and soft-step walk); acc_valid = 1: h_a_soft / h_a_hard are INPUTS too -- the accelerations this
  * call returned for exactly these positions the last time -- so a run whose state lives on the host advances
- * one call per cycle with nothing computed twice.  The device buffer (particles + workspace, the library's
- * only device allocation) and its stream are kept for the next call on the same device (freed by
+ * one call per cycle with nothing computed twice, and with the bits a device-resident context gives.  The device
+ * buffer (particles + workspace, the library's only device allocation), its stream and -- while n and the
+ * parameters stay the same -- the context are kept for the next call on the same device (freed by
  * hyb_run_host_release, or replaced when a larger n comes); concurrent calls are serialised.  Every pointer is
  * a HOST pointer to n elements; h_interactions (optional) receives uint64[4] as HYB_X_INTERACTIONS. */
 int hyb_run_host(const hyb_params *params, int64_t n, hyb_float4 *h_pos_m, hyb_float4 *h_vel,

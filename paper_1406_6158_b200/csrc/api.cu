@@ -54,6 +54,7 @@ Layout plan_workspace(int64_t n)
     L.gfirst = take(4 * GC); L.gcount = take(4 * GC); L.glo = take(16 * GC); L.ghi = take(16 * GC);
     L.ncell = take(4 * GC); L.npart = take(4 * GC); L.nhard = take(4 * GC);
     L.splitq = take(4 * 4 * GC);
+    L.scost = take(4 * GC);
     L.gnode = take(4 * GC); L.ganc = take(4 * GC);
     // scratch of hyb_energy and hyb_let_count (partial sums; domain boxes and counts)
     L.scratch_bytes = 8 * (N / 16 + 32768);
@@ -127,6 +128,7 @@ static int do_build(Ctx *c, bool hard_only = false)
     if (hard_only && c->p.grouping == HYB_GROUP_AUTO)                 // smaller runs: fewer listed particles beyond r_out
         c->group_max_now = c->p.group_max / 2 > c->p.leaf_max ? c->p.group_max / 2 : c->p.leaf_max;      // (cfg2: 16 / 24 / 40 / 48 / 64 are 4-25 % slower than 32)
     c->boxes_only = hard_only && !c->p.hard_tree;      // the tree-approximated hard walk needs the moments
+    c->next_kind = hard_only ? 1 : 2;                  // whose work order ginfo_kernel prepares
     cudaError_t e = launch_build_tree(c);
     if (e != cudaSuccess) return cuda_fail(c, e, "build_tree");
     c->tree_valid = true;
@@ -179,13 +181,20 @@ static int do_hard(Ctx *c)
 
 using namespace hyb;
 
-// device buffer and stream kept between hyb_run_host calls
-static struct { char *ptr; size_t bytes; int device; cudaStream_t st; } g_host = {nullptr, 0, -1, nullptr};
+// device buffer, stream and context kept between hyb_run_host calls
+static struct { char *ptr; size_t bytes; int device; cudaStream_t st; hyb_ctx *ctx; hyb_params p; int64_t n; } g_host =
+    {nullptr, 0, -1, nullptr, nullptr, {}, 0};
 static std::mutex g_host_mutex;
 static void release_host_cache()
 {
-    if (g_host.ptr) { cudaSetDevice(g_host.device); if (g_host.st) { cudaStreamSynchronize(g_host.st); cudaStreamDestroy(g_host.st); } cudaFree(g_host.ptr); }
-    g_host.ptr = nullptr; g_host.bytes = 0; g_host.device = -1; g_host.st = nullptr;
+    if (g_host.ptr) {
+        cudaSetDevice(g_host.device);
+        if (g_host.st) cudaStreamSynchronize(g_host.st);
+        if (g_host.ctx) hyb_free(g_host.ctx);
+        if (g_host.st) cudaStreamDestroy(g_host.st);
+        cudaFree(g_host.ptr);
+    }
+    g_host.ptr = nullptr; g_host.bytes = 0; g_host.device = -1; g_host.st = nullptr; g_host.ctx = nullptr; g_host.n = 0;
 }
 
 extern "C" {
@@ -235,11 +244,19 @@ int hyb_init(hyb_ctx **out, const hyb_params *params, int64_t n, hyb_float4 *d_p
         if (e != cudaSuccess) { const int rc = cuda_fail(nullptr, e, "cudaEventCreate"); hyb_free(reinterpret_cast<hyb_ctx *>(c)); return rc; }
     }
     c->timing = true;
+    // with fewer than a few sink groups per resident warp the longest groups set the duration of the fused walk: it
+    // then follows the work order of split_group (measured: cfg1 soft walk 0.60 -> 0.45 ms; from 2^20 particles up the
+    // Morton order is 1-2 % faster, its neighbours share cache lines)
+    c->soft_split = params->split && n < (int64_t)160 * c->num_sms * 2 * WK_WARPS;
     e = cudaMemsetAsync(c->ctl, 0, sizeof(DevCtl), c->stream);
     if (e == cudaSuccess) e = cudaMemsetAsync(c->ws + L.nhard, 0, 4 * (size_t)L.group_cap, c->stream);
+    if (e == cudaSuccess) e = cudaMemsetAsync(c->ws + L.scost, 0, 4 * (size_t)L.group_cap, c->stream);
     {
-        // hard walk scheduling (split_group): estimated pairs above which a group is queued in front / cut in 2 / cut in 4
-        const u32 t[4] = {8192u, 24576u, 65536u, (u32)imin64(4 * L.group_cap, 0xFFFFFFFFll)};
+        // walk scheduling (split_group).  Hard walk: estimated pairs above which a group is queued in front / cut in 2 /
+        // cut in 4.  Fused walk: the same three in 1/64 of the ideal makespan (all pairs / resident warps).
+        // (cfg1, soft walk: 0.60 ms in Morton order; 0.44-0.46 ms with 0-24 / 48 / 96; 0.50-0.52 with x / 64 / 128 or x / 32 / 64)
+        const u32 t[8] = {8192u, 24576u, 65536u, (u32)imin64(4 * L.group_cap, 0xFFFFFFFFll), 16u, 48u, 96u, (u32)c->num_sms * 2u * (u32)WK_WARPS};
+        static_assert(offsetof(DevCtl, soft_slots) - offsetof(DevCtl, split_t) == 7 * sizeof(u32), "split_t .. soft_slots are contiguous");
         if (e == cudaSuccess) e = cudaMemcpyAsync(&c->ctl->split_t[0], t, sizeof t, cudaMemcpyHostToDevice, c->stream);
     }
     if (e != cudaSuccess) { const int rc = cuda_fail(nullptr, e, "cudaMemsetAsync"); hyb_free(reinterpret_cast<hyb_ctx *>(c)); return rc; }
@@ -256,6 +273,8 @@ int hyb_set_params(hyb_ctx *ctx, const hyb_params *params)
     if (params->leaf_max != c->p.leaf_max || params->group_max != c->p.group_max || params->grouping != c->p.grouping)
         return fail(c, HYB_ERR_INVALID_ARG, "leaf_max / group_max / grouping cannot change after hyb_init");
     c->p = *params;
+    c->soft_split = params->split && c->n < (int64_t)160 * c->num_sms * 2 * WK_WARPS;
+    c->split_ready = false;
     c->tree_valid = false; c->acc_valid = false;
     return HYB_OK;
 }
@@ -445,7 +464,8 @@ int hyb_export(hyb_ctx *ctx, int32_t what, void *host_dst, size_t bytes, size_t 
     std::vector<char> tmp;
     switch (what) {
     case HYB_X_COUNTS: {
-        int64_t v[8] = {(int64_t)n, (int64_t)nn, (int64_t)ng, L.node_cap, (int64_t)h.status, (int64_t)h.nn_total, (int64_t)c->launches, 0};
+        int64_t v[8] = {(int64_t)n, (int64_t)nn, (int64_t)ng, L.node_cap, (int64_t)h.status, (int64_t)h.nn_total, (int64_t)c->launches,
+                        (int64_t)h.nheavy[c->walk_par ^ 1u]};
         if (bytes < sizeof v) return fail(c, HYB_ERR_INVALID_ARG, "buffer too small");
         memcpy(host_dst, v, sizeof v); if (written) *written = sizeof v; return HYB_OK; }
     case HYB_X_LEVEL_OFFSET:
@@ -545,7 +565,13 @@ int hyb_run_host(const hyb_params *params, int64_t n, hyb_float4 *h_pos_m, hyb_f
     char *d = g_host.ptr;
     cudaStream_t st = g_host.st;
     int rc = HYB_OK;
-    hyb_ctx *ctx = nullptr;
+    // the context is kept as well while n and the parameters stay the same: a run that advances call by call then
+    // keeps what a device-resident run keeps (the work order of the walks follows the list lengths of the previous
+    // ones, split_group), and gives the same bits
+    if (g_host.ctx && (g_host.n != n || memcmp(&g_host.p, params, sizeof(hyb_params)) != 0)) {
+        cudaStreamSynchronize(st);
+        hyb_free(g_host.ctx); g_host.ctx = nullptr;
+    }
     do {
         cudaMemcpyAsync(d + o_pos, h_pos_m, 16 * N, cudaMemcpyHostToDevice, st);
         cudaMemcpyAsync(d + o_vel, h_vel, 16 * N, cudaMemcpyHostToDevice, st);
@@ -554,12 +580,18 @@ int hyb_run_host(const hyb_params *params, int64_t n, hyb_float4 *h_pos_m, hyb_f
             cudaMemcpyAsync(d + o_as, h_a_soft, 16 * N, cudaMemcpyHostToDevice, st);
             cudaMemcpyAsync(d + o_ah, h_a_hard, 16 * N, cudaMemcpyHostToDevice, st);
         }
-        rc = hyb_init(&ctx, params, n, (hyb_float4 *)(d + o_pos), (hyb_float4 *)(d + o_vel), (hyb_float4 *)(d + o_as),
-                      (hyb_float4 *)(d + o_ah), (uint32_t *)(d + o_id), d + o_ws, ws_bytes, device, st);
-        if (rc != HYB_OK) break;
-        reinterpret_cast<Ctx *>(ctx)->timing = false;
-        reinterpret_cast<Ctx *>(ctx)->acc_valid = acc_valid != 0 && params->hard_refit == 0;
-        rc = hyb_step(ctx, n_soft_steps);
+        if (!g_host.ctx) {
+            rc = hyb_init(&g_host.ctx, params, n, (hyb_float4 *)(d + o_pos), (hyb_float4 *)(d + o_vel), (hyb_float4 *)(d + o_as),
+                          (hyb_float4 *)(d + o_ah), (uint32_t *)(d + o_id), d + o_ws, ws_bytes, device, st);
+            if (rc != HYB_OK) { g_host.ctx = nullptr; break; }
+            g_host.p = *params; g_host.n = n;
+        }
+        Ctx *c = reinterpret_cast<Ctx *>(g_host.ctx);
+        c->timing = false;
+        discard_pending_bbox(c);                              // new positions: nothing of the last call's tree applies
+        c->tree_valid = false; c->tree_refit = false;
+        c->acc_valid = acc_valid != 0 && params->hard_refit == 0;
+        rc = hyb_step(g_host.ctx, n_soft_steps);
         if (rc != HYB_OK) break;
         cudaMemcpyAsync(h_pos_m, d + o_pos, 16 * N, cudaMemcpyDeviceToHost, st);
         cudaMemcpyAsync(h_vel, d + o_vel, 16 * N, cudaMemcpyDeviceToHost, st);
@@ -567,14 +599,12 @@ int hyb_run_host(const hyb_params *params, int64_t n, hyb_float4 *h_pos_m, hyb_f
         cudaMemcpyAsync(h_a_hard, d + o_ah, 16 * N, cudaMemcpyDeviceToHost, st);
         cudaMemcpyAsync(h_id, d + o_id, 4 * N, cudaMemcpyDeviceToHost, st);
         if ((e = cudaStreamSynchronize(st)) != cudaSuccess) { rc = cuda_fail(nullptr, e, "copy back"); break; }
-        if (h_interactions) {
-            uint64_t v[4];
-            rc = hyb_export(ctx, HYB_X_INTERACTIONS, v, sizeof v, nullptr);
+        uint64_t v[4];                                        // (read every time: the counters run since the last read)
+        rc = hyb_export(g_host.ctx, HYB_X_INTERACTIONS, v, sizeof v, nullptr);
+        if (h_interactions)
             for (int i = 0; i < 4; i++) h_interactions[i] = v[i];
-        }
     } while (0);
-    if (ctx) hyb_free(ctx);
-    if (rc != HYB_OK) release_host_cache();
+    if (rc != HYB_OK) release_host_cache();      // (the message stays in the thread's hyb_last_error(NULL))
     return rc;
 }
 

@@ -61,14 +61,19 @@ struct DevCtl {
     // ---- walk ----
     // work distribution: launch k uses slot k & 1 and clears the other slot for launch k + 1 (no memset)
     u32 group_counter[2];
-    u32 nheavy[2];              // sink ranges of split groups (hard walk)
+    u32 nheavy[2];              // sink ranges of split groups (split_group)
     u32 walk_ng;                // number of groups of the last walk (is its nhard[] comparable?)
     u32 split_t[3];             // hard walk scheduling thresholds (pairs): queue first / cut in 2 / cut in 4 (set by hyb_init)
     u32 split_cap;              // entries the queue of sink ranges can hold
+    // fused (soft) walk scheduling: thresholds in 1/64 of the ideal makespan soft_work / soft_slots (hyb_init)
+    u32 soft_a[3];              // queue first / cut in 2 / cut in 4
+    u32 soft_slots;             // warps the fused walk keeps resident (hyb_init)
+    u32 soft_ng;                // number of groups of the last fused walk (is its scost[] comparable?)
+    u64 soft_work[2];           // sum over the groups of the last fused walk of members x cost (slot: WalkArgs::spar)
     u64 inter_soft, inter_hard, inter_hard_fused;   // pair counts: soft lists, hard lists (all walks), hard lists of fused walks
     u64 inter_hard_leaf;        // hard-only walks: members x particles of the leaves within r_out (the hard list without the particle cut)
     // ---- bounding box reduction: filled by bbox_kernel or by the drift, cleared again by keys_kernel ----
-    u32 bbox_enc[6];            // order-preserving encodings: ~min xyz, max xyz (atomicMax from 0 for both)
+    alignas(32) u32 bbox_enc[6]; // (one 32-byte sector with bbox_done) order-preserving encodings: ~min xyz, max xyz (atomicMax from 0 for both)
     u32 bbox_done;              // CTAs that have contributed (the last one derives the root cube)
     // ---- zero at the start of every build (keep last) ----
     u32 build_zero_begin;       // (marks the start of the memset range)
@@ -132,6 +137,7 @@ struct Layout {   // byte offsets into the workspace; computed by plan_workspace
     size_t gfirst, gcount, glo, ghi, ncell, npart, nhard;   // [group_cap]
     size_t gnode, ganc;         // u32[group_cap]: tree node a group hangs from; start node of its hard walk
     size_t splitq;              // u32[4 group_cap]: sink ranges of split groups, processed first (walk.cu)
+    size_t scost;               // u32[group_cap]: list length of the group at the last fused walk (ncell + npart + nhard)
     size_t scratch, scratch_bytes; // hyb_energy / hyb_let_count
     size_t zero_begin, zero_end; // look-back statuses and group flags: cleared by one memset per build
     size_t total;
@@ -147,6 +153,10 @@ Layout plan_workspace(int64_t n);
 struct Ctx {
     bool split_ready = false;   // ginfo_kernel has already queued the heavy groups for the walk that uses slot split_par
     u32 split_par = 0;
+    int split_kind = 0;         // ... and that walk is a hard-only walk (1) or a fused walk (2)
+    int next_kind = 2;          // the walk the build being enqueued is for
+    u32 soft_par = 0;           // slot of DevCtl::soft_work the next fused walk adds to
+    bool soft_split = false;    // the fused walk follows a prepared work order (few groups per resident warp; hyb_init)
     bool bbox_ready = false;    // the last drift has already reduced the bounding box of the current positions
     u32 walk_par = 0;           // slot of the walk work counters the next launch uses (DevCtl::group_counter)
     hyb_params p;
@@ -267,30 +277,52 @@ __device__ __forceinline__ void bbox_block_reduce(const float lo[3], const float
     }
 }
 
-// Hard walk scheduling: a group whose hard list was long at the previous walk (n x nhard of the group with the
-// same index -- an estimate that steers the order of work: the lists are the group's either way, only the
-// last bits of a sum can differ, because a range of fewer sinks combines its partial sums differently) is queued
+// Walk scheduling: a group whose list was long at the previous walk of the same kind (members x list length of the
+// group with the same index -- an estimate that steers the order of work: the lists are the group's either way, only
+// the last bits of a sum can differ, because a range of fewer sinks combines its partial sums differently) is queued
 // in front of everything else, the heaviest ones cut into 2 or 4 sink ranges; the walk skips it in the ordinary
-// sequence.
+// sequence.  kind 1: the hard-only walk, estimate from nhard[], fixed thresholds (DevCtl::split_t).  kind 2: the
+// fused walk, estimate from scost[], thresholds relative to the ideal makespan of the previous fused walk (all its
+// pairs / the warps that run side by side): with few groups per warp the longest group sets the duration of the
+// kernel, so it has to start first, and be shared by several warps when it alone is longer than the rest.
 // Called once per group by ginfo_kernel (during the build, off the critical path) or by split_kernel.
-__device__ __forceinline__ void split_group(DevCtl *ctl, u32 g, u32 n, u32 h_prev, bool comparable, u32 *__restrict__ heavy,
-                                            unsigned char *__restrict__ is_split, u32 par)
+struct SplitArgs {
+    DevCtl *ctl; const u32 *nhard_prev, *scost_prev; u32 *heavy; unsigned char *is_split;
+    u32 par, kind, soft_slot;
+};
+
+__device__ __forceinline__ void split_group(const SplitArgs &x, u32 g, u32 ng, u32 n)
 {
-    const unsigned long long est = (unsigned long long)n * (unsigned long long)(comparable ? h_prev : 0u);
+    DevCtl *ctl = x.ctl;
+    unsigned long long est, t0, t1, t2;
+    if (x.kind == 0u) { x.is_split[g] = 0; return; }
+    if (x.kind == 1u) {
+        const u32 prev = ctl->walk_ng;
+        const bool comparable = (prev > ng ? prev - ng : ng - prev) <= ng / 16u;
+        est = (unsigned long long)n * (unsigned long long)(comparable ? x.nhard_prev[g] : 0u);
+        t0 = ctl->split_t[0]; t1 = ctl->split_t[1]; t2 = ctl->split_t[2];
+    } else {
+        const u32 prev = ctl->soft_ng;
+        const bool comparable = (prev > ng ? prev - ng : ng - prev) <= ng / 16u;
+        est = (unsigned long long)n * (unsigned long long)(comparable ? x.scost_prev[g] : 0u);
+        const unsigned long long u = ctl->soft_work[x.soft_slot] / (64ull * (unsigned long long)ctl->soft_slots) + 1ull;
+        t0 = u * ctl->soft_a[0]; t1 = u * ctl->soft_a[1]; t2 = u * ctl->soft_a[2];
+    }
     u32 nsub = 0;                                   // 0: stays in the ordinary sequence
-    if (est >= ctl->split_t[2] && n >= 32u) nsub = 4;
-    else if (est >= ctl->split_t[1] && n >= 16u) nsub = 2;
-    else if (est >= ctl->split_t[0]) nsub = 1;      // whole, but queued in front
+    if (est >= t2 && n >= 32u) nsub = 4;
+    else if (est >= t1 && n >= 16u) nsub = 2;
+    else if (est >= t0) nsub = 1;                   // whole, but queued in front
+    if (est == 0ull) nsub = 0;
     if (nsub) {
-        const u32 at = atomicAdd(&ctl->nheavy[par], nsub);
+        const u32 at = atomicAdd(&ctl->nheavy[x.par], nsub);
         if (at + nsub <= ctl->split_cap) {
-            for (u32 i = 0; i < nsub; i++) heavy[at + i] = g | (i << 28) | ((nsub - 1u) << 30);
+            for (u32 i = 0; i < nsub; i++) x.heavy[at + i] = g | (i << 28) | ((nsub - 1u) << 30);
         } else {
-            atomicSub(&ctl->nheavy[par], nsub);     // the queue is full (it cannot be: 4 entries per group): leave the group where it is
+            atomicSub(&ctl->nheavy[x.par], nsub);   // the queue is full (it cannot be: 4 entries per group): leave the group where it is
             nsub = 0;
         }
     }
-    is_split[g] = nsub > 0;
+    x.is_split[g] = nsub > 0;
 }
 
 // Decoupled look-back over one value per tile (status word: bits 63..62 flag, low 62 bits value).

@@ -522,7 +522,7 @@ struct AncArgs {       // what ginfo_kernel<true> needs beyond the boxes (one th
     const u32 *gnode; const unsigned char *level; const u32 *parent;
     float r_out;
     u32 *ganc;
-    DevCtl *ctl_rw; const u32 *nhard_prev; u32 *heavy; unsigned char *is_split; u32 par;      // split_group (common.cuh)
+    SplitArgs sp;                                                                             // split_group (common.cuh)
 };
 
 __device__ __forceinline__ u32 node_anc(const DevCtl *__restrict__ ctl, const AncArgs &x, u32 node, const float3 lo, const float3 hi)
@@ -546,10 +546,7 @@ __device__ __forceinline__ u32 node_anc(const DevCtl *__restrict__ ctl, const An
 __device__ __forceinline__ void group_anc(const DevCtl *__restrict__ ctl, const AncArgs &x, u32 g, u32 ng, u32 count,
                                           const float3 lo, const float3 hi)
 {
-    {   // work order of the next hard walk (the group flags of the build are free again by now)
-        const u32 prev = ctl->walk_ng;
-        split_group(x.ctl_rw, g, count, x.nhard_prev[g], (prev > ng ? prev - ng : ng - prev) <= ng / 16u, x.heavy, x.is_split, x.par);
-    }
+    split_group(x.sp, g, ng, count);      // work order of the next walk (the group flags of the build are free again by now)
     x.ganc[g] = node_anc(ctl, x, x.gnode[g], lo, hi);
 }
 
@@ -603,7 +600,7 @@ cudaError_t launch_build_tree(Ctx *c)
     // one memset: the build block of the control words, the look-back statuses and the group flags
     char *zb = reinterpret_cast<char *>(ctl) + offsetof(DevCtl, build_zero_begin);
     cudaMemsetAsync(zb, 0, (size_t)((c->ws + L.zero_end) - zb), st);
-    // the queue of sink ranges this build fills for the next hard walk (ginfo_kernel): a build that no walk
+    // the queue of sink ranges this build fills for the next walk (ginfo_kernel): a build that no walk
     // consumed (two builds in a row) must not leave its entries behind
     if (c->p.split) cudaMemsetAsync(&ctl->nheavy[c->walk_par], 0, sizeof(u32), st);
 
@@ -646,17 +643,18 @@ cudaError_t launch_build_tree(Ctx *c)
     gscan_kernel<<<sc_grid, SC_THREADS, 0, ax>>>(gflag, n, ctl, sc_status + L.po_tiles, gfirst, wsptr<u32>(c, L.gnode_at),
                                                  wsptr<u32>(c, L.gnode));
     // group boxes; with the force split also the start node of each group's hard walk and the work order of
-    // the next hard walk (split_group), for the counter slot that walk will use
+    // the next walk (split_group), for the counter slot that walk will use
     const int gi_grid = (int)imin64((c->n + 255) / 256, (int64_t)c->num_sms * 8);
     AncArgs anc = {};
     c->split_ready = false;
     if (c->p.split) {
         anc.gnode = wsptr<u32>(c, L.gnode); anc.level = level; anc.parent = parent; anc.r_out = c->p.r_out;
-        anc.ganc = wsptr<u32>(c, L.ganc); anc.ctl_rw = ctl; anc.nhard_prev = wsptr<u32>(c, L.nhard);
-        anc.heavy = wsptr<u32>(c, L.splitq); anc.is_split = gflag; anc.par = c->walk_par;
+        anc.ganc = wsptr<u32>(c, L.ganc);
+        anc.sp = SplitArgs{ctl, wsptr<u32>(c, L.nhard), wsptr<u32>(c, L.scost), wsptr<u32>(c, L.splitq), gflag,
+                           c->walk_par, (u32)(c->next_kind == 2 && !c->soft_split ? 0 : c->next_kind), c->soft_par ^ 1u};
         ginfo_kernel<true><<<gi_grid, 256, 0, ax>>>(ctl, n, pos_t, gfirst, wsptr<u32>(c, L.gcount), wsptr<float4>(c, L.glo),
                                                     wsptr<float4>(c, L.ghi), anc);
-        c->split_ready = true; c->split_par = c->walk_par;
+        c->split_ready = true; c->split_par = c->walk_par; c->split_kind = c->next_kind;
     } else {
         ginfo_kernel<false><<<gi_grid, 256, 0, ax>>>(ctl, n, pos_t, gfirst, wsptr<u32>(c, L.gcount), wsptr<float4>(c, L.glo),
                                                      wsptr<float4>(c, L.ghi), anc);

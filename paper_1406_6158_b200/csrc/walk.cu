@@ -30,10 +30,12 @@ struct WalkArgs {
     const u32 *gfirst, *gcount;
     const float4 *glo, *ghi;
     u32 *ncell, *npart, *nhard;
-    const u32 *heavy;             // hard walk: sink ranges of split groups (see split_kernel)
+    u32 *scost;                   // fused walk: list length per group, the estimate of the next fused walk's work order
+    const u32 *heavy;             // sink ranges of split groups (split_group, common.cuh)
     u32 par;                      // which slot of DevCtl::group_counter / nheavy this launch uses
+    u32 spar;                     // fused walk: which slot of DevCtl::soft_work it adds to
     const u32 *ganc;              // hard walk: start node of every group (octree.cu, group_anc)
-    const unsigned char *is_split; // hard walk: group is handled as ranges
+    const unsigned char *is_split; // group is handled as ranges
     float4 *a_soft, *a_hard;
     DevCtl *ctl;
     u32 sink_lo, sink_hi;            // only groups whose first sink lies in [sink_lo, sink_hi) are evaluated
@@ -67,7 +69,9 @@ struct SmemLayout {                 // per warp
 // r_out is opened, i.e. the hard force is the direct K-weighted sum (R20).
 // CUT (hyb_params.hard_cut, R30): the hard list holds only the particles that are themselves within
 // r_out of the group box; the other particles of a near leaf are plain Eq. 2 pairs (monopole buffer).
-template <int MODE, int KF, bool TREE, bool CUT>
+// SPLIT: the work order prepared by split_group is followed (always in the hard-only walk; in the fused walk when
+// the particle number is small, Ctx::soft_split).
+template <int MODE, int KF, bool TREE, bool CUT, bool SPLIT>
 __global__ void __launch_bounds__(SmemLayout<MODE>::warps * 32, SmemLayout<MODE>::ctas_per_sm) walk_kernel(const WalkArgs a)
 {
     using SL = SmemLayout<MODE>;
@@ -94,19 +98,19 @@ __global__ void __launch_bounds__(SmemLayout<MODE>::warps * 32, SmemLayout<MODE>
     const u32 lt_mask = (1u << lane) - 1u;
     const u32 ng = a.ctl->ng;
     if (blockIdx.x == 0 && threadIdx.x == 0) {
-        a.ctl->walk_ng = ng;                                            // read by the next split_kernel
+        if (MODE == WALK_HARD) a.ctl->walk_ng = ng;                     // read by the next split_group
+        else { a.ctl->soft_ng = ng; a.ctl->soft_work[a.spar ^ 1u] = 0ull; }
         a.ctl->group_counter[a.par ^ 1u] = 0u; a.ctl->nheavy[a.par ^ 1u] = 0u;      // the next launch's slots
     }
     const float rout2 = __fmul_rn(a.rout, a.rout);
     const float eps2 = a.eps2, kc0 = a.kc0, kc1 = a.kc1;
     unsigned long long isoft = 0, ihard = 0, ileaf = 0;
 
-    // Work items come from one atomic counter.  In the hard walk the heaviest sink groups (by the
-    // estimate of split_kernel) have been cut into 2 or 4 sink ranges that are handed out first, so
+    // Work items come from one atomic counter.  The heaviest sink groups (by the estimate of split_group)
+    // have been queued, some cut into 2 or 4 sink ranges, and are handed out first, so
     // that the longest items start early and run side by side; then the other groups in Morton order.
     // Every range walks with the box of the WHOLE group, so its lists are the group's lists (T12-T13);
     // only the sinks differ.
-    constexpr bool SPLIT = MODE == WALK_HARD;
     const u32 nheavy = SPLIT ? a.ctl->nheavy[a.par] : 0u;
     const u32 nitems = ng + nheavy;
     u32 item = 0;
@@ -497,7 +501,10 @@ __global__ void __launch_bounds__(SmemLayout<MODE>::warps * 32, SmemLayout<MODE>
             }
         }
         if (lane == 0) {
-            if (rsub == 0) { a.ncell[g] = ncell; a.npart[g] = npart; a.nhard[g] = nhard; }
+            if (rsub == 0) {
+                a.ncell[g] = ncell; a.npart[g] = npart; a.nhard[g] = nhard;
+                if (MODE != WALK_HARD) a.scost[g] = ncell + npart + nhard;
+            }
             if (MODE != WALK_HARD) isoft += (unsigned long long)n * (unsigned long long)(ncell + npart);
             if (MODE != WALK_NORMAL) ihard += (unsigned long long)n * (unsigned long long)nhard;
             if (MODE == WALK_HARD) ileaf += (unsigned long long)n * (unsigned long long)npart;
@@ -509,20 +516,17 @@ __global__ void __launch_bounds__(SmemLayout<MODE>::warps * 32, SmemLayout<MODE>
         if (ihard) atomicAdd(&a.ctl->inter_hard, ihard);
         if (ihard && MODE == WALK_HYBRID) atomicAdd(&a.ctl->inter_hard_fused, ihard);
         if (ileaf) atomicAdd(&a.ctl->inter_hard_leaf, ileaf);
+        if (MODE != WALK_HARD && isoft + ihard) atomicAdd(&a.ctl->soft_work[a.spar], isoft + ihard);
     }
 }
 
-// Hard walk scheduling (split_group, common.cuh) for a walk whose tree build has not done it: a second
-// hyb_hard_force on the same tree, or a refitted tree.
-__global__ void __launch_bounds__(256) split_kernel(DevCtl *ctl, const u32 *__restrict__ gcount,
-                                                    const u32 *__restrict__ nhard, u32 *__restrict__ heavy,
-                                                    unsigned char *__restrict__ is_split, u32 par)
+// Walk scheduling (split_group, common.cuh) for a walk whose tree build has not done it: a second
+// force call on the same tree, a refitted tree, or a build that expected the other kind of walk.
+__global__ void __launch_bounds__(256) split_kernel(const SplitArgs x, const u32 *__restrict__ gcount)
 {
-    const u32 ng = ctl->ng, prev = ctl->walk_ng;
-    // the estimate is only meaningful when the previous walk had about the same groups
-    const bool comparable = (prev > ng ? prev - ng : ng - prev) <= ng / 16u;
+    const u32 ng = x.ctl->ng;
     for (u32 g = blockIdx.x * blockDim.x + threadIdx.x; g < ng; g += gridDim.x * blockDim.x)
-        split_group(ctl, g, gcount[g], nhard[g], comparable, heavy, is_split, par);
+        split_group(x, g, ng, gcount[g]);
 }
 
 __global__ void zero_acc_kernel(float4 *a, u32 n)
@@ -538,7 +542,7 @@ cudaError_t launch_zero_acc(Ctx *c, hyb_float4 *a)
     return cudaGetLastError();
 }
 
-template <int MODE, int KF, bool TREE, bool CUT>
+template <int MODE, int KF, bool TREE, bool CUT, bool SPLIT>
 static cudaError_t launch_walk_mode(Ctx *c, const WalkArgs &a)
 {
     using SL = SmemLayout<MODE>;
@@ -549,11 +553,11 @@ static cudaError_t launch_walk_mode(Ctx *c, const WalkArgs &a)
         sink_layout(t);
         cudaError_t e = cudaMemcpyToSymbol(c_layout, t, sizeof t);
         if (e != cudaSuccess) return e;
-        e = cudaFuncSetAttribute(walk_kernel<MODE, KF, TREE, CUT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        e = cudaFuncSetAttribute(walk_kernel<MODE, KF, TREE, CUT, SPLIT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
         device_set_ready(&ready, c->device);
     }
-    walk_kernel<MODE, KF, TREE, CUT><<<c->num_sms * SL::ctas_per_sm, SL::warps * 32, smem, c->stream>>>(a);
+    walk_kernel<MODE, KF, TREE, CUT, SPLIT><<<c->num_sms * SL::ctas_per_sm, SL::warps * 32, smem, c->stream>>>(a);
     return cudaGetLastError();
 }
 
@@ -581,25 +585,31 @@ cudaError_t launch_walk(Ctx *c, int mode)
     a.ganc = c->tree_refit ? nullptr : wsptr<u32>(c, L.ganc);      // refitted boxes: the Morton cells are stale
     a.is_split = wsptr<unsigned char>(c, L.gflag);      // the build's flag array is free between builds
     a.par = c->walk_par; c->walk_par ^= 1u;      // both slots start at zero (hyb_init); each walk clears the other one
-    if (mode == WALK_HARD && !(c->split_ready && c->split_par == a.par)) {
+    a.scost = wsptr<u32>(c, L.scost);
+    a.spar = c->soft_par;
+    const int kind = mode == WALK_HARD ? 1 : 2;
+    const bool sched = mode == WALK_HARD || (mode == WALK_HYBRID && c->soft_split);
+    if (sched && !(c->split_ready && c->split_par == a.par && c->split_kind == kind)) {
+        if (c->split_ready && c->split_par == a.par)       // the build queued the groups for the other kind of walk
+            cudaMemsetAsync(&c->ctl->nheavy[a.par], 0, sizeof(u32), c->stream);
         split_kernel<<<(int)imin64((c->n + 255) / 256, (int64_t)c->num_sms * 4), 256, 0, c->stream>>>(
-            c->ctl, a.gcount, a.nhard, wsptr<u32>(c, L.splitq), wsptr<unsigned char>(c, L.gflag), a.par);
+            SplitArgs{c->ctl, a.nhard, a.scost, wsptr<u32>(c, L.splitq), wsptr<unsigned char>(c, L.gflag), a.par, (u32)kind,
+                      c->soft_par ^ 1u}, a.gcount);
         c->launches += 1;
     }
+    if (mode != WALK_HARD) c->soft_par ^= 1u;
     c->split_ready = false;
     const bool poly7 = c->p.kfunc == HYB_K_POLY7, tree = c->p.hard_tree != 0, cut = c->p.hard_cut != 0;
-    if (mode == WALK_NORMAL) return launch_walk_mode<WALK_NORMAL, HYB_K_PAPER, false, false>(c, a);
-#define HYB_WALK_CASE(M, K, T, C) if (poly7 == (K == HYB_K_POLY7) && tree == T && cut == C) return launch_walk_mode<M, K, T, C>(c, a)
-    if (mode == WALK_HYBRID) {
-        HYB_WALK_CASE(WALK_HYBRID, HYB_K_PAPER, false, false); HYB_WALK_CASE(WALK_HYBRID, HYB_K_PAPER, false, true);
-        HYB_WALK_CASE(WALK_HYBRID, HYB_K_PAPER, true, false); HYB_WALK_CASE(WALK_HYBRID, HYB_K_PAPER, true, true);
-        HYB_WALK_CASE(WALK_HYBRID, HYB_K_POLY7, false, false); HYB_WALK_CASE(WALK_HYBRID, HYB_K_POLY7, false, true);
-        HYB_WALK_CASE(WALK_HYBRID, HYB_K_POLY7, true, false); HYB_WALK_CASE(WALK_HYBRID, HYB_K_POLY7, true, true);
-    }
-    HYB_WALK_CASE(WALK_HARD, HYB_K_PAPER, false, false); HYB_WALK_CASE(WALK_HARD, HYB_K_PAPER, false, true);
-    HYB_WALK_CASE(WALK_HARD, HYB_K_PAPER, true, false); HYB_WALK_CASE(WALK_HARD, HYB_K_PAPER, true, true);
-    HYB_WALK_CASE(WALK_HARD, HYB_K_POLY7, false, false); HYB_WALK_CASE(WALK_HARD, HYB_K_POLY7, false, true);
-    HYB_WALK_CASE(WALK_HARD, HYB_K_POLY7, true, false); HYB_WALK_CASE(WALK_HARD, HYB_K_POLY7, true, true);
+    if (mode == WALK_NORMAL) return launch_walk_mode<WALK_NORMAL, HYB_K_PAPER, false, false, false>(c, a);
+#define HYB_WALK_CASE(M, K, T, C, S) if (poly7 == (K == HYB_K_POLY7) && tree == T && cut == C && sched == S) return launch_walk_mode<M, K, T, C, S>(c, a)
+#define HYB_WALK_CASES(M, S) \
+    HYB_WALK_CASE(M, HYB_K_PAPER, false, false, S); HYB_WALK_CASE(M, HYB_K_PAPER, false, true, S); \
+    HYB_WALK_CASE(M, HYB_K_PAPER, true, false, S); HYB_WALK_CASE(M, HYB_K_PAPER, true, true, S); \
+    HYB_WALK_CASE(M, HYB_K_POLY7, false, false, S); HYB_WALK_CASE(M, HYB_K_POLY7, false, true, S); \
+    HYB_WALK_CASE(M, HYB_K_POLY7, true, false, S); HYB_WALK_CASE(M, HYB_K_POLY7, true, true, S)
+    if (mode == WALK_HYBRID) { HYB_WALK_CASES(WALK_HYBRID, false); HYB_WALK_CASES(WALK_HYBRID, true); }
+    HYB_WALK_CASES(WALK_HARD, true);
+#undef HYB_WALK_CASES
 #undef HYB_WALK_CASE
     return cudaErrorInvalidValue;
 }

@@ -58,6 +58,10 @@ def test_random_configuration(seed):
         a_s, a_h, _ = th.forces(O.MODE_HYBRID)
         rms, mx = acc_errors(h.a_hard.cpu().numpy()[:, :3], a_h, a_s + a_h)
         assert rms < RMS_TOL and mx < MAX_TOL, (rms, mx)
+    store = h.pos_m.cpu().numpy()                          # once more on the same store: this fused walk follows the work
+    h.build_tree(); h.sync()                               # order prepared from the first one's list lengths
+    h.export("interactions")                               # (the counters run since the last read)
+    check_forces(h, O.Tree(store, O.params_from(cfg)), split=cfg.split == 1)
     h.step(1); h.sync()
     assert np.all(np.isfinite(h.pos_m.cpu().numpy()))
     h.close()
