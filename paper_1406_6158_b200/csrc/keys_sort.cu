@@ -39,8 +39,9 @@ __device__ __forceinline__ u32 quantise(float x, double o, double inv)
     return f >= 2097151.0 ? 2097151u : (f > 0.0 ? (u32)f : 0u);
 }
 
+constexpr int KEYS_THREADS = 1024;      // few CTAs (each ends with up to 2048 global atomics), many warps (the loop is a chain of latencies)
 // also accumulates the eight 8-bit digit histograms the onesweep sort needs; its last CTA turns them into bases
-__global__ void __launch_bounds__(256) keys_kernel(const float4 *__restrict__ pos, u32 n, DevCtl *ctl,
+__global__ void __launch_bounds__(KEYS_THREADS) keys_kernel(const float4 *__restrict__ pos, u32 n, DevCtl *ctl,
                                                    u64 *__restrict__ key)
 {
     __shared__ u32 hist[RS_PASSES * 256];
@@ -66,10 +67,10 @@ __global__ void __launch_bounds__(256) keys_kernel(const float4 *__restrict__ po
     __syncthreads();
     if (threadIdx.x == 0) last = atomicAdd(&ctl->tile_counter[13], 1u) == gridDim.x - 1;
     __syncthreads();
-    if (!last) return;
+    if (!last || threadIdx.x >= 256) return;
     __threadfence();
     {   // warp w scans the histogram of pass w: lane l takes bins 8 l .. 8 l + 7
-        static_assert(RS_PASSES == 8, "one warp of the 256-thread CTA per pass");
+        static_assert(RS_PASSES == 8 && KEYS_THREADS >= 256, "one warp of the CTA's first eight per pass");
         const int pass = threadIdx.x >> 5, lane = threadIdx.x & 31;
         u32 v[8], sum = 0;
 #pragma unroll
@@ -114,8 +115,8 @@ cudaError_t launch_keys_sort_permute(Ctx *c)
     u64 *key_orig = wsptr<u64>(c, L.key_orig), *key_a = wsptr<u64>(c, L.key_a), *key_b = wsptr<u64>(c, L.key_b);
     u32 *val_a = wsptr<u32>(c, L.val_a), *val_b = wsptr<u32>(c, L.val_b);
     // few CTAs: every CTA ends with up to 2048 global atomics for its share of the digit histograms
-    const int kgrid = (int)imin64((c->n + 255) / 256, (int64_t)c->num_sms * 2);
-    keys_kernel<<<kgrid, 256, 0, st>>>(reinterpret_cast<const float4 *>(c->pos), n, ctl, key_orig);
+    const int kgrid = (int)imin64((c->n + KEYS_THREADS - 1) / KEYS_THREADS, (int64_t)c->num_sms * 2);
+    keys_kernel<<<kgrid, KEYS_THREADS, 0, st>>>(reinterpret_cast<const float4 *>(c->pos), n, ctl, key_orig);
 
     u32 *status = wsptr<u32>(c, L.rs_status);
     const int sgrid = (int)imin64(L.rs_tiles, (int64_t)c->num_sms * 3);
