@@ -271,7 +271,9 @@ __global__ void __launch_bounds__(128) upsweep_kernel(NodeArrays na, const float
 {
     const u32 nn = ctl->nn;
     const float Lf = ctl->Lf;
-    for (u32 b = blockIdx.x * blockDim.x + threadIdx.x; b < nn; b += gridDim.x * blockDim.x) {
+    // deepest leaves first (breadth-first numbering: the highest indices): their climbs are the longest chains
+    for (u32 idx = blockIdx.x * blockDim.x + threadIdx.x; idx < nn; idx += gridDim.x * blockDim.x) {
+    const u32 b = nn - 1u - idx;
     if (na.child[b] != NOCHILD) continue;
     u32 par = na.parent[b];            // requested now, needed after the leaf sums
     // ---- leaf: sequential sums over its particles, ascending (T9)
