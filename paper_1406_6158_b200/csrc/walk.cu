@@ -314,11 +314,14 @@ __global__ void __launch_bounds__(SmemLayout<MODE>::warps * 32, SmemLayout<MODE>
             // ---- traversal iteration: pop up to eight descriptors, lane (oct, sub) tests child sub of
             //      descriptors oct and oct + 4
             const int npop = min(8, sp);
+            // hard walk: its first iterations below the start node pop four descriptors or fewer, and then no lane has a
+            // second node to test (uniform branch; the other walks are wide almost always and keep the straight code)
+            const bool wide = MODE != WALK_HARD || npop > 4;
             bool have[2];
             float4 nA[2], nB[2], nC[2];
             uint2 mt[2];
 #pragma unroll
-            for (int h = 0; h < 2; h++) {
+            for (int h = 0; h < 2; h++) if (h == 0 || wide) {
                 have[h] = false;
                 const int slot = oct + 4 * h;
                 if (slot < npop) {
@@ -335,7 +338,7 @@ __global__ void __launch_bounds__(SmemLayout<MODE>::warps * 32, SmemLayout<MODE>
             __syncwarp();
             bool accept[2], accept_near[2], open_int[2], leaf_far[2], leaf_near[2], cell_run[2];
 #pragma unroll
-            for (int h = 0; h < 2; h++) {
+            for (int h = 0; h < 2; h++) if (h == 0 || wide) {
                 accept[h] = accept_near[h] = open_int[h] = leaf_far[h] = leaf_near[h] = cell_run[h] = false;
                 if (have[h]) {
                     // T12: box-box distance (rule (b)), fp32, one rounding per operation
@@ -369,7 +372,7 @@ __global__ void __launch_bounds__(SmemLayout<MODE>::warps * 32, SmemLayout<MODE>
             }
             // opened cells: push one descriptor each
 #pragma unroll
-            for (int h = 0; h < 2; h++) {
+            for (int h = 0; h < 2; h++) if (h == 0 || wide) {
                 const u32 bal = __ballot_sync(FULL, open_int[h]);
                 const int npush = __popc(bal);
                 if (sp + npush > SL::stack_cap) { overflow = true; break; }
@@ -380,7 +383,7 @@ __global__ void __launch_bounds__(SmemLayout<MODE>::warps * 32, SmemLayout<MODE>
             // cells with accepted children only -> queue of runs of node records (counted as cells now)
             if (HAS_RUNS) {
 #pragma unroll
-                for (int h = 0; h < 2; h++) {
+                for (int h = 0; h < 2; h++) if (h == 0 || wide) {
                     const u32 bal = __ballot_sync(FULL, cell_run[h]);
                     if (bal) {
                         const u32 cnt = cell_run[h] ? mt[h].y : 0u;
@@ -393,7 +396,7 @@ __global__ void __launch_bounds__(SmemLayout<MODE>::warps * 32, SmemLayout<MODE>
             // accepted cells -> monopole buffer
             if (HAS_MONO) {
 #pragma unroll
-                for (int h = 0; h < 2; h++) {
+                for (int h = 0; h < 2; h++) if (h == 0 || wide) {
                     const u32 bal = __ballot_sync(FULL, accept[h]);
                     if (accept[h]) cellbuf[ncb + __popc(bal & lt_mask)] = nA[h];
                     ncb += __popc(bal);
@@ -403,7 +406,7 @@ __global__ void __launch_bounds__(SmemLayout<MODE>::warps * 32, SmemLayout<MODE>
             // TREE: cells accepted within r_out -> K-weighted buffer (counted as cells and as hard-list entries)
             if (TREE && HAS_NEAR) {
 #pragma unroll
-                for (int h = 0; h < 2; h++) {
+                for (int h = 0; h < 2; h++) if (h == 0 || wide) {
                     const u32 bal = __ballot_sync(FULL, accept_near[h]);
                     if (accept_near[h]) partbuf[npb + __popc(bal & lt_mask)] = nA[h];
                     npb += __popc(bal);
@@ -413,7 +416,7 @@ __global__ void __launch_bounds__(SmemLayout<MODE>::warps * 32, SmemLayout<MODE>
             // opened leaves -> queues
             if (HAS_MONO) {
 #pragma unroll
-                for (int h = 0; h < 2; h++) {
+                for (int h = 0; h < 2; h++) if (h == 0 || wide) {
                     const u32 bal = __ballot_sync(FULL, leaf_far[h]);
                     if (bal) {
                         const u32 cnt = leaf_far[h] ? (mt[h].y & 0x7FFFFFFFu) : 0u;
@@ -425,7 +428,7 @@ __global__ void __launch_bounds__(SmemLayout<MODE>::warps * 32, SmemLayout<MODE>
             }
             if (HAS_NEAR) {
 #pragma unroll
-                for (int h = 0; h < 2; h++) {
+                for (int h = 0; h < 2; h++) if (h == 0 || wide) {
                     const u32 bal = __ballot_sync(FULL, leaf_near[h]);
                     if (bal) {
                         const u32 cnt = leaf_near[h] ? (mt[h].y & 0x7FFFFFFFu) : 0u;
