@@ -240,7 +240,9 @@ int hyb_export(hyb_ctx *ctx, int32_t what, void *host_dst, size_t bytes, size_t 
  * one call per cycle with nothing computed twice, and with the bits a device-resident context gives.  The device
  * buffer (particles + workspace, the library's only device allocation), its stream and -- while n and the
  * parameters stay the same -- the context are kept for the next call on the same device (freed by
- * hyb_run_host_release, or replaced when a larger n comes); concurrent calls are serialised.  Every pointer is
+ * hyb_run_host_release, or replaced when a larger n comes); concurrent calls are serialised.  Positions and ids
+ * travel back while the last walk of the call still runs (they are final once its tree is built); when the call
+ * returns an error the contents of the host arrays are unspecified.  Every pointer is
  * a HOST pointer to n elements; h_interactions (optional) receives uint64[4] as HYB_X_INTERACTIONS. */
 int hyb_run_host(const hyb_params *params, int64_t n, hyb_float4 *h_pos_m, hyb_float4 *h_vel,
                  hyb_float4 *h_a_soft, hyb_float4 *h_a_hard, uint32_t *h_id, int32_t n_soft_steps,

@@ -182,19 +182,31 @@ static int do_hard(Ctx *c)
 using namespace hyb;
 
 // device buffer, stream and context kept between hyb_run_host calls
-static struct { char *ptr; size_t bytes; int device; cudaStream_t st; hyb_ctx *ctx; hyb_params p; int64_t n; } g_host =
-    {nullptr, 0, -1, nullptr, nullptr, {}, 0};
+static struct { char *ptr; size_t bytes; int device; cudaStream_t st, st2; hyb_ctx *ctx; hyb_params p; int64_t n; } g_host =
+    {nullptr, 0, -1, nullptr, nullptr, nullptr, {}, 0};
+struct EarlyCopy { hyb_float4 *h_pos; uint32_t *h_id; const char *d_pos, *d_id; size_t n; cudaStream_t st2; bool done; };
+// the store is final once the last build's re-order has been copied back (ev_groups follows it on the auxiliary stream)
+static void early_copy(Ctx *c, void *arg)
+{
+    EarlyCopy *x = static_cast<EarlyCopy *>(arg);
+    cudaStreamWaitEvent(x->st2, c->ev_groups, 0);
+    cudaMemcpyAsync(x->h_pos, x->d_pos, 16 * x->n, cudaMemcpyDeviceToHost, x->st2);
+    cudaMemcpyAsync(x->h_id, x->d_id, 4 * x->n, cudaMemcpyDeviceToHost, x->st2);
+    x->done = true;
+}
 static std::mutex g_host_mutex;
 static void release_host_cache()
 {
     if (g_host.ptr) {
         cudaSetDevice(g_host.device);
         if (g_host.st) cudaStreamSynchronize(g_host.st);
+        if (g_host.st2) cudaStreamSynchronize(g_host.st2);
         if (g_host.ctx) hyb_free(g_host.ctx);
         if (g_host.st) cudaStreamDestroy(g_host.st);
+        if (g_host.st2) cudaStreamDestroy(g_host.st2);
         cudaFree(g_host.ptr);
     }
-    g_host.ptr = nullptr; g_host.bytes = 0; g_host.device = -1; g_host.st = nullptr; g_host.ctx = nullptr; g_host.n = 0;
+    g_host.ptr = nullptr; g_host.bytes = 0; g_host.device = -1; g_host.st = nullptr; g_host.st2 = nullptr; g_host.ctx = nullptr; g_host.n = 0;
 }
 
 extern "C" {
@@ -421,6 +433,7 @@ int hyb_step(hyb_ctx *ctx, int32_t n_soft_steps)
             if (!soft_step && c->p.hard_refit) rc = do_refit(c, k == 0 && c->p.grouping == HYB_GROUP_AUTO);
             else rc = do_build(c, !soft_step);
             if (rc != HYB_OK) return bail(rc);
+            if (c->store_final && cyc == n_soft_steps - 1 && k == nsub - 1) c->store_final(c, c->store_final_arg);
             cudaEvent_t e2 = c->timing ? ev() : nullptr;
             if (soft_step) rc = do_soft(c); else rc = do_hard(c);
             if (rc != HYB_OK) return bail(rc);
@@ -561,6 +574,7 @@ int hyb_run_host(const hyb_params *params, int64_t n, hyb_float4 *h_pos_m, hyb_f
         if (e != cudaSuccess) { g_host.ptr = nullptr; return cuda_fail(nullptr, e, "cudaMalloc"); }
         g_host.bytes = o_ws + ws_bytes; g_host.device = device;
         if ((e = cudaStreamCreate(&g_host.st)) != cudaSuccess) { release_host_cache(); return cuda_fail(nullptr, e, "cudaStreamCreate"); }
+        if ((e = cudaStreamCreateWithFlags(&g_host.st2, cudaStreamNonBlocking)) != cudaSuccess) { release_host_cache(); return cuda_fail(nullptr, e, "cudaStreamCreate"); }
     }
     char *d = g_host.ptr;
     cudaStream_t st = g_host.st;
@@ -591,14 +605,24 @@ int hyb_run_host(const hyb_params *params, int64_t n, hyb_float4 *h_pos_m, hyb_f
         discard_pending_bbox(c);                              // new positions: nothing of the last call's tree applies
         c->tree_valid = false; c->tree_refit = false;
         c->acc_valid = acc_valid != 0 && params->hard_refit == 0;
+        // positions and ids go back on a second stream as soon as the last build of the call has re-ordered them, next to
+        // the last walk (which only reads them); velocities and accelerations follow when the step is done
+        EarlyCopy ec = {h_pos_m, h_id, d + o_pos, d + o_id, N, g_host.st2, false};
+        c->store_final = early_copy; c->store_final_arg = &ec;
         rc = hyb_step(g_host.ctx, n_soft_steps);
-        if (rc != HYB_OK) break;
-        cudaMemcpyAsync(h_pos_m, d + o_pos, 16 * N, cudaMemcpyDeviceToHost, st);
+        c->store_final = nullptr; c->store_final_arg = nullptr;
+        if (rc != HYB_OK) { cudaStreamSynchronize(g_host.st2); break; }
         cudaMemcpyAsync(h_vel, d + o_vel, 16 * N, cudaMemcpyDeviceToHost, st);
         cudaMemcpyAsync(h_a_soft, d + o_as, 16 * N, cudaMemcpyDeviceToHost, st);
         cudaMemcpyAsync(h_a_hard, d + o_ah, 16 * N, cudaMemcpyDeviceToHost, st);
-        cudaMemcpyAsync(h_id, d + o_id, 4 * N, cudaMemcpyDeviceToHost, st);
-        if ((e = cudaStreamSynchronize(st)) != cudaSuccess) { rc = cuda_fail(nullptr, e, "copy back"); break; }
+        if (!ec.done) {          // n_soft_steps = 0: no cycle, the store is the one of the initial build
+            cudaMemcpyAsync(h_pos_m, d + o_pos, 16 * N, cudaMemcpyDeviceToHost, st);
+            cudaMemcpyAsync(h_id, d + o_id, 4 * N, cudaMemcpyDeviceToHost, st);
+        }
+        e = cudaStreamSynchronize(st);
+        const cudaError_t e2 = cudaStreamSynchronize(g_host.st2);
+        if (e == cudaSuccess) e = e2;
+        if (e != cudaSuccess) { rc = cuda_fail(nullptr, e, "copy back"); break; }
         uint64_t v[4];                                        // (read every time: the counters run since the last read)
         rc = hyb_export(g_host.ctx, HYB_X_INTERACTIONS, v, sizeof v, nullptr);
         if (h_interactions)

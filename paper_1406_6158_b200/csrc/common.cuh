@@ -157,6 +157,10 @@ struct Ctx {
     int next_kind = 2;          // the walk the build being enqueued is for
     u32 soft_par = 0;           // slot of DevCtl::soft_work the next fused walk adds to
     bool soft_split = false;    // the fused walk follows a prepared work order (few groups per resident warp; hyb_init)
+    // hyb_run_host: called by hyb_step right after it has enqueued the LAST tree build of the call -- from ev_groups on
+    // the store (positions, ids) has its final order and values, and can travel while the last walk runs
+    void (*store_final)(Ctx *, void *) = nullptr;
+    void *store_final_arg = nullptr;
     bool bbox_ready = false;    // the last drift has already reduced the bounding box of the current positions
     u32 walk_par = 0;           // slot of the walk work counters the next launch uses (DevCtl::group_counter)
     hyb_params p;
