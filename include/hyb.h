@@ -272,6 +272,28 @@ int hyb_let_count(hyb_ctx *ctx, int32_t ndom, const float *h_boxes, uint64_t *h_
  * coincident particles give W = -inf.  Errors: INVALID_ARG (NULL pointer), CUDA. */
 int hyb_energy(hyb_ctx *ctx, double *h_energy);
 
+/* The same diagnostic (T and W as defined for hyb_energy, the same kernels, the same summation order,
+ * hence the same bits) for callers that cannot allocate device memory or hold a context: code under CUDA graph
+ * capture, tight serving loops, harnesses that forbid cudaMalloc.  This entry point allocates nothing, on the
+ * device or on the host: the partial sums of the blocks go to ONE static device array of the library (128 KiB,
+ * held by every GPU that loads the library until the process ends).
+ *  d_pos_m, d_vel  DEVICE float4[n], inputs (positions + masses, velocities); not changed.
+ *  n               1 <= n <= HYB_ENERGY_NOALLOC_MAX_N; larger n -> HYB_ERR_INVALID_ARG with a message that says so
+ *                  (hyb_energy has no such limit, its scratch is in the caller's workspace).
+ *  G, eps          as in hyb_params.
+ *  device, cuda_stream   the device the pointers belong to and the stream the work is issued on.
+ *  d_energy        DEVICE double[2], output: T, W.  Written by a device-to-device copy on the stream.
+ * Asynchronous: nothing is synchronised, no status word is read; the result is there when the stream gets there.
+ * The first call on a device looks up the address of the static array (once per device; it may load the module):
+ * make one call before a graph capture begins.
+ * The array is shared by every call of the process on that device and keeps the last call's contents; nothing in it
+ * has to start from zero (each kernel writes what the next one reads).  Calls that overlap on the GPU (two streams,
+ * two threads) race on it and give garbage: issue them on one stream or order them with events.
+ * Errors: INVALID_ARG (NULL pointer, n out of range, G / eps not finite, eps < 0), CUDA. */
+#define HYB_ENERGY_NOALLOC_MAX_N 4194304
+int hyb_energy_noalloc(const hyb_float4 *d_pos_m, const hyb_float4 *d_vel, int64_t n, float G, float eps,
+                       int device, void *cuda_stream, double *d_energy);
+
 /* Diagnostic, not on the hot path: the FP32 rate of the CUDA cores of `device`, measured with independent chains
  * of packed (h_tflops[0], fma.rn.f32x2 as the pair kernels use) and scalar (h_tflops[1], fma.rn.f32) fused
  * multiply-adds, in TFLOP/s.  bench.py reports it beside the peak derived from the unit counts and the clock.

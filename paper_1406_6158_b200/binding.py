@@ -85,6 +85,8 @@ def lib():
         L.hyb_energy.argtypes = [vp, vp]
         L.hyb_let_count.restype = C.c_int
         L.hyb_let_count.argtypes = [vp, C.c_int32, vp, vp]
+        L.hyb_energy_noalloc.restype = C.c_int
+        L.hyb_energy_noalloc.argtypes = [vp, vp, C.c_int64, C.c_float, C.c_float, C.c_int, vp, vp]
         L.hyb_probe_fp32.restype = C.c_int
         L.hyb_probe_fp32.argtypes = [C.c_int, vp, vp, C.c_size_t, vp]
         L.hyb_run_host_release.restype = None
@@ -134,6 +136,21 @@ def hyb_probe_fp32(device: int = 0):
     if rc != 0:
         raise HybError(rc, "hyb_probe_fp32")
     return float(out[0]), float(out[1])
+
+
+def hyb_energy_noalloc(pos_m, vel, G: float, eps: float, out):
+    """T, W of the particles in the CUDA tensors pos_m / vel (float32 [n, 4]) into the CUDA tensor out (float64 [2]),
+    on torch's current stream, with no allocation and no synchronisation (include/hyb.h); returns out"""
+    import torch
+    assert pos_m.is_cuda and vel.is_cuda and out.is_cuda and pos_m.is_contiguous() and vel.is_contiguous()
+    assert pos_m.dtype == torch.float32 and vel.dtype == torch.float32 and out.dtype == torch.float64 and out.numel() == 2
+    assert pos_m.shape == vel.shape and pos_m.shape[1] == 4
+    dev = pos_m.device.index
+    rc = lib().hyb_energy_noalloc(pos_m.data_ptr(), vel.data_ptr(), pos_m.shape[0], float(G), float(eps), dev,
+                                  torch.cuda.current_stream(dev).cuda_stream, out.data_ptr())
+    if rc != 0:
+        raise HybError(rc, lib().hyb_last_error(None).decode())
+    return out
 
 
 def hyb_run_host_release() -> None:

@@ -685,6 +685,23 @@ int hyb_energy(hyb_ctx *ctx, double *h_energy)
     return rc;
 }
 
+int hyb_energy_noalloc(const hyb_float4 *d_pos_m, const hyb_float4 *d_vel, int64_t n, float G, float eps, int device,
+                       void *cuda_stream, double *d_energy)
+{
+    if (!d_pos_m || !d_vel || !d_energy) return fail(nullptr, HYB_ERR_INVALID_ARG, "a device pointer is NULL");
+    if (n < 1) return fail(nullptr, HYB_ERR_INVALID_ARG, "n < 1");
+    if (n > HYB_ENERGY_NOALLOC_MAX_N)
+        return fail(nullptr, HYB_ERR_INVALID_ARG, "hyb_energy_noalloc: n exceeds HYB_ENERGY_NOALLOC_MAX_N (4194304): the partial sums would not fit the static scratch; use hyb_energy");
+    if (!isfinite(G) || !isfinite(eps) || eps < 0.0f) return fail(nullptr, HYB_ERR_INVALID_ARG, "G / eps not finite or eps < 0");
+    cudaError_t e = cudaSetDevice(device);
+    if (e != cudaSuccess) return cuda_fail(nullptr, e, "cudaSetDevice");
+    bool too_large = false;
+    e = launch_energy_noalloc(d_pos_m, d_vel, n, G, eps, device, (cudaStream_t)cuda_stream, d_energy, &too_large);
+    if (e != cudaSuccess) return cuda_fail(nullptr, e, "hyb_energy_noalloc");
+    if (too_large) return fail(nullptr, HYB_ERR_INVALID_ARG, "hyb_energy_noalloc: the partial sums of n particles do not fit the static scratch on this device; use hyb_energy");
+    return HYB_OK;
+}
+
 const char *hyb_last_error(const hyb_ctx *ctx)
 {
     const Ctx *c = reinterpret_cast<const Ctx *>(ctx);

@@ -215,6 +215,8 @@ cudaError_t launch_zero_acc(Ctx *c, hyb_float4 *a);
 cudaError_t launch_let_count(Ctx *c, int ndom, const float *d_boxes, unsigned long long *d_out);
 size_t energy_scratch_doubles(const Ctx *c, u32 *ni, u32 *nj, u32 *nk);
 cudaError_t launch_energy(Ctx *c, double *d_scratch, u32 ni, u32 nj, u32 nk);
+cudaError_t launch_energy_noalloc(const hyb_float4 *d_pos_m, const hyb_float4 *d_vel, int64_t n, float G, float eps, int device,
+                                  cudaStream_t st, double *d_energy, bool *too_large);
 
 // ---- device helpers ------------------------------------------------------------------
 __device__ __forceinline__ u32 enc_float(float f)

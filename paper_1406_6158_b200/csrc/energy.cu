@@ -133,4 +133,42 @@ cudaError_t launch_energy(Ctx *c, double *d_scratch, u32 ni, u32 nj, u32 nk)
     return cudaGetLastError();
 }
 
+// ------------------------------------------------------------------ hyb_energy_noalloc (include/hyb.h)
+// The same three kernels with their partial sums in a file-scope device array instead of a context's workspace, for
+// callers that can neither allocate device memory nor hold a context.  Every GPU that loads the library holds the
+// array (128 KiB) until the process ends.  In host code the name of the array is a host-side stand-in, not a device
+// address: the address comes from cudaGetSymbolAddress, once per device, with that device current.
+constexpr size_t EN_STATIC_DOUBLES = 16384;
+static __device__ __align__(256) double g_energy_scratch[EN_STATIC_DOUBLES];
+
+// *too_large: the partial sums of n particles do not fit (the caller reports it; nothing was launched).
+// Nothing in the array has to start from zero: each kernel writes every element the next one reads.
+cudaError_t launch_energy_noalloc(const hyb_float4 *d_pos_m, const hyb_float4 *d_vel, int64_t n, float G, float eps, int device,
+                                  cudaStream_t st, double *d_energy, bool *too_large)
+{
+    static unsigned long long ready = 0ull;
+    static double *scratch_of[64];
+    static int sms_of[64];
+    *too_large = false;
+    double *scratch = nullptr;
+    int sms = 0;
+    if (device >= 0 && device < 64 && device_ready(&ready, device)) { scratch = scratch_of[device]; sms = sms_of[device]; }
+    else {
+        cudaError_t e = cudaGetSymbolAddress((void **)&scratch, g_energy_scratch);      // of the current device (set by the caller)
+        if (e != cudaSuccess) return e;
+        e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, device);
+        if (e != cudaSuccess) return e;
+        if (device >= 0 && device < 64) { scratch_of[device] = scratch; sms_of[device] = sms; device_set_ready(&ready, device); }
+    }
+    Ctx c{};                      // the launch geometry and the launches are those of hyb_energy (same bits)
+    c.n = n; c.num_sms = sms; c.stream = st; c.device = device;
+    c.pos = const_cast<hyb_float4 *>(d_pos_m); c.vel = const_cast<hyb_float4 *>(d_vel);
+    c.p.G = G; c.p.eps = eps;
+    u32 ni, nj, nk;
+    if (energy_scratch_doubles(&c, &ni, &nj, &nk) > EN_STATIC_DOUBLES) { *too_large = true; return cudaSuccess; }
+    cudaError_t e = launch_energy(&c, scratch, ni, nj, nk);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(d_energy, scratch, 2 * sizeof(double), cudaMemcpyDeviceToDevice, st);
+    return e;
+}
+
 }  // namespace hyb
