@@ -157,6 +157,7 @@ struct Ctx {
     int next_kind = 2;          // the walk the build being enqueued is for
     u32 soft_par = 0;           // slot of DevCtl::soft_work the next fused walk adds to
     bool soft_split = false;    // the fused walk follows a prepared work order (few groups per resident warp; hyb_init)
+    bool hard_small = false;    // the hard walk runs its small-N variant (SmemLayout<WALK_HARD, true>; hyb_init)
     // hyb_run_host: called by hyb_step right after it has enqueued the LAST tree build of the call -- from ev_groups on
     // the store (positions, ids) has its final order and values, and can travel while the last walk runs
     void (*store_final)(Ctx *, void *) = nullptr;

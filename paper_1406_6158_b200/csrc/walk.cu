@@ -46,11 +46,15 @@ struct WalkArgs {
 // hard walk: estimated pair count (members x hard-list length) above which a group is cut in 2 / 4 ranges
 constexpr u32 DESC_MASK = 0x1FFFFFFFu;      // node index bits of a stack descriptor
 
-template <int MODE>
+// SMALL (hard walk only): the variant for runs with about one work item per resident warp (Ctx::hard_small), where
+// the walk is a chain of round trips and nothing else: 128 particles per expansion step instead of 64, and 2 CTAs per SM
+// with 128 registers (no spills) instead of 3 with 80.
+template <int MODE, bool SMALL = false>
 struct SmemLayout {                 // per warp
     static constexpr int cell_cap = MODE == WALK_HARD ? 0 : WK_CELL_CAP;
     // the hard walk has no monopole buffer, so its K-weighted buffer can be larger (fewer flushes) at 3 CTAs per SM
-    static constexpr int part_cap = MODE == WALK_NORMAL ? 0 : (MODE == WALK_HARD ? 256 : WK_PART_CAP);
+    static constexpr int part_cap = MODE == WALK_NORMAL ? 0 : (MODE == WALK_HARD ? (SMALL ? 384 : 256) : WK_PART_CAP);
+    static constexpr int NE = SMALL ? 4 : 2;          // x 32 particles per expansion step
     static constexpr int stack_cap = MODE == WALK_HYBRID ? 320 : 512;
     static constexpr int lq_cap = 96;
     static constexpr int nqueues = MODE == WALK_HYBRID ? 3 : 2;      // far leaves, near leaves, runs of accepted children
@@ -59,7 +63,7 @@ struct SmemLayout {                 // per warp
     static constexpr size_t bytes = 16 * (size_t)(cell_alloc + part_alloc) + 4 * (size_t)stack_cap + 8 * (size_t)nqueues * (size_t)lq_cap;
     // measured in round 2 (profiles/r02_profile.md): 2 x 8, 2 x 10, 3 x 7, 4 x 6 warps per SM make no difference to the hard
     // walk; the fused walk needs its 128 registers (anything that caps them lower spills and loses 20 %)
-    static constexpr int ctas_per_sm = MODE == WALK_HARD ? 3 : 2;
+    static constexpr int ctas_per_sm = (MODE == WALK_HARD && !SMALL) ? 3 : 2;
     static constexpr int warps = WK_WARPS;      // per CTA
 };
 
@@ -71,10 +75,10 @@ struct SmemLayout {                 // per warp
 // r_out of the group box; the other particles of a near leaf are plain Eq. 2 pairs (monopole buffer).
 // SPLIT: the work order prepared by split_group is followed (always in the hard-only walk; in the fused walk when
 // the particle number is small, Ctx::soft_split).
-template <int MODE, int KF, bool TREE, bool CUT, bool SPLIT>
-__global__ void __launch_bounds__(SmemLayout<MODE>::warps * 32, SmemLayout<MODE>::ctas_per_sm) walk_kernel(const WalkArgs a)
+template <int MODE, int KF, bool TREE, bool CUT, bool SPLIT, bool SMALL>
+__global__ void __launch_bounds__(SmemLayout<MODE, SMALL>::warps * 32, SmemLayout<MODE, SMALL>::ctas_per_sm) walk_kernel(const WalkArgs a)
 {
-    using SL = SmemLayout<MODE>;
+    using SL = SmemLayout<MODE, SMALL>;
     constexpr bool HAS_MONO = MODE != WALK_HARD;      // monopole buffer (cells, far particles)
     constexpr bool HAS_NEAR = MODE != WALK_NORMAL;    // K-weighted buffer
     constexpr int C = MODE == WALK_HYBRID ? 6 : 3;    // accumulated components per sink
@@ -207,12 +211,14 @@ __global__ void __launch_bounds__(SmemLayout<MODE>::warps * 32, SmemLayout<MODE>
                 if (ex_done < ex_T) {
                     const bool tonear = HAS_NEAR && (!HAS_MONO || ex_near == 1);
                     const bool cutting = CUT && tonear;
-                    if (tonear && npb + 64 > SL::part_cap) { flush_near = true; continue; }
-                    if (HAS_MONO && (!tonear || cutting) && ncb + 64 > SL::cell_cap) { flush_mono = true; continue; }
-                    float4 p[2];
-                    bool ok[2];
+                    constexpr int NE = SL::NE;
+                    if (tonear && npb + 32 * NE > SL::part_cap) { flush_near = true; continue; }
+                    if (HAS_MONO && (!tonear || cutting) && ncb + 32 * NE > SL::cell_cap) { flush_mono = true; continue; }
+                    float4 p[NE];
+                    bool ok[NE];
 #pragma unroll
-                    for (int u = 0; u < 2; u++) {
+                    for (int u = 0; u < NE; u++) {
+                        if (NE > 2 && ex_done + 32u * u >= ex_T) { ok[u] = false; continue; }      // (uniform) nothing left for this quarter
                         const u32 slot = ex_done + 32u * u + (u32)lane;
                         ok[u] = slot < ex_T;
                         int j = 0;                      // the last leaf that starts at or before this particle
@@ -225,7 +231,8 @@ __global__ void __launch_bounds__(SmemLayout<MODE>::warps * 32, SmemLayout<MODE>
                         if (ok[u]) p[u] = __ldg(a.pos + fj + (slot - oj));
                     }
 #pragma unroll
-                    for (int u = 0; u < 2; u++) {
+                    for (int u = 0; u < NE; u++) {
+                        if (NE > 2 && ex_done + 32u * u >= ex_T) continue;
                         if (cutting) {
                             bool nr = false;
                             if (ok[u]) {
@@ -249,7 +256,7 @@ __global__ void __launch_bounds__(SmemLayout<MODE>::warps * 32, SmemLayout<MODE>
                             else { if (ok[u]) cellbuf[ncb + lane] = p[u]; ncb += cnt; }
                         }
                     }
-                    ex_done += 64u;
+                    ex_done += 32u * NE;
                     continue;
                 }
                 // ---- runs of accepted children: eight runs per step, lane (oct, sub) copies child sub of runs oct and
@@ -545,10 +552,10 @@ cudaError_t launch_zero_acc(Ctx *c, hyb_float4 *a)
     return cudaGetLastError();
 }
 
-template <int MODE, int KF, bool TREE, bool CUT, bool SPLIT>
+template <int MODE, int KF, bool TREE, bool CUT, bool SPLIT, bool SMALL>
 static cudaError_t launch_walk_mode(Ctx *c, const WalkArgs &a)
 {
-    using SL = SmemLayout<MODE>;
+    using SL = SmemLayout<MODE, SMALL>;
     const size_t smem = SL::bytes * SL::warps;
     static unsigned long long ready = 0ull;
     if (!device_ready(&ready, c->device)) {
@@ -556,11 +563,11 @@ static cudaError_t launch_walk_mode(Ctx *c, const WalkArgs &a)
         sink_layout(t);
         cudaError_t e = cudaMemcpyToSymbol(c_layout, t, sizeof t);
         if (e != cudaSuccess) return e;
-        e = cudaFuncSetAttribute(walk_kernel<MODE, KF, TREE, CUT, SPLIT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        e = cudaFuncSetAttribute(walk_kernel<MODE, KF, TREE, CUT, SPLIT, SMALL>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
         device_set_ready(&ready, c->device);
     }
-    walk_kernel<MODE, KF, TREE, CUT, SPLIT><<<c->num_sms * SL::ctas_per_sm, SL::warps * 32, smem, c->stream>>>(a);
+    walk_kernel<MODE, KF, TREE, CUT, SPLIT, SMALL><<<c->num_sms * SL::ctas_per_sm, SL::warps * 32, smem, c->stream>>>(a);
     return cudaGetLastError();
 }
 
@@ -603,15 +610,21 @@ cudaError_t launch_walk(Ctx *c, int mode)
     if (mode != WALK_HARD) c->soft_par ^= 1u;
     c->split_ready = false;
     const bool poly7 = c->p.kfunc == HYB_K_POLY7, tree = c->p.hard_tree != 0, cut = c->p.hard_cut != 0;
-    if (mode == WALK_NORMAL) return launch_walk_mode<WALK_NORMAL, HYB_K_PAPER, false, false, false>(c, a);
-#define HYB_WALK_CASE(M, K, T, C, S) if (poly7 == (K == HYB_K_POLY7) && tree == T && cut == C && sched == S) return launch_walk_mode<M, K, T, C, S>(c, a)
+    if (mode == WALK_NORMAL) return launch_walk_mode<WALK_NORMAL, HYB_K_PAPER, false, false, false, false>(c, a);
+#define HYB_WALK_CASE(M, K, T, C, S) if (poly7 == (K == HYB_K_POLY7) && tree == T && cut == C && sched == S && small == SM) return launch_walk_mode<M, K, T, C, S, SM>(c, a)
 #define HYB_WALK_CASES(M, S) \
     HYB_WALK_CASE(M, HYB_K_PAPER, false, false, S); HYB_WALK_CASE(M, HYB_K_PAPER, false, true, S); \
     HYB_WALK_CASE(M, HYB_K_PAPER, true, false, S); HYB_WALK_CASE(M, HYB_K_PAPER, true, true, S); \
     HYB_WALK_CASE(M, HYB_K_POLY7, false, false, S); HYB_WALK_CASE(M, HYB_K_POLY7, false, true, S); \
     HYB_WALK_CASE(M, HYB_K_POLY7, true, false, S); HYB_WALK_CASE(M, HYB_K_POLY7, true, true, S)
+    const bool small = mode == WALK_HARD && c->hard_small;
+#define SM false
     if (mode == WALK_HYBRID) { HYB_WALK_CASES(WALK_HYBRID, false); HYB_WALK_CASES(WALK_HYBRID, true); }
     HYB_WALK_CASES(WALK_HARD, true);
+#undef SM
+#define SM true
+    HYB_WALK_CASES(WALK_HARD, true);
+#undef SM
 #undef HYB_WALK_CASES
 #undef HYB_WALK_CASE
     return cudaErrorInvalidValue;
