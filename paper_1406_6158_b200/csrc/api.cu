@@ -259,8 +259,10 @@ int hyb_init(hyb_ctx **out, const hyb_params *params, int64_t n, hyb_float4 *d_p
     // with fewer than a few sink groups per resident warp the longest groups set the duration of the fused walk: it
     // then follows the work order of split_group (measured: cfg1 soft walk 0.60 -> 0.45 ms; from 2^20 particles up the
     // Morton order is 1-2 % faster, its neighbours share cache lines)
-    c->soft_split = params->split && n < (int64_t)160 * c->num_sms * 2 * WK_WARPS;
-    c->hard_small = c->soft_split;      // (cfg1: 7 hard walks 0.29 -> 0.24 ms, cfg0 0.094 -> 0.077; at N = 2^20 the same variant is 6 % slower)
+    c->soft_split = params->split && n < (int64_t)SMALL_RUN_PER_WARP * c->num_sms * 2 * WK_WARPS;
+    // (cfg1: 7 hard walks 0.29 -> 0.24 ms, cfg0 0.094 -> 0.077; at N = 2^20 the same variant is 6 % slower for the direct
+    // hard sum, but 3-6 % faster for the tree-approximated hard walk, whose 80-register instantiation spills)
+    c->hard_small = c->soft_split || params->hard_tree != 0;
     e = cudaMemsetAsync(c->ctl, 0, sizeof(DevCtl), c->stream);
     if (e == cudaSuccess) e = cudaMemsetAsync(c->ws + L.nhard, 0, 4 * (size_t)L.group_cap, c->stream);
     if (e == cudaSuccess) e = cudaMemsetAsync(c->ws + L.scost, 0, 4 * (size_t)L.group_cap, c->stream);
@@ -286,8 +288,8 @@ int hyb_set_params(hyb_ctx *ctx, const hyb_params *params)
     if (params->leaf_max != c->p.leaf_max || params->group_max != c->p.group_max || params->grouping != c->p.grouping)
         return fail(c, HYB_ERR_INVALID_ARG, "leaf_max / group_max / grouping cannot change after hyb_init");
     c->p = *params;
-    c->soft_split = params->split && c->n < (int64_t)160 * c->num_sms * 2 * WK_WARPS;
-    c->hard_small = c->soft_split;
+    c->soft_split = params->split && c->n < (int64_t)SMALL_RUN_PER_WARP * c->num_sms * 2 * WK_WARPS;
+    c->hard_small = c->soft_split || params->hard_tree != 0;
     c->split_ready = false;
     c->tree_valid = false; c->acc_valid = false;
     return HYB_OK;

@@ -39,6 +39,9 @@ constexpr int PO_TILE = SC_THREADS * PO_IPT;
 
 // walk kernel geometry
 constexpr int WK_WARPS = 8;              // warps per CTA
+#ifndef SMALL_RUN_PER_WARP
+#define SMALL_RUN_PER_WARP 160         // particles per resident warp below which a run counts as small (Ctx::soft_split, hard_small)
+#endif
 constexpr int WK_U = 4;                  // sources per iteration of the pair loops (pairs.cuh)
 constexpr int WK_CELL_CAP = 320;         // monopole buffer entries per warp
 constexpr int WK_PART_CAP = 192;         // K-weighted (near) particle buffer entries per warp
