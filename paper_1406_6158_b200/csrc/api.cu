@@ -184,14 +184,14 @@ using namespace hyb;
 // device buffer, stream and context kept between hyb_run_host calls
 static struct { char *ptr; size_t bytes; int device; cudaStream_t st, st2; hyb_ctx *ctx; hyb_params p; int64_t n; } g_host =
     {nullptr, 0, -1, nullptr, nullptr, nullptr, {}, 0};
-struct EarlyCopy { hyb_float4 *h_pos; uint32_t *h_id; const char *d_pos, *d_id; size_t n; cudaStream_t st2; bool done; };
+struct EarlyCopy { hyb_float4 *h_pos; uint32_t *h_id; size_t n; cudaStream_t st2; bool done; };
 // the store is final once the last build's re-order has been copied back (ev_groups follows it on the auxiliary stream)
 static void early_copy(Ctx *c, void *arg)
 {
     EarlyCopy *x = static_cast<EarlyCopy *>(arg);
     cudaStreamWaitEvent(x->st2, c->ev_groups, 0);
-    cudaMemcpyAsync(x->h_pos, x->d_pos, 16 * x->n, cudaMemcpyDeviceToHost, x->st2);
-    cudaMemcpyAsync(x->h_id, x->d_id, 4 * x->n, cudaMemcpyDeviceToHost, x->st2);
+    cudaMemcpyAsync(x->h_pos, c->pos, 16 * x->n, cudaMemcpyDeviceToHost, x->st2);      // (wherever the store is right now)
+    cudaMemcpyAsync(x->h_id, c->id, 4 * x->n, cudaMemcpyDeviceToHost, x->st2);
     x->done = true;
 }
 static std::mutex g_host_mutex;
@@ -241,6 +241,7 @@ int hyb_init(hyb_ctx **out, const hyb_params *params, int64_t n, hyb_float4 *d_p
     c->sink_lo = 0u; c->sink_hi = (u32)n;
     c->p = *params; c->n = n; c->device = device; c->stream = (cudaStream_t)cuda_stream;
     c->pos = d_pos_m; c->vel = d_vel; c->a_soft = d_a_soft; c->a_hard = d_a_hard; c->id = d_id;
+    c->pos_home = d_pos_m; c->vel_home = d_vel; c->id_home = d_id;
     c->ws = (char *)d_workspace; c->L = L; c->ctl = (DevCtl *)(c->ws + L.ctl);
     e = cudaDeviceGetAttribute(&c->num_sms, cudaDevAttrMultiProcessorCount, device);
     if (e != cudaSuccess) { const int rc = cuda_fail(nullptr, e, "cudaDeviceGetAttribute"); hyb_free(reinterpret_cast<hyb_ctx *>(c)); return rc; }
@@ -419,7 +420,11 @@ int hyb_step(hyb_ctx *ctx, int32_t n_soft_steps)
     }
     size_t ev_used = 0;
     auto ev = [&]() { cudaEvent_t e = c->evpool[ev_used++]; cudaEventRecord(e, c->stream); return e; };
-    auto bail = [&](int code) { c->tree_valid = false; c->acc_valid = false; return code; };
+    auto bail = [&](int code) {
+        c->defer_copy = false; store_come_home(c);
+        c->tree_valid = false; c->acc_valid = false; return code;
+    };
+    c->defer_copy = true;      // builds leave the store where they re-ordered it to; it is home again when the call returns
     for (int32_t cyc = 0; cyc < n_soft_steps; cyc++) {
         for (int k = 0; k < nsub; k++) {
             cudaEvent_t e0 = c->timing ? ev() : nullptr;
@@ -456,6 +461,11 @@ int hyb_step(hyb_ctx *ctx, int32_t n_soft_steps)
             }
         }
         c->acc_valid = true;
+    }
+    c->defer_copy = false;
+    {
+        const cudaError_t e = store_come_home(c);
+        if (e != cudaSuccess) return bail(cuda_fail(c, e, "store copy"));
     }
     rc = hyb_sync(ctx);
     if (rc == HYB_OK)
@@ -611,7 +621,7 @@ int hyb_run_host(const hyb_params *params, int64_t n, hyb_float4 *h_pos_m, hyb_f
         c->acc_valid = acc_valid != 0 && params->hard_refit == 0;
         // positions and ids go back on a second stream as soon as the last build of the call has re-ordered them, next to
         // the last walk (which only reads them); velocities and accelerations follow when the step is done
-        EarlyCopy ec = {h_pos_m, h_id, d + o_pos, d + o_id, N, g_host.st2, false};
+        EarlyCopy ec = {h_pos_m, h_id, N, g_host.st2, false};
         c->store_final = early_copy; c->store_final_arg = &ec;
         rc = hyb_step(g_host.ctx, n_soft_steps);
         c->store_final = nullptr; c->store_final_arg = nullptr;

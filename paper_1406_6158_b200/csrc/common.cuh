@@ -160,6 +160,14 @@ struct Ctx {
     int next_kind = 2;          // the walk the build being enqueued is for
     u32 soft_par = 0;           // slot of DevCtl::soft_work the next fused walk adds to
     bool soft_split = false;    // the fused walk follows a prepared work order (few groups per resident warp; hyb_init)
+    // The store (positions, velocities, ids) lives in the caller's arrays.  A build re-orders it into the workspace copy
+    // and copies it back -- unless hyb_step has set defer_copy: then pos / vel / id simply point to the workspace copy
+    // afterwards (store_away) and the next build re-orders straight back into the caller's arrays; hyb_step returns with
+    // the store at home (one copy if the number of builds of the call was odd).
+    const float4 *pos_sorted = nullptr;          // where the build being enqueued puts the re-ordered positions
+    hyb_float4 *pos_home = nullptr, *vel_home = nullptr;
+    u32 *id_home = nullptr;
+    bool defer_copy = false, store_away = false;
     bool hard_small = false;    // the hard walk runs its small-N variant (SmemLayout<WALK_HARD, true>; hyb_init)
     // hyb_run_host: called by hyb_step right after it has enqueued the LAST tree build of the call -- from ev_groups on
     // the store (positions, ids) has its final order and values, and can travel while the last walk runs
@@ -211,6 +219,7 @@ static inline T *wsptr(const Ctx *c, size_t off) { return reinterpret_cast<T *>(
 
 // stage launchers (each enqueues on c->stream and returns the last CUDA error)
 cudaError_t launch_build_tree(Ctx *c);
+cudaError_t store_come_home(Ctx *c);        // no-op unless store_away: the workspace copy goes to the caller's arrays
 cudaError_t launch_regroup(Ctx *c);        // sink groups again (group_max_now / grouping_now) on the existing topology
 cudaError_t launch_refit_tree(Ctx *c);     // tight boxes of nodes and groups for the current positions, same topology
 cudaError_t launch_walk(Ctx *c, int mode);

@@ -137,14 +137,37 @@ cudaError_t launch_keys_sort_permute(Ctx *c)
     cudaStream_t ax = c->aux;
     cudaEventRecord(c->ev_sorted, st);
     cudaStreamWaitEvent(ax, c->ev_sorted, 0);
-    float4 *pos_t = wsptr<float4>(c, L.pos_tmp), *vel_t = wsptr<float4>(c, L.vel_tmp);
-    u32 *id_t = wsptr<u32>(c, L.id_tmp);
+    float4 *pos_w = wsptr<float4>(c, L.pos_tmp), *vel_w = wsptr<float4>(c, L.vel_tmp);
+    u32 *id_w = wsptr<u32>(c, L.id_tmp);
+    // destination: the copy the store is not in
+    float4 *pos_t = c->store_away ? reinterpret_cast<float4 *>(c->pos_home) : pos_w;
+    float4 *vel_t = c->store_away ? reinterpret_cast<float4 *>(c->vel_home) : vel_w;
+    u32 *id_t = c->store_away ? c->id_home : id_w;
     permute_kernel<<<grid, 256, 0, ax>>>(val_b, n, reinterpret_cast<const float4 *>(c->pos),
                                          reinterpret_cast<const float4 *>(c->vel), c->id, pos_t, vel_t, id_t);
     cudaEventRecord(c->ev_perm, ax);
-    cudaMemcpyAsync(c->pos, pos_t, sizeof(float4) * (size_t)n, cudaMemcpyDeviceToDevice, ax);
-    cudaMemcpyAsync(c->vel, vel_t, sizeof(float4) * (size_t)n, cudaMemcpyDeviceToDevice, ax);
-    cudaMemcpyAsync(c->id, id_t, sizeof(u32) * (size_t)n, cudaMemcpyDeviceToDevice, ax);
+    c->pos_sorted = pos_t;
+    if (c->store_away) {                    // re-ordered straight into the caller's arrays
+        c->pos = c->pos_home; c->vel = c->vel_home; c->id = c->id_home; c->store_away = false;
+    } else if (c->defer_copy) {             // hyb_step: stay in the workspace copy until the next build
+        c->pos = reinterpret_cast<hyb_float4 *>(pos_w); c->vel = reinterpret_cast<hyb_float4 *>(vel_w); c->id = id_w;
+        c->store_away = true;
+    } else {
+        cudaMemcpyAsync(c->pos, pos_t, sizeof(float4) * (size_t)n, cudaMemcpyDeviceToDevice, ax);
+        cudaMemcpyAsync(c->vel, vel_t, sizeof(float4) * (size_t)n, cudaMemcpyDeviceToDevice, ax);
+        cudaMemcpyAsync(c->id, id_t, sizeof(u32) * (size_t)n, cudaMemcpyDeviceToDevice, ax);
+    }
+    return cudaGetLastError();
+}
+
+cudaError_t store_come_home(Ctx *c)
+{
+    if (!c->store_away) return cudaSuccess;
+    const size_t n = (size_t)c->n;
+    cudaMemcpyAsync(c->pos_home, c->pos, sizeof(float4) * n, cudaMemcpyDeviceToDevice, c->stream);
+    cudaMemcpyAsync(c->vel_home, c->vel, sizeof(float4) * n, cudaMemcpyDeviceToDevice, c->stream);
+    cudaMemcpyAsync(c->id_home, c->id, sizeof(u32) * n, cudaMemcpyDeviceToDevice, c->stream);
+    c->pos = c->pos_home; c->vel = c->vel_home; c->id = c->id_home; c->store_away = false;
     return cudaGetLastError();
 }
 

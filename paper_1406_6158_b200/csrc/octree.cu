@@ -635,7 +635,7 @@ cudaError_t launch_build_tree(Ctx *c)
                                            first, count, child, nchild, parent, arrived, rec, bmax2);
     // sink groups need only the topology and the permuted positions: auxiliary stream, next to the upsweep
     cudaStream_t ax = c->aux;
-    const float4 *pos_t = wsptr<float4>(c, L.pos_tmp);      // == the re-ordered store (copied back on aux)
+    const float4 *pos_t = c->pos_sorted;      // the re-ordered store (launch_keys_sort_permute)
     cudaEventRecord(c->ev_linked, st);
     cudaStreamWaitEvent(ax, c->ev_linked, 0);
     unsigned char *gflag = wsptr<unsigned char>(c, L.gflag);
