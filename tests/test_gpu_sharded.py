@@ -61,14 +61,16 @@ def test_ranges_sum_to_the_full_result():
     h.close()
 
 
-@pytest.mark.parametrize("split", [1, 0])
-def test_call_by_call_cycle_equals_hyb_step(split):
+@pytest.mark.parametrize("split,n_sub", [(1, 4), (0, 4), (1, 3), (1, 1)])
+def test_call_by_call_cycle_equals_hyb_step(split, n_sub):
+    """(n_sub = 3, 1: an odd number of builds per hyb_step call -- inside the call the builds move the store between the
+    caller's arrays and the workspace copy, and it has to be home again when the call returns)"""
     from types import SimpleNamespace
     from paper_1406_6158_b200.sharded import ShardedHyb
-    cfg = CONFIGS[1].with_(n=50021, split=split)
+    cfg = CONFIGS[1].with_(n=50021, split=split, n_sub=n_sub)
     pos, vel = make_ic(cfg.kind, cfg.n, 8)
     ref = make_hyb(cfg, pos, vel)
-    ref.step(2); ref.sync()
+    ref.step(1); ref.step(1); ref.sync()                   # (two calls: n_sub builds in the second one)
     h = make_hyb(cfg, pos, vel)
     sh = ShardedHyb(h, SimpleNamespace(split=cfg.split, n_sub=cfg.n_sub, dt_soft=cfg.dt_soft), 0, 1, lambda t: None)
     sh.step(2); h.sync()
