@@ -65,3 +65,41 @@ def test_random_configuration(seed):
     h.step(1); h.sync()
     assert np.all(np.isfinite(h.pos_m.cpu().numpy()))
     h.close()
+
+
+@pytest.mark.parametrize("seed", range(4))
+def test_random_configuration_medium(seed):
+    """the same on both sides of the size where the walks change their work order and the hard walk its instantiation
+    (3.8e5 particles on a B200), accelerations and list lengths on sampled groups"""
+    from workloads import make_ic
+    rng = np.random.default_rng(5000 + seed)
+    n = int(rng.choice([378879, 378881, 400003, 524288]))
+    kind = str(rng.choice(["plummer", "hernquist", "cold_sphere", "two_plummer"]))
+    leaf = int(rng.choice([4, 8, 16, 24])); group = int(rng.choice([g for g in (16, 32, 48, 64) if g >= leaf]))
+    r_out = float(rng.choice([0.01, 0.03, 0.08]))
+    cfg = CONFIGS[2].with_(n=n, kind=kind, leaf_max=leaf, group_max=group, r_out=r_out, r_in=float(r_out * rng.choice([0.0, 0.1, 0.5])),
+                           theta=float(rng.choice([0.4, 0.5, 0.8])), eps=float(rng.choice([1e-3, 0.01])), mac=int(rng.integers(0, 2)),
+                           grouping=int(rng.integers(0, 3)), kfunc=int(rng.integers(0, 2)), hard_cut=int(rng.integers(0, 2)),
+                           hard_tree=int(rng.random() < 0.3))
+    pos, vel = make_ic(kind, n, 100 + seed)
+    h = make_hyb(cfg, pos, vel)
+    h.build_tree(); h.sync()
+    t = O.Tree(pos, O.params_from(cfg))
+    compare_tree(h, t, abs_mode=cfg.mac == 1)
+    sample = lambda ng, k, s: np.sort(np.random.default_rng(s).choice(ng, size=min(k, ng), replace=False)).astype(np.int64)
+    check_forces(h, t, gsel=sample(t.ng, 2048, seed))
+    store = h.pos_m.cpu().numpy()                          # second walk on the same store: prepared work order
+    h.build_tree(); h.sync(); h.export("interactions")
+    t2 = O.Tree(store, O.params_from(cfg))
+    check_forces(h, t2, gsel=sample(t2.ng, 1024, seed + 1))
+    if not cfg.hard_tree:
+        store = h.pos_m.cpu().numpy()
+        h.build_tree_hard(); h.sync()
+        gm = max(cfg.group_max // 2, cfg.leaf_max) if cfg.grouping == 2 else cfg.group_max
+        th = O.Tree(store, O.params_from(cfg, group_max=gm))
+        compare_tree(h, th, boxes_only=True)
+        h.hard_force(); h.sync()
+        compare_lists(h, th, O.MODE_HARD)
+    h.step(1); h.sync()
+    assert np.all(np.isfinite(h.pos_m.cpu().numpy()))
+    h.close()
