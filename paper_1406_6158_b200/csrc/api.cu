@@ -24,8 +24,10 @@ Layout plan_workspace(int64_t n)
     L.n = n;
     L.node_cap = node_capacity(n);
     L.group_cap = n;
-    L.rs_tiles = (n + RS_TILE - 1) / RS_TILE;
-    L.node_tiles = (L.node_cap + RS_TILE - 1) / RS_TILE;
+    L.rs_kpt = rs_kpt_for(n);
+    const int64_t rs_tile = (int64_t)RS_THREADS * L.rs_kpt;
+    L.rs_tiles = (n + rs_tile - 1) / rs_tile;
+    L.node_tiles = (L.node_cap + rs_tile - 1) / rs_tile;
     L.sc_tiles = (n + SC_TILE - 1) / SC_TILE;
     L.po_tiles = (n + PO_TILE - 1) / PO_TILE;
     L.rs_blocks = (L.rs_tiles + LB_WIN - 1) / LB_WIN;

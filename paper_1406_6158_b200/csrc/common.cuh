@@ -25,8 +25,12 @@ constexpr u32 ST_WAIT_EXPIRED = 8u;
 // radix sort tiling (onesweep): 256 threads x 14 keys = 3584 keys per tile (2^20 keys = 293 tiles, two per SM on
 // 148 SMs; with 4096-key tiles 40 SMs had one tile and 108 had two)
 constexpr int RS_THREADS = 256;
-constexpr int RS_KPT = 14;
-constexpr int RS_TILE = RS_THREADS * RS_KPT;
+constexpr int RS_KPT = 14;        // keys per thread of a radix tile: 3584 keys per tile ...
+constexpr int RS_KPT_SMALL = 4;   // ... 1024 for small runs, where a pass is one tile's chain of latencies and most SMs have none
+#ifndef RS_SMALL_N
+#define RS_SMALL_N 300000         // (4 against 14 keys per thread: build -20 % at n = 2^12, -15 % at 2^17, -6 % at 2^18, +17 % at 2^19)
+#endif
+inline int rs_kpt_for(int64_t n) { return n < RS_SMALL_N ? RS_KPT_SMALL : RS_KPT; }
 constexpr int RS_PASSES = 8;      // 8 x 8 bits >= 63 bits
 constexpr int LB_WIN = 16;        // radix look-back: tiles per block = status words requested together
 
@@ -147,6 +151,7 @@ struct Layout {   // byte offsets into the workspace; computed by plan_workspace
     int64_t n, node_cap, group_cap;
     int64_t rs_tiles, node_tiles, sc_tiles, po_tiles;
     int64_t rs_blocks, node_blocks;      // look-back blocks of LB_WIN tiles
+    int rs_kpt;                          // keys per thread of the radix tiles this workspace is planned for (rs_kpt_for(n))
 };
 
 inline int64_t node_capacity(int64_t n) { return 2 * n + 4096; }

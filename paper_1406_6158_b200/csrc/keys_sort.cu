@@ -127,7 +127,7 @@ cudaError_t launch_keys_sort_permute(Ctx *c)
         cudaError_t e = launch_radix_pass<u64>(kin, vin, kout, vout, nullptr, n, nullptr, 8 * pass,
                                                ctl->digit_base + pass * 256,
                                                status + (size_t)pass * (L.rs_tiles + L.rs_blocks) * 256, (u32)L.rs_tiles,
-                                               &ctl->tile_counter[pass], &ctl->status, sgrid, st, c->device);
+                                               &ctl->tile_counter[pass], &ctl->status, sgrid, st, c->device, L.rs_kpt);
         if (e != cudaSuccess) return e;
         kin = kout; vin = vout;
     }

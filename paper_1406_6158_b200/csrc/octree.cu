@@ -622,7 +622,7 @@ cudaError_t launch_build_tree(Ctx *c)
     const int ngrid = (int)imin64(L.node_tiles, (int64_t)c->num_sms * 3);
     e = launch_radix_pass<unsigned char>(pre_level, nullptr, level, pre_of_bfs, bfs_of_pre, 0, &ctl->nn, 0,
                                          ctl->node_base, wsptr<u32>(c, L.node_status), (u32)L.node_tiles, &ctl->tile_counter[10],
-                                         &ctl->status, ngrid, st, c->device);
+                                         &ctl->status, ngrid, st, c->device, L.rs_kpt);
     if (e != cudaSuccess) return e;
 
     u32 *first = wsptr<u32>(c, L.first), *count = wsptr<u32>(c, L.count), *child = wsptr<u32>(c, L.child);

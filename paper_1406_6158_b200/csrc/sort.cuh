@@ -10,9 +10,10 @@ namespace hyb {
 
 constexpr u32 RS_FLAG_AGG = 1u << 30, RS_FLAG_PREFIX = 2u << 30, RS_VALUE_MASK = (1u << 30) - 1;
 
+template <int KPT>
 struct RadixSmem {
-    u64 keys[RS_TILE];
-    u32 vals[RS_TILE];
+    u64 keys[RS_THREADS * KPT];
+    u32 vals[RS_THREADS * KPT];
     u32 warp_cnt[RS_THREADS / 32][256];
     u32 digit_start[256];
     u32 global_off[256];
@@ -23,14 +24,15 @@ struct RadixSmem {
 // n_dev (optional) overrides n with a device-side count (tree nodes).
 // vin == nullptr: values are the global input indices (first pass).
 // inv_out (optional): inv_out[value] = output position (the inverse permutation).
-template <typename KeyT>
+template <typename KeyT, int KPT>
 __global__ void __launch_bounds__(RS_THREADS) radix_pass_kernel(
     const KeyT *__restrict__ kin, const u32 *__restrict__ vin, KeyT *__restrict__ kout, u32 *__restrict__ vout,
     u32 *__restrict__ inv_out, u32 n_host, const u32 *__restrict__ n_dev, int shift,
     const u32 *__restrict__ digit_base, u32 *status, u32 tiles_alloc, u32 *tile_counter, u32 *dev_status, int static_first)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    RadixSmem &sm = *reinterpret_cast<RadixSmem *>(smem_raw);
+    constexpr int RS_KPT = KPT, RS_TILE = RS_THREADS * KPT;      // (shadow the names of the large-run tile)
+    RadixSmem<KPT> &sm = *reinterpret_cast<RadixSmem<KPT> *>(smem_raw);
     pdl_begin();
     const u32 n = n_dev ? *n_dev : n_host;
     const u32 ntiles = (n + RS_TILE - 1) / RS_TILE;
@@ -202,23 +204,36 @@ __global__ void __launch_bounds__(RS_THREADS) radix_pass_kernel(
     }
 }
 
-template <typename KeyT>
-static cudaError_t launch_radix_pass(const KeyT *kin, const u32 *vin, KeyT *kout, u32 *vout, u32 *inv_out, u32 n_host,
-                                     const u32 *n_dev, int shift, const u32 *digit_base, u32 *status, u32 tiles_alloc,
-                                     u32 *tile_counter, u32 *dev_status, int grid, cudaStream_t st, int device)
+template <typename KeyT, int KPT>
+static cudaError_t launch_radix_pass_kpt(const KeyT *kin, const u32 *vin, KeyT *kout, u32 *vout, u32 *inv_out, u32 n_host,
+                                         const u32 *n_dev, int shift, const u32 *digit_base, u32 *status, u32 tiles_alloc,
+                                         u32 *tile_counter, u32 *dev_status, int grid, cudaStream_t st, int device)
 {
     static unsigned long long ready = 0ull;
     if (!device_ready(&ready, device)) {
-        cudaError_t e = cudaFuncSetAttribute(radix_pass_kernel<KeyT>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                             (int)sizeof(RadixSmem));
+        cudaError_t e = cudaFuncSetAttribute(radix_pass_kernel<KeyT, KPT>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                             (int)sizeof(RadixSmem<KPT>));
         if (e != cudaSuccess) return e;
         device_set_ready(&ready, device);
     }
     int sms = 0;
     cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, device);
     const int static_first = grid <= 2 * sms ? 1 : 0;
-    return launch_pdl(radix_pass_kernel<KeyT>, dim3((unsigned)grid), dim3(RS_THREADS), sizeof(RadixSmem), st, kin, vin, kout, vout,
-                      inv_out, n_host, n_dev, shift, digit_base, status, tiles_alloc, tile_counter, dev_status, static_first);
+    return launch_pdl(radix_pass_kernel<KeyT, KPT>, dim3((unsigned)grid), dim3(RS_THREADS), sizeof(RadixSmem<KPT>), st, kin, vin, kout,
+                      vout, inv_out, n_host, n_dev, shift, digit_base, status, tiles_alloc, tile_counter, dev_status, static_first);
+}
+
+// kpt: Layout::rs_kpt (the status arrays were planned for tiles of RS_THREADS x kpt keys)
+template <typename KeyT>
+static cudaError_t launch_radix_pass(const KeyT *kin, const u32 *vin, KeyT *kout, u32 *vout, u32 *inv_out, u32 n_host,
+                                     const u32 *n_dev, int shift, const u32 *digit_base, u32 *status, u32 tiles_alloc,
+                                     u32 *tile_counter, u32 *dev_status, int grid, cudaStream_t st, int device, int kpt)
+{
+    if (kpt == RS_KPT_SMALL)
+        return launch_radix_pass_kpt<KeyT, RS_KPT_SMALL>(kin, vin, kout, vout, inv_out, n_host, n_dev, shift, digit_base, status,
+                                                        tiles_alloc, tile_counter, dev_status, grid, st, device);
+    return launch_radix_pass_kpt<KeyT, RS_KPT>(kin, vin, kout, vout, inv_out, n_host, n_dev, shift, digit_base, status, tiles_alloc,
+                                               tile_counter, dev_status, grid, st, device);
 }
 
 }  // namespace hyb
